@@ -1,0 +1,440 @@
+"""CPU ORACLE (TEST INFRASTRUCTURE, NOT PRODUCT CODE) for the per-time-step MPS
+algebra of the quantics-tensor-train (QTT/MPS) 2D Navier-Stokes solver of
+arxiv 2406.17823 (Hoelscher et al.), written from /root/reference/PAPER.md.
+
+Plain, slow, obviously-correct NumPy fp64.  LAPACK ``qr``/``svd`` and
+``einsum``/``matmul`` are the only library steps.  It shares no code with the
+CUDA path (paper_2406_17823_b200/) and neither imports the other.  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this module.
+
+Data model (Sec. II.B, Eq. 3-4): a field F[x][y] on an N x N
+grid, N = 2**n, becomes an n-site MPS; site k = 1..n carries
+omega_k = 2*x_bit_k + y_bit_k with bit 1 the MOST significant (PAPER.md:59-67
+Eq. 3; "alpha_{m+1} connected to the tensor of the less
+significant bits").  An MPS is a Python list of n arrays ``core[k]`` of shape
+(r_{k-1}, 4, r_k), r_0 = r_n = 1.  An MPO is a list of n arrays of shape
+(D_{k-1}, 4, 4, D_k) indexed [alpha_{k-1}][omega (output)][omega' (input)][alpha_k],
+D_0 = D_n = 1 (boundary vectors L, R of PAPER.md:90-98 Eq. 7 folded into the
+end cores).
+
+Functions and the passage each follows (DESIGN.md "Readings" lists every point
+where the paper is silent/garbled and the reading taken):
+
+  O1  encode / decode           PAPER.md:59-67  Eq. 3 (quantics bit interleave)
+  O2  from_dense                PAPER.md:67-72  Eq. 4; R->L TT-SVD (ref. [15])
+  O3  apply_mpo                 PAPER.md:85     "act on them by contracting the respective indices"
+  O4  hadamard                  PAPER.md:100-105 Eq. 8, Fig. 2(a) (bond chi^2)
+  O5  lincomb / axpy            PAPER.md:126-130 Eq. 11 (sum of RK4 pieces)
+  O6  round                     PAPER.md:130 ("compression ... repeated SVDs"), ref. [15];
+                                eps semantics PAPER.md:238 Eq. 16
+  O7  round_product (zip-up)    PAPER.md:105 ("needs to be compressed down to chi again");
+                                the chi^2 product is never formed
+  O8  rhs                       PAPER.md:49-53 Eq. 2 without pressure (Burgers form)
+  O9  rk4_step                  PAPER.md:124-128 Eq. 11
+  O10 mpo_d1 / mpo_d2 / mpo_laplacian   PAPER.md:391-424 App. A, Eq. A1-A3, Table II
+
+Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
+grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
+analytic finite-difference of sin/cos, bond-2 closed forms, the root-sum-square
+truncation identity, norm preservation, dense TT-SVD, dense RK4 of the same
+stencils.
+
+Parity-pin status: O1-O6, O8-O10 pinned.  O7 is pinned where chi_work >= every
+intermediate rank (then it equals O6 applied to O4, checked against dense brute
+force) and by its error bound; for a finite chi_work that really truncates, the
+result is DEFINED by the step-by-step algorithm below (the paper gives none) --
+"parity unpinned" for that regime beyond the error bound.
+"""
+from __future__ import annotations
+
+import math
+import numpy as np
+
+D_PHYS = 4  # physical dimension d = 2^k for a k-dimensional grid, k = 2
+
+
+# --------------------------------------------------------------------------- O1
+def encode(F: np.ndarray) -> np.ndarray:
+    """Dense F[x][y] (N x N) -> tensor U[w_1]...[w_n], w_k = 2*x_bit_k + y_bit_k,
+    bit 1 most significant (Eq. 3)."""
+    N = F.shape[0]
+    n = int(round(math.log2(N)))
+    assert F.shape == (N, N) and (1 << n) == N
+    T = np.asarray(F, dtype=np.float64).reshape((2,) * n + (2,) * n)  # x bits msb..lsb, y bits msb..lsb
+    perm = []
+    for k in range(n):
+        perm += [k, n + k]
+    return T.transpose(perm).reshape((D_PHYS,) * n)
+
+
+def decode(U: np.ndarray) -> np.ndarray:
+    """Inverse of :func:`encode`."""
+    n = U.ndim
+    N = 1 << n
+    T = U.reshape((2, 2) * n)  # x1 y1 x2 y2 ...
+    perm = [2 * k for k in range(n)] + [2 * k + 1 for k in range(n)]
+    return T.transpose(perm).reshape(N, N)
+
+
+# ---------------------------------------------------------------- rank rule (O6)
+def _rank_rule(s: np.ndarray, chi_max: int, delta) -> int:
+    """Kept rank r' for singular values s (descending).
+
+    eps = 0 (delta is None): r' = min(chi_max, len(s))  (static shapes, no thresholding).
+    eps > 0: smallest r with sqrt(sum_{i>r} s_i^2) <= delta, then
+    r' <- max(1, min(r, chi_max)).  (reading 6; eps is the total
+    relative error of PAPER.md:238 Eq. 16, split evenly over the n-1 bonds.)
+    """
+    m = len(s)
+    if delta is None:
+        return max(1, min(int(chi_max), m))
+    tail = np.sqrt(np.cumsum((s[::-1]) ** 2))[::-1]  # tail[r] = sqrt(sum_{i>=r} s_i^2)
+    r = m
+    for cand in range(m + 1):
+        t = tail[cand] if cand < m else 0.0
+        if t <= delta:
+            r = cand
+            break
+    return max(1, min(r, int(chi_max), m))
+
+
+# --------------------------------------------------------------------------- O2
+def from_dense(F: np.ndarray, chi_max: int = 1 << 30, eps: float = 0.0):
+    """TT-SVD proceeding right-to-left (Eq. 4; reading 9):
+    for k = n..2, SVD the 4^{k-1} x (4 r_k) unfolding, keep r by the rank rule,
+    core_k = V^T, carry U S; core_1 = carry."""
+    U = encode(F)
+    n = U.ndim
+    nrm = float(np.linalg.norm(U))
+    delta = eps * nrm / math.sqrt(max(n - 1, 1)) if eps > 0 else None
+    cores = [None] * n
+    carry = U.reshape(-1, 1)  # (4^n) x r_n, r_n = 1
+    r = 1
+    for k in range(n, 1, -1):
+        M = carry.reshape(D_PHYS ** (k - 1), D_PHYS * r)
+        Um, s, Vt = np.linalg.svd(M, full_matrices=False)
+        rk = _rank_rule(s, chi_max, delta)
+        cores[k - 1] = Vt[:rk].reshape(rk, D_PHYS, r)
+        carry = Um[:, :rk] * s[:rk]
+        r = rk
+    cores[0] = carry.reshape(1, D_PHYS, r)
+    return cores
+
+
+def to_tensor(cores) -> np.ndarray:
+    """Contract an MPS to the full tensor U[w_1..w_n] (Eq. 4)."""
+    T = cores[0].reshape(D_PHYS, -1)
+    for c in cores[1:]:
+        r0, d, r1 = c.shape
+        T = (T @ c.reshape(r0, d * r1)).reshape(-1, r1)
+    return T.reshape((D_PHYS,) * len(cores))
+
+
+def to_dense(cores) -> np.ndarray:
+    """MPS -> dense F[x][y]."""
+    return decode(to_tensor(cores))
+
+
+def bonds(cores):
+    return [1] + [c.shape[2] for c in cores]
+
+
+# --------------------------------------------------------------------------- O3
+def apply_mpo(W, A):
+    """B[(alpha,a), w, (beta,b)] = sum_{w'} W[alpha, w, w', beta] * A[a, w', b]
+    (MPO bond index major).  Exact, bond D*chi."""
+    out = []
+    for Wk, Ak in zip(W, A):
+        Dl, d, _, Dr = Wk.shape
+        a, _, b = Ak.shape
+        B = np.einsum("xopy,apb->xaoyb", Wk, Ak)
+        out.append(B.reshape(Dl * a, d, Dr * b))
+    return out
+
+
+# --------------------------------------------------------------------------- O4
+def hadamard(A, B):
+    """C[(a,b), w, (a',b')] = A[a,w,a'] * B[b,w,b'] (Eq. 8:
+    |u_i> (.) as an MPO with rank-3 Kronecker deltas; bond chi_a*chi_b)."""
+    out = []
+    for Ak, Bk in zip(A, B):
+        a, d, a2 = Ak.shape
+        b, _, b2 = Bk.shape
+        C = np.einsum("awc,bwd->abwcd", Ak, Bk)
+        out.append(C.reshape(a * b, d, a2 * b2))
+    return out
+
+
+# --------------------------------------------------------------------------- O5
+def lincomb(terms):
+    """sum_j alpha_j |X_j> as an MPS by direct sum: first core
+    [alpha_1 X_1 | alpha_2 X_2 | ...], middle cores block-diagonal, last cores
+    stacked.  ``terms`` = [(alpha, cores), ...].  The scalar sits on the first core."""
+    n = len(terms[0][1])
+    k = len(terms)
+    out = []
+    for site in range(n):
+        cs = [t[1][site] for t in terms]
+        if site == 0:
+            out.append(np.concatenate([t[0] * c for t, c in zip(terms, cs)], axis=2))
+        elif site == n - 1:
+            out.append(np.concatenate(cs, axis=0))
+        else:
+            rl = sum(c.shape[0] for c in cs)
+            rr = sum(c.shape[2] for c in cs)
+            blk = np.zeros((rl, D_PHYS, rr))
+            i = j = 0
+            for c in cs:
+                blk[i : i + c.shape[0], :, j : j + c.shape[2]] = c
+                i += c.shape[0]
+                j += c.shape[2]
+            out.append(blk)
+    assert k >= 1
+    return out
+
+
+def axpy(alpha, X, Y):
+    """alpha*X + Y (exact)."""
+    return lincomb([(alpha, X), (1.0, Y)])
+
+
+# --------------------------------------------------------------------------- O6
+def _sweep_lr(cores):
+    """(i) L->R: thin QR of each left unfolding, R into the next core."""
+    cores = [c.copy() for c in cores]
+    n = len(cores)
+    for k in range(n - 1):
+        r0, d, r1 = cores[k].shape
+        Q, R = np.linalg.qr(cores[k].reshape(r0 * d, r1))  # reduced
+        rq = Q.shape[1]
+        cores[k] = Q.reshape(r0, d, rq)
+        nr0, _, nr1 = cores[k + 1].shape
+        cores[k + 1] = (R @ cores[k + 1].reshape(nr0, d * nr1)).reshape(rq, d, nr1)
+    return cores
+
+
+def _sweep_rl(cores, chi_max, eps, info=None):
+    """(ii) R->L for k = n..2: SVD of the right unfolding; rank rule; core_k <- V^T[:r'],
+    left neighbour <- left * (U[:, :r'] S[:r']).  ``cores`` must be left-orthogonal
+    up to the last site, so ||A||_F = ||last core||."""
+    n = len(cores)
+    nrm = float(np.linalg.norm(cores[-1]))
+    delta = eps * nrm / math.sqrt(max(n - 1, 1)) if eps > 0 else None
+    if info is not None:
+        info["norm"] = nrm
+        info["singular_values"] = [None] * (n + 1)
+        info["discarded"] = [0.0] * (n + 1)
+    for k in range(n - 1, 0, -1):
+        r0, d, r1 = cores[k].shape
+        U, s, Vt = np.linalg.svd(cores[k].reshape(r0, d * r1), full_matrices=False)
+        rk = _rank_rule(s, chi_max, delta)
+        cores[k] = Vt[:rk].reshape(rk, d, r1)
+        US = U[:, :rk] * s[:rk]
+        p0, _, _ = cores[k - 1].shape
+        cores[k - 1] = (cores[k - 1].reshape(p0 * d, r0) @ US).reshape(p0, d, rk)
+        if info is not None:
+            info["singular_values"][k] = s.copy()
+            info["discarded"][k] = float(np.sqrt(np.sum(s[rk:] ** 2)))
+    return cores
+
+
+def round_mps(cores, chi_max: int = 1 << 30, eps: float = 0.0, info=None):
+    """TT-rounding (ref. [15] of the paper).  Never normalises; a zero
+    MPS stays zero.  Output is right-canonical (norm on site 1)."""
+    return _sweep_rl(_sweep_lr(cores), chi_max, eps, info)
+
+
+# --------------------------------------------------------------------------- O7
+def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None):
+    """Fused Hadamard + round ("zip-up" with working bond chi_work; reading 8).
+
+    carry R_0 = [1]; for l = 1..n-1:
+        T = contract(R, A_l, B_l) as (4 r) x (a' b');
+        if 4r <= min(a'b', chi_work):            Q = I,  R' = T
+        elif a'b' < 4r and a'b' <= chi_work:     thin QR
+        else:                                    truncated SVD keeping the chi_work largest
+                                                 (Q = U, R' = S V^T)
+        core_l = Q.
+    Last site: core_n = contract(R, A_n, B_n).  Then step (ii) of O6 with (chi_max, eps).
+    Default chi_work = 2*chi_max.  With chi_work >= every intermediate rank this IS
+    round_mps(hadamard(A, B))."""
+    if chi_work is None:
+        chi_work = 2 * int(chi_max)
+    n = len(A)
+    R = np.ones((1, 1, 1))
+    cores = []
+    for l in range(n - 1):
+        T4 = np.einsum("rab,awc,bwd->rwcd", R, A[l], B[l], optimize=True)
+        r, d, a2, b2 = T4.shape
+        T = T4.reshape(r * d, a2 * b2)
+        m, k = T.shape
+        if m <= min(k, chi_work):
+            Q = np.eye(m)
+            Rn = T
+        elif k < m and k <= chi_work:
+            Q, Rn = np.linalg.qr(T)
+        else:
+            U, s, Vt = np.linalg.svd(T, full_matrices=False)
+            keep = min(chi_work, len(s))
+            Q = U[:, :keep]
+            Rn = s[:keep, None] * Vt[:keep]
+        rn = Q.shape[1]
+        cores.append(Q.reshape(r, d, rn))
+        R = Rn.reshape(rn, a2, b2)
+    T4 = np.einsum("rab,awc,bwd->rwcd", R, A[n - 1], B[n - 1], optimize=True)
+    cores.append(T4.reshape(T4.shape[0], D_PHYS, 1))
+    return _sweep_rl(cores, chi_max, eps, info)
+
+
+# -------------------------------------------------------------------------- O10
+# Table II of the paper, verbatim: (alpha_m, alpha_{m+1}, omega, omega') -> 1.
+# C_{alpha_m alpha_{m+1}}^{omega omega'}.  omega = (x_m y_m)_2.
+_TABLE_II = [
+    (0, 0, 0, 0), (0, 0, 1, 1), (0, 0, 2, 2), (0, 0, 3, 3),   # alpha_{m+1} = 0: x +- 0
+    (0, 1, 0, 2), (0, 1, 1, 3), (1, 1, 2, 0), (1, 1, 3, 1),   # alpha_{m+1} = 1: x + 1
+    (2, 2, 0, 2), (2, 2, 1, 3), (0, 2, 2, 0), (0, 2, 3, 1),   # alpha_{m+1} = 2: x - 1
+]
+
+
+def _swap_bits(w: int) -> int:
+    """Exchange the x and y bit of omega = (x y)_2."""
+    return ((w & 1) << 1) | (w >> 1)
+
+
+def shift_core(direction: int) -> np.ndarray:
+    """Central core C[alpha_m][omega][omega'][alpha_{m+1}] of Table II, with omega the
+    OUTPUT (row) index and omega' the index contracted with the MPS (reading 1:
+    the literal text "output index omega'" yields -D, since D^T = -D).
+    direction 1: shifts in x (Table II verbatim); direction 2: the same table with
+    the roles of the x and y bit exchanged ("same logic")."""
+    C = np.zeros((3, D_PHYS, D_PHYS, 3))
+    for am, am1, w, wp in _TABLE_II:
+        if direction == 2:
+            w, wp = _swap_bits(w), _swap_bits(wp)
+        C[am, w, wp, am1] = 1.0
+    return C
+
+
+def _fold_boundaries(core_list, L, R):
+    out = [c.copy() for c in core_list]
+    out[0] = np.einsum("x,xopy->opy", L, out[0])[None]
+    out[-1] = np.einsum("xopy,y->xop", out[-1], R)[..., None]
+    return out
+
+
+def mpo_d1(n: int, dx: float):
+    """Central-difference MPO D_1 (PAPER.md:395-404 Eq. A1-A3): L = (1,1,1) on the
+    most-significant end, R = (0, 1, -1)/(2 dx) on the least-significant end."""
+    C = shift_core(1)
+    return _fold_boundaries([C] * n, np.ones(3), np.array([0.0, 1.0, -1.0]) / (2.0 * dx))
+
+
+def mpo_d2(n: int, dx: float):
+    """Same for the y direction."""
+    C = shift_core(2)
+    return _fold_boundaries([C] * n, np.ones(3), np.array([0.0, 1.0, -1.0]) / (2.0 * dx))
+
+
+def mpo_laplacian(n: int, dx: float):
+    """Compact 5-point Laplacian MPO, bond 5 (reading 3; not printed in the paper):
+    channel 0 = identity, channels 1,2 = the alpha=1,2 entries of Table II for the
+    x bit, channels 3,4 = the same for the y bit; L = (1,1,1,1,1),
+    R = (-4, 1, 1, 1, 1)/dx^2."""
+    C = np.zeros((5, D_PHYS, D_PHYS, 5))
+    Cx, Cy = shift_core(1), shift_core(2)
+    C[0, :, :, 0] = Cx[0, :, :, 0]  # identity channel
+    for src, base in ((Cx, 0), (Cy, 2)):
+        for a in (1, 2):
+            C[0, :, :, base + a] = src[0, :, :, a]       # start a shift, no carry out
+            C[base + a, :, :, base + a] = src[a, :, :, a]  # shift with carry out
+    return _fold_boundaries([C] * n, np.ones(5), np.array([-4.0, 1.0, 1.0, 1.0, 1.0]) / dx**2)
+
+
+def mpo_to_dense(W) -> np.ndarray:
+    """Dense 4^n x 4^n matrix of an MPO in the (w_1..w_n) ordering (rows = output)."""
+    M = W[0][0]  # (4,4,D)
+    for Wk in W[1:]:
+        M = np.einsum("opx,xqry->oqpry", M, Wk)
+        o, q, p, r, y = M.shape
+        M = M.reshape(o * q, p * r, y)
+    return M[:, :, 0]
+
+
+# --------------------------------------------------------------------------- O8
+def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None):
+    """f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i, i = 1,2 (PAPER.md:49-53
+    Eq. 2 without the pressure term; convective form, reading 4), with one rounding
+    after every apply, product and sum (reading 7)."""
+    Dj = (Dx, Dy)
+    f = []
+    for i in range(2):
+        g = [round_mps(apply_mpo(Dj[j], u[i]), chi_max, eps) for j in range(2)]
+        lap = round_mps(apply_mpo(Lap, u[i]), chi_max, eps)
+        c = [round_product(u[j], g[j], chi_max, eps, chi_work) for j in range(2)]
+        f.append(round_mps(lincomb([(-1.0, c[0]), (-1.0, c[1]), (1.0 / Re, lap)]), chi_max, eps))
+    return f
+
+
+# --------------------------------------------------------------------------- O9
+def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None):
+    """Classical RK4 (Eq. 11) on the MPS pair u = [u_1, u_2]; all
+    roundings with the same (chi_max, eps); final combination as one 5-term sum
+    and one rounding (reading 10)."""
+    def stage(k, h):
+        return [round_mps(lincomb([(1.0, u[i]), (h, k[i])]), chi_max, eps) for i in range(2)]
+
+    k1 = rhs(u, Dx, Dy, Lap, Re, chi_max, eps, chi_work)
+    k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
+    k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
+    k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
+    return [
+        round_mps(
+            lincomb([(1.0, u[i]), (dt / 6, k1[i]), (dt / 3, k2[i]), (dt / 3, k3[i]), (dt / 6, k4[i])]),
+            chi_max, eps)
+        for i in range(2)
+    ]
+
+
+# ------------------------------------------------------------ harness utilities
+def norm(cores) -> float:
+    return math.sqrt(max(dot(cores, cores), 0.0))
+
+
+def dot(A, B) -> float:
+    """<A|B> by transfer matrices."""
+    E = np.ones((1, 1))
+    for a, b in zip(A, B):
+        E = np.einsum("xy,xwa,ywb->ab", E, a, b, optimize=True)
+    return float(E[0, 0])
+
+
+def diff_norm(A, B) -> float:
+    """||A - B||_F without cancellation: norm of the exact difference MPS obtained
+    from a QR sweep (reading 19)."""
+    D = _sweep_lr(lincomb([(1.0, A), (-1.0, B)]))
+    return float(np.linalg.norm(D[-1]))
+
+
+def schmidt_values(cores):
+    """Singular values at every bond 1..n-1 (Eq. 16-17): SVD of the
+    centre matrix while sweeping the orthogonality centre right-to-left."""
+    C = _sweep_lr(cores)
+    n = len(C)
+    out = [None] * (n + 1)
+    for k in range(n - 1, 0, -1):
+        r0, d, r1 = C[k].shape
+        U, s, Vt = np.linalg.svd(C[k].reshape(r0, d * r1), full_matrices=False)
+        out[k] = s
+        C[k] = Vt.reshape(len(s), d, r1)
+        p0 = C[k - 1].shape[0]
+        C[k - 1] = (C[k - 1].reshape(p0 * d, r0) @ (U * s)).reshape(p0, d, len(s))
+    return out
+
+
+def canonical_random(raw_cores):
+    """BASELINE config 5: left-canonicalise raw random cores and scale the last
+    core to unit norm."""
+    C = _sweep_lr(raw_cores)
+    C[-1] = C[-1] / np.linalg.norm(C[-1])
+    return C
