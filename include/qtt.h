@@ -1,0 +1,129 @@
+/* qtt.h -- C ABI of the B200-native QTT/MPS time-step algebra (arxiv 2406.17823, Hoelscher et al.).
+ *
+ * The library implements the per-time-step matrix-product-state (MPS) algebra of the paper's
+ * quantics-tensor-train Navier-Stokes solver on ONE GPU, in fp64, with hand-written sm_100a kernels.
+ * Citations are to /root/reference/PAPER.md (line, section / equation); DESIGN.md lists the readings
+ * taken where the paper is silent.
+ *
+ * Data model (Sec. II.B, Eq. 3-4).  A field F[x][y] on an N x N periodic grid,
+ * N = 2^n, x_j = y_j = j/N, is an n-site MPS.  Site k = 1..n carries the physical index
+ * w_k = 2*x_bit_k + y_bit_k (d = 4) with bit 1 the MOST significant.  A site tensor ("core") is a dense
+ * row-major array  core_k[r_{k-1}][4][r_k]  of doubles in device memory, r_0 = r_n = 1.  An MPO is a list
+ * of n arrays  W_k[D_{k-1}][4 (output w)][4 (input w')][D_k], D_0 = D_n = 1 (Eq. 7 with the
+ * boundary vectors L, R folded into the end cores).
+ *
+ * Conventions.
+ *  - Handles (qtt_ctx, qtt_mps, qtt_mpo) are opaque, created by the library and released by the caller
+ *    with the matching *_free / *_destroy.  A handle belongs to the context that created it.
+ *  - Device memory comes ONLY from the caller's alloc/release callbacks (the Python binding hands out
+ *    torch-owned memory): one workspace of `workspace_bytes` at qtt_ctx_create and one block per MPS.
+ *  - All work is enqueued on the caller's CUDA stream given at qtt_ctx_create.  With eps == 0 every call
+ *    that takes only device data is asynchronous (static shapes: rank = min(chi_max, rows, cols));
+ *    with eps > 0 the rank of each bond is read back, i.e. ONE stream synchronisation per bond.
+ *  - Every function returns a qtt_status; on error outputs are untouched and qtt_last_error() gives text.
+ *    There is NO CPU fallback: without a usable CUDA device qtt_ctx_create fails with QTT_CUDA.
+ *  - "dev" pointers are device pointers, "host" pointers are host pointers.
+ *  - Lazy results.  qtt_apply_mpo, qtt_hadamard and qtt_axpy return / produce handles that DENOTE the
+ *    exact result (bond D*chi, chi_a*chi_b, chi_x+chi_y) and keep references to their operands; nothing
+ *    is computed until qtt_round (fused sweeps; the chi^2 bond of a product is never formed),
+ *    qtt_to_dense / qtt_mps_get_core (materialise, bounded by the materialisation limit ->
+ *    QTT_CAPACITY) or qtt_mps_dot.
+ *  - Gauge is not part of the contract.  qtt_round / qtt_mps_from_dense return right-canonical cores
+ *    (norm on site 1); compare only gauge-invariant quantities (dense field, norms, Schmidt values).
+ */
+#ifndef QTT_B200_H
+#define QTT_B200_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qtt_ctx qtt_ctx;
+typedef struct qtt_mps qtt_mps;
+typedef struct qtt_mpo qtt_mpo;
+typedef int qtt_status;
+#define QTT_OK 0
+#define QTT_INVALID_ARG (-1)
+#define QTT_SHAPE_MISMATCH (-2)
+#define QTT_CAPACITY (-3) /* workspace / materialisation limit exceeded */
+#define QTT_CUDA (-4)     /* CUDA error, text in qtt_last_error */
+#define QTT_NUMERIC (-5)  /* Jacobi sweep limit hit */
+
+typedef void* (*qtt_alloc_fn)(size_t bytes, void* user); /* returns a device pointer, 256-byte aligned, or NULL */
+typedef void (*qtt_release_fn)(void* dev_ptr, void* user);
+
+/* Create a context on CUDA device `device`, enqueueing on `cuda_stream` (a cudaStream_t; NULL = legacy
+ * default stream).  `workspace_bytes` of scratch are taken once through `alloc`. */
+qtt_status qtt_ctx_create(qtt_ctx** out, int device, void* cuda_stream, qtt_alloc_fn alloc, qtt_release_fn release,
+                          void* user, size_t workspace_bytes);
+void qtt_ctx_destroy(qtt_ctx* ctx);
+const char* qtt_last_error(const qtt_ctx* ctx);
+/* Working bond chi_work of the fused Hadamard+round ("zip-up", reading 8); 0 = 2*chi_max. */
+qtt_status qtt_ctx_set_chi_work(qtt_ctx* ctx, int chi_work);
+/* Largest lazy result (bytes of all cores) that qtt_to_dense / qtt_mps_get_core may materialise. */
+qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes);
+/* 1: qtt_rk4_step with eps == 0 is captured once into a CUDA graph per shape signature and replayed
+ * (default); 0: launches are issued eagerly every step. */
+qtt_status qtt_ctx_set_graphs(qtt_ctx* ctx, int enabled);
+/* Synchronises the stream and reports the Jacobi convergence record since the last call:
+ * the largest number of sweeps any SVD used, and how many SVDs hit the sweep limit (then QTT_NUMERIC). */
+qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits);
+/* Number of kernels launched (or graph nodes replayed) by this context so far. */
+long long qtt_ctx_launch_count(const qtt_ctx* ctx);
+
+/* PAPER.md:67-72 Eq. 4 (reading 9): right-to-left TT-SVD of the dense field dense_dev[x*N + y], N = 2^n_bits,
+ * keeping per bond r = rank rule(chi_max, eps) (see qtt_round). */
+qtt_status qtt_mps_from_dense(qtt_ctx* ctx, const double* dense_dev, int n_bits, int chi_max, double eps,
+                              qtt_mps** out);
+/* Upload explicit cores (host arrays, core k is bonds[k] x 4 x bonds[k+1] row-major, bonds has n+1 entries). */
+qtt_status qtt_mps_from_cores(qtt_ctx* ctx, int n_sites, const int* bonds, const double* const* cores_host,
+                              qtt_mps** out);
+/* PAPER.md:69 Eq. 4: contract the MPS and undo the bit interleave; dense_dev_out holds N*N doubles. */
+qtt_status qtt_to_dense(qtt_ctx* ctx, const qtt_mps* x, double* dense_dev_out);
+
+/* MPO from host cores W_k[D_{k-1}][4 out][4 in][D_k] (Eq. 7, App. A Table II); bonds has n+1
+ * entries with both ends 1. */
+qtt_status qtt_mpo_create(qtt_ctx* ctx, int n_sites, const int* bonds, const double* const* cores_host,
+                          qtt_mpo** out);
+void qtt_mpo_free(qtt_mpo* w);
+
+/* y = W x, exact, bond D*chi, composite bond index = alpha*chi + a (lazy). */
+qtt_status qtt_apply_mpo(qtt_ctx* ctx, const qtt_mpo* w, const qtt_mps* x, qtt_mps** y);
+/* PAPER.md:100-105 Eq. 8: c = a (.) b element-wise, exact, bond chi_a*chi_b (lazy, never formed by qtt_round). */
+qtt_status qtt_hadamard(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, qtt_mps** c);
+/* PAPER.md:126-130 Eq. 11: y <- alpha*x + y, exact, direct sum of the bonds (lazy; sums nest flat). */
+qtt_status qtt_axpy(qtt_ctx* ctx, double alpha, const qtt_mps* x, qtt_mps* y);
+/* PAPER.md:130 ("compression ... repeated SVDs"), ref. [15]; eps semantics PAPER.md:238 Eq. 16.
+ * Left-to-right orthogonalisation, then right-to-left truncated SVD, in place on the handle.
+ * Rank rule per bond: eps == 0: r' = min(chi_max, rows, cols) of the unfolding (static shapes);
+ * eps > 0: smallest r with sqrt(sum_{i>r} sigma_i^2) <= eps*||x||_F/sqrt(n-1), clamped to [1, chi_max].
+ * A product handle is rounded by the zip-up (reading 8) with working bond chi_work. */
+qtt_status qtt_round(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps);
+/* The same for `batch` independent operands in single launches per site. */
+qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_max, double eps);
+/* PAPER.md:124-128 Eq. 11 on u = (u_1, u_2), in place: classical RK4 of
+ * f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i   (Eq. 2 without pressure),
+ * one rounding after every apply, product and sum (readings 4, 5, 7, 10). */
+qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, const qtt_mpo* Dy, const qtt_mpo* Lap,
+                        double Re, double dt, int chi_max, double eps);
+
+/* Inspection. */
+int qtt_mps_num_sites(const qtt_mps* x);
+qtt_status qtt_mps_bonds(const qtt_mps* x, int* bonds_out /* n+1 */);
+/* Copy core k (0-based) to host_out (bonds[k]*4*bonds[k+1] doubles); materialises lazy handles. Synchronous. */
+qtt_status qtt_mps_get_core(qtt_ctx* ctx, const qtt_mps* x, int k, double* host_out);
+/* <a|b> by transfer matrices; result written to *out_host after a stream synchronisation. */
+qtt_status qtt_mps_dot(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, double* out_host);
+/* ||x||_F from an orthogonalisation sweep (no cancellation); synchronous. */
+qtt_status qtt_mps_norm(qtt_ctx* ctx, const qtt_mps* x, double* out_host);
+/* Schmidt values of every bond 1..n-1 (Eq. 16-17): sigma_host[bond*cap + i], counts[bond];
+ * entries beyond counts[bond] are untouched.  Synchronous. */
+qtt_status qtt_mps_schmidt(qtt_ctx* ctx, const qtt_mps* x, double* sigma_host, int cap, int* counts /* n+1 */);
+qtt_status qtt_mps_clone(qtt_ctx* ctx, const qtt_mps* x, qtt_mps** out);
+void qtt_mps_free(qtt_mps* x);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,41 @@
+/* qtt_diag.h -- kernel-level diagnostic entry points of libqtt_b200 (tests, profiling, peak probes).
+ * Plain device pointers, no handles.  All return 0 on success or a cudaError_t value.  `stream` is a
+ * cudaStream_t.  These run the SAME kernels the qtt_* calls of qtt.h are built from. */
+#ifndef QTT_B200_DIAG_H
+#define QTT_B200_DIAG_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* C = alpha * op(A) * op(B) + beta * C, row-major, strided batch; op = transpose if trans* != 0.
+ * A is M x K (lda) or, transposed, stored K x M (lda); B likewise; C is M x N (ldc).
+ * SURVEY.md section 8 row a2 (site contractions on the fp64 tensor pipe). */
+int qtt_diag_gemm(void* stream, const double* A_dev, const double* B_dev, double* C_dev, int M, int N, int K,
+                  int transA, int transB, long long lda, long long ldb, long long ldc, double alpha, double beta,
+                  int nbatch, long long strideA, long long strideB, long long strideC);
+
+/* Q-less LQ of `batch` matrices Y_i (k x m, k <= m <= 16384, leading dimension ld, consecutive with stride
+ * k*ld, DESTROYED); R_i = L_i^T (k x k upper triangular, row-major, consecutive) with Y = L Q.
+ * scratch_dev: batch * 2 * 16 * m doubles.  SURVEY.md section 8 row a4. */
+int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, double* R_dev, double* scratch_dev);
+
+/* One-sided Jacobi on the rows of `batch` matrices X_i (p x q, ld, stride p*ld), in place: rows of the result
+ * are mutually orthogonal (X = J^T Sigma V^T).  status_dev: 2 ints (zero them first): [0] <- max sweeps,
+ * [1] += matrices that hit the sweep limit.  SURVEY.md section 8 row a5. */
+int qtt_diag_rowjacobi(void* stream, double* X_dev, int batch, int p, int q, int ld, int* status_dev);
+
+/* Sort rows by norm, apply the rank rule (delta < 0: r = min(chi_max, p, q); else smallest r whose discarded
+ * tail is <= delta, clamped to [1, chi_max]), write sigma (p), rank (1 int) and the normalised top rows
+ * (r_cap x q) to out_dev. */
+int qtt_diag_select(void* stream, const double* X_dev, int p, int q, int ld, double* out_dev, int r_cap,
+                    double* sigma_dev, int* rank_dev, int chi_max, double delta);
+
+/* fp64 issue-rate probes: kind 0 = register-only DMMA.8x8x4 loop, kind 1 = register-only DFMA loop, on
+ * `ctas` CTAs of 256 threads, `iters` iterations of 64 independent instructions per warp / thread chain set.
+ * *tflops_out <- achieved TFLOP/s (host pointer).  Synchronous. */
+int qtt_diag_fp64_probe(void* stream, int kind, int ctas, int iters, double* tflops_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,138 @@
+// Host-side engine behind the qtt_* C ABI: handles, the two-ended workspace stack, and the batched
+// sweeps that sequence the kernels of common.cuh.  Everything here only ENQUEUES work on the context's
+// stream; with eps == 0 no call synchronises, so a whole RK4 step can be stream-captured.
+#pragma once
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "../../include/qtt.h"
+#include "common.cuh"
+
+struct QttError {
+  int status;
+  std::string msg;
+};
+#define QTT_THROW(st, m) throw QttError{(st), std::string(m)}
+#define QTT_CU(expr)                                                                                   \
+  do {                                                                                                 \
+    cudaError_t _e = (expr);                                                                           \
+    if (_e != cudaSuccess)                                                                             \
+      throw QttError{QTT_CUDA, std::string(#expr) + ": " + cudaGetErrorString(_e)};                    \
+  } while (0)
+
+// Workspace: "keep" stack grows from the bottom (results that outlive one rounding), "tmp" stack grows
+// from the top (scratch of one rounding level).
+struct Arena {
+  char* base = nullptr;
+  size_t size = 0, lo = 0, hi = 0;
+  double* keep(size_t doubles);
+  double* tmp(size_t doubles);
+};
+
+// An MPS with explicit dense cores in device memory: core[k] is r[k] x 4 x r[k+1], row-major.
+struct View {
+  int n = 0;
+  std::vector<int> r;
+  std::vector<const double*> core;
+};
+
+struct MpoData {
+  int refs = 1;
+  qtt_ctx* ctx = nullptr;
+  int n = 0;
+  std::vector<int> D;
+  double* storage = nullptr;
+  std::vector<const double*> core;
+};
+
+enum BodyKind { BODY_DENSE = 0, BODY_APPLIED = 1, BODY_PRODUCT = 2, BODY_SUM = 3 };
+struct Body {
+  int refs = 1;
+  qtt_ctx* ctx = nullptr;
+  int kind = BODY_DENSE;
+  int n = 0;
+  std::vector<int> r;
+  // DENSE
+  double* storage = nullptr;
+  size_t storage_doubles = 0;
+  bool tight = false;  // cores packed back to back in storage with exactly the bonds r
+  std::vector<double*> core;
+  // lazy kinds
+  MpoData* mpo = nullptr;
+  Body* x = nullptr;
+  Body *a = nullptr, *b = nullptr;
+  std::vector<std::pair<double, Body*>> terms;
+};
+
+struct qtt_mps {
+  qtt_ctx* ctx;
+  Body* body;
+};
+struct qtt_mpo {
+  MpoData* data;
+};
+
+struct Rk4Plan;
+
+struct qtt_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  qtt_alloc_fn alloc = nullptr;
+  qtt_release_fn release = nullptr;
+  void* user = nullptr;
+  Arena arena;
+  std::string err;
+  int chi_work = 0;
+  size_t mat_limit = (size_t)2 << 30;
+  int graphs = 1;
+  double* ones = nullptr;   // device: 1.0
+  int* jac_status = nullptr;  // device: [max sweeps, limit hits]
+  long long graph_launches = 0;
+  std::vector<Rk4Plan*> plans;
+};
+
+// Output of a rounding: cores are written into caller-provided slots sized for the capacity bonds.
+struct OutMps {
+  int n = 0;
+  std::vector<int> rcap;  // capacity bonds (= exact bonds when eps == 0)
+  std::vector<int> r;     // actual bonds, filled by the sweep
+  std::vector<double*> core;
+};
+
+// static (eps == 0) bonds of round(dense MPS with bonds r, chi)
+std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi);
+// working bonds of the zip-up and static bonds of its result
+void qtt_zip_caps(const std::vector<int>& ra, const std::vector<int>& rb, int chi, int chi_work,
+                  std::vector<int>& rwork, std::vector<int>& rout);
+
+struct SigmaCapture {
+  // per item, per bond k (1..n-1): device pointer to the singular values (count[k] of them)
+  std::vector<std::vector<double*>> sigma;
+  std::vector<std::vector<int>> count;
+};
+
+// Oracle O6 on a batch of dense MPS (same n).  out[i].core slots must be allocated by the caller.
+void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, double eps, std::vector<OutMps>& out,
+                           SigmaCapture* cap = nullptr);
+// Oracle O7 on a batch of pairs (A, B).
+void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std::vector<View>& B, int chi, double eps,
+                             int chi_work, std::vector<OutMps>& out);
+
+// exact lazy results materialised as dense cores in the tmp stack
+View qtt_expand_apply(qtt_ctx* ctx, const MpoData* W, const View& x);
+void qtt_expand_apply_batch(qtt_ctx* ctx, const std::vector<const MpoData*>& W, const std::vector<View>& x,
+                            std::vector<View>& out);
+void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double, View>>>& terms,
+                      std::vector<View>& out);
+View qtt_kron(qtt_ctx* ctx, const View& a, const View& b);
+
+void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
+                   double dt, int chi, double eps, int chi_work, OutMps out[2]);
+
+void qtt_to_dense_view(qtt_ctx* ctx, const View& v, double* dense_dev_out);
+void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, double eps, OutMps& out);
+double* qtt_dot_view(qtt_ctx* ctx, const View& a, const View& b);  // device scalar in tmp
+
+
+

@@ -1,0 +1,237 @@
+// Bandwidth-bound data movement of the QTT step (SURVEY.md section 8 rows a1, a3 and the boundary):
+// MPO x MPS site expand, direct-sum concatenation, Hadamard (Kronecker) site tensors, the quantics
+// bit interleave, transposes and copies.  All grid-stride, coalesced along the innermost index.
+#include "common.cuh"
+
+namespace {
+
+constexpr int NT = 256;
+
+inline int grid_for(i64 n) {
+  i64 b = (n + NT - 1) / NT;
+  const i64 cap = 148 * 16;
+  return (int)(b < 1 ? 1 : (b > cap ? cap : b));
+}
+
+// out[(al,a), w, (be,b)] = sum_w' W[al,w,w',be] * A[a,w',b]      (MPO bond index major)
+__global__ void qtt_expand_kernel(const __grid_constant__ ExpandGroup g) {
+  const ExpandProb& P = g.p[blockIdx.y];
+  const int Dl = P.Dl, Dr = P.Dr, a = P.a, b = P.b;
+  const i64 n = (i64)Dl * a * 4 * Dr * b;
+  const i64 rowlen = (i64)Dr * b;
+  for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
+    i64 t = idx;
+    int bb = (int)(t % b); t /= b;
+    int be = (int)(t % Dr); t /= Dr;
+    int w = (int)(t % 4); t /= 4;
+    int aa = (int)(t % a);
+    int al = (int)(t / a);
+    double s = 0.0;
+#pragma unroll
+    for (int wp = 0; wp < 4; ++wp) {
+      double wv = P.W[((al * 4 + w) * 4 + wp) * Dr + be];
+      if (wv != 0.0) s += wv * P.A[((i64)aa * 4 + wp) * b + bb];
+    }
+    P.out[idx] = s;
+    (void)rowlen;
+  }
+}
+
+__global__ void qtt_concat_kernel(const __grid_constant__ ConcatGroup g) {
+  const ConcatProb& P = g.p[blockIdx.y];
+  int RL = 0, RR = 0;
+  if (P.mode == 0) {
+    RL = P.rl[0];
+    for (int t = 0; t < P.nterm; ++t) RR += P.rr[t];
+  } else if (P.mode == 2) {
+    RR = P.rr[0];
+    for (int t = 0; t < P.nterm; ++t) RL += P.rl[t];
+  } else {
+    for (int t = 0; t < P.nterm; ++t) {
+      RL += P.rl[t];
+      RR += P.rr[t];
+    }
+  }
+  const i64 n = (i64)RL * 4 * RR;
+  for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
+    int c = (int)(idx % RR);
+    i64 t2 = idx / RR;
+    int w = (int)(t2 % 4);
+    int r = (int)(t2 / 4);
+    // locate the term of the row and of the column
+    int tr = 0, tc = 0, r_in = r, c_in = c;
+    if (P.mode != 0) {
+      while (tr < P.nterm - 1 && r_in >= P.rl[tr]) { r_in -= P.rl[tr]; ++tr; }
+    }
+    if (P.mode != 2) {
+      while (tc < P.nterm - 1 && c_in >= P.rr[tc]) { c_in -= P.rr[tc]; ++tc; }
+    }
+    double v = 0.0;
+    if (P.mode == 0) {
+      v = P.alpha[tc] * P.src[tc][((i64)r * 4 + w) * P.rr[tc] + c_in];
+    } else if (P.mode == 2) {
+      v = P.src[tr][((i64)r_in * 4 + w) * P.rr[tr] + c];
+    } else if (tr == tc) {
+      v = P.src[tr][((i64)r_in * 4 + w) * P.rr[tr] + c_in];
+    }
+    P.out[idx] = v;
+  }
+}
+
+// out[(a,b), w, (a2,b2)] = A[a,w,a2] * B[b,w,b2]                  (Eq. 8)
+__global__ void qtt_kron_kernel(const __grid_constant__ KronGroup g) {
+  const KronProb& P = g.p[blockIdx.y];
+  const i64 n = (i64)P.a * P.b * 4 * P.a2 * P.b2;
+  for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
+    i64 t = idx;
+    int bb2 = (int)(t % P.b2); t /= P.b2;
+    int aa2 = (int)(t % P.a2); t /= P.a2;
+    int w = (int)(t % 4); t /= 4;
+    int bb = (int)(t % P.b);
+    int aa = (int)(t / P.b);
+    P.out[idx] = P.A[((i64)aa * 4 + w) * P.a2 + aa2] * P.B[((i64)bb * 4 + w) * P.b2 + bb2];
+  }
+}
+
+// Quantics interleave (Eq. 3): tensor index t = (w_1 ... w_n)_4, w_k = 2 x_k + y_k, bit 1
+// most significant;  dense index = x * N + y.
+__device__ __forceinline__ unsigned compact_even_bits(unsigned long long v) {
+  // gathers bits 0,2,4,... of v
+  v &= 0x5555555555555555ull;
+  v = (v | (v >> 1)) & 0x3333333333333333ull;
+  v = (v | (v >> 2)) & 0x0f0f0f0f0f0f0f0full;
+  v = (v | (v >> 4)) & 0x00ff00ff00ff00ffull;
+  v = (v | (v >> 8)) & 0x0000ffff0000ffffull;
+  v = (v | (v >> 16)) & 0x00000000ffffffffull;
+  return (unsigned)v;
+}
+__global__ void qtt_interleave_kernel(const double* __restrict__ src, double* __restrict__ dst, int nbits,
+                                      int inverse) {
+  const i64 n = 1ll << (2 * nbits);
+  for (i64 t = (i64)blockIdx.x * NT + threadIdx.x; t < n; t += (i64)gridDim.x * NT) {
+    unsigned y = compact_even_bits((unsigned long long)t);
+    unsigned x = compact_even_bits((unsigned long long)t >> 1);
+    i64 d = ((i64)x << nbits) | y;
+    if (inverse)
+      dst[d] = src[t];  // tensor -> dense
+    else
+      dst[t] = src[d];  // dense -> tensor
+  }
+}
+
+__global__ void qtt_transpose_kernel(const double* __restrict__ src, int rows, int cols, int lds,
+                                     double* __restrict__ dst, int ldd) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.y * 32, by = blockIdx.x * 32;  // x runs over row blocks (the long direction)
+  for (int j = threadIdx.y; j < 32; j += 8) {
+    int r = by + j, c = bx + threadIdx.x;
+    if (r < rows && c < cols) tile[j][threadIdx.x] = src[(i64)r * lds + c];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += 8) {
+    int c = bx + j, r = by + threadIdx.x;  // dst row = c, dst col = r
+    if (r < rows && c < cols) dst[(i64)c * ldd + r] = tile[threadIdx.x][j];
+  }
+}
+
+__global__ void qtt_copy2d_kernel(const double* __restrict__ src, int rows, int cols, int lds,
+                                  double* __restrict__ dst, int ldd) {
+  const i64 n = (i64)rows * cols;
+  for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
+    int r = (int)(idx / cols), c = (int)(idx - (i64)r * cols);
+    dst[(i64)r * ldd + c] = src[(i64)r * lds + c];
+  }
+}
+
+__global__ void qtt_fill_kernel(double* dst, i64 n, double v) {
+  for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) dst[idx] = v;
+}
+
+}  // namespace
+
+cudaError_t qtt_launch_expand(const ExpandProb* probs, int n, cudaStream_t stream) {
+  for (int b0 = 0; b0 < n; b0 += QTT_MOVE_MAX_BATCH) {
+    ExpandGroup g;
+    g.nprob = n - b0 < QTT_MOVE_MAX_BATCH ? n - b0 : QTT_MOVE_MAX_BATCH;
+    i64 mx = 1;
+    for (int i = 0; i < g.nprob; ++i) {
+      g.p[i] = probs[b0 + i];
+      i64 sz = (i64)g.p[i].Dl * g.p[i].a * 4 * g.p[i].Dr * g.p[i].b;
+      mx = sz > mx ? sz : mx;
+    }
+    qtt_expand_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    ++g_qtt_launch_count;
+    QTT_CHECK_CUDA(cudaGetLastError());
+  }
+  return cudaSuccess;
+}
+
+cudaError_t qtt_launch_concat(const ConcatProb* probs, int n, cudaStream_t stream) {
+  for (int b0 = 0; b0 < n; b0 += QTT_MOVE_MAX_BATCH) {
+    ConcatGroup g;
+    g.nprob = n - b0 < QTT_MOVE_MAX_BATCH ? n - b0 : QTT_MOVE_MAX_BATCH;
+    i64 mx = 1;
+    for (int i = 0; i < g.nprob; ++i) {
+      g.p[i] = probs[b0 + i];
+      i64 RL = 0, RR = 0;
+      for (int t = 0; t < g.p[i].nterm; ++t) {
+        RL += g.p[i].rl[t];
+        RR += g.p[i].rr[t];
+      }
+      i64 sz = RL * 4 * RR;
+      mx = sz > mx ? sz : mx;
+    }
+    qtt_concat_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    ++g_qtt_launch_count;
+    QTT_CHECK_CUDA(cudaGetLastError());
+  }
+  return cudaSuccess;
+}
+
+cudaError_t qtt_launch_kron(const KronProb* probs, int n, cudaStream_t stream) {
+  for (int b0 = 0; b0 < n; b0 += QTT_MOVE_MAX_BATCH) {
+    KronGroup g;
+    g.nprob = n - b0 < QTT_MOVE_MAX_BATCH ? n - b0 : QTT_MOVE_MAX_BATCH;
+    i64 mx = 1;
+    for (int i = 0; i < g.nprob; ++i) {
+      g.p[i] = probs[b0 + i];
+      i64 sz = (i64)g.p[i].a * g.p[i].b * 4 * g.p[i].a2 * g.p[i].b2;
+      mx = sz > mx ? sz : mx;
+    }
+    qtt_kron_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    ++g_qtt_launch_count;
+    QTT_CHECK_CUDA(cudaGetLastError());
+  }
+  return cudaSuccess;
+}
+
+cudaError_t qtt_launch_interleave(const double* src, double* dst, int nbits, int inverse, cudaStream_t stream) {
+  qtt_interleave_kernel<<<grid_for(1ll << (2 * nbits)), NT, 0, stream>>>(src, dst, nbits, inverse);
+  ++g_qtt_launch_count;
+  return cudaGetLastError();
+}
+
+cudaError_t qtt_launch_transpose(const double* src, int rows, int cols, int lds, double* dst, int ldd,
+                                 cudaStream_t stream) {
+  if (rows <= 0 || cols <= 0) return cudaSuccess;
+  dim3 grid((rows + 31) / 32, (cols + 31) / 32);
+  if (grid.y > 65535) return cudaErrorInvalidValue;
+  qtt_transpose_kernel<<<grid, dim3(32, 8), 0, stream>>>(src, rows, cols, lds, dst, ldd);
+  ++g_qtt_launch_count;
+  return cudaGetLastError();
+}
+
+cudaError_t qtt_launch_copy2d(const double* src, int rows, int cols, int lds, double* dst, int ldd,
+                              cudaStream_t stream) {
+  if (rows <= 0 || cols <= 0) return cudaSuccess;
+  qtt_copy2d_kernel<<<grid_for((i64)rows * cols), NT, 0, stream>>>(src, rows, cols, lds, dst, ldd);
+  ++g_qtt_launch_count;
+  return cudaGetLastError();
+}
+
+cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t stream) {
+  if (n <= 0) return cudaSuccess;
+  qtt_fill_kernel<<<grid_for(n), NT, 0, stream>>>(dst, n, value);
+  ++g_qtt_launch_count;
+  return cudaGetLastError();
+}

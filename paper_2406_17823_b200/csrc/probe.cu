@@ -1,0 +1,85 @@
+// fp64 issue-rate probes (include/qtt_diag.h: qtt_diag_fp64_probe) -- the measured denominators of the
+// fp64 roofline (MEASURED_PEAKS.json carries no fp64 figure), and the one-time
+// kernel attribute setup.
+#include <cstdio>
+
+#include "../../include/qtt_diag.h"
+#include "common.cuh"
+
+namespace {
+
+// 16 independent DMMA.8x8x4 accumulator pairs per warp, 4 rounds per iteration = 64 DMMA per warp-iteration
+__global__ void __launch_bounds__(256) qtt_probe_dmma_kernel(int iters, double* sink) {
+  double d0[16], d1[16];
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) d0[i] = d1[i] = (double)i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int i = 0; i < 16; ++i)
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                     : "+d"(d0[i]), "+d"(d1[i])
+                     : "d"(a), "d"(b));
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += d0[i] + d1[i];
+  if (s == 123.456) sink[0] = s;
+}
+
+// 16 independent DFMA chains per thread, 4 rounds per iteration = 64 DFMA per thread-iteration
+__global__ void __launch_bounds__(256) qtt_probe_dfma_kernel(int iters, double* sink) {
+  double d[16];
+  double a = 1.0 + threadIdx.x * 1e-12, b = 1e-9 * threadIdx.x;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) d[i] = (double)i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int i = 0; i < 16; ++i) d[i] = fma(d[i], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += d[i];
+  if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace
+
+long long g_qtt_launch_count = 0;
+
+void qtt_kernels_init() {}
+
+extern "C" int qtt_diag_fp64_probe(void* stream, int kind, int ctas, int iters, double* tflops_out) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (ctas < 1 || iters < 1 || !tflops_out) return (int)cudaErrorInvalidValue;
+  double* sink = nullptr;
+  QTT_CHECK_CUDA(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t e0, e1;
+  QTT_CHECK_CUDA(cudaEventCreate(&e0));
+  QTT_CHECK_CUDA(cudaEventCreate(&e1));
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {  // first repetition is the warm-up
+    QTT_CHECK_CUDA(cudaEventRecord(e0, st));
+    if (kind == 0)
+      qtt_probe_dmma_kernel<<<ctas, 256, 0, st>>>(iters, sink);
+    else
+      qtt_probe_dfma_kernel<<<ctas, 256, 0, st>>>(iters, sink);
+    QTT_CHECK_CUDA(cudaGetLastError());
+    QTT_CHECK_CUDA(cudaEventRecord(e1, st));
+    QTT_CHECK_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    QTT_CHECK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    if (rep > 0 && ms < best) best = ms;
+  }
+  // DMMA.8x8x4: 8*8*4*2 = 512 flop per warp instruction; DFMA: 2 flop per thread instruction
+  const double per_cta_iter = (kind == 0) ? 8.0 * 64.0 * 512.0 : 256.0 * 64.0 * 2.0;
+  *tflops_out = per_cta_iter * (double)ctas * (double)iters / ((double)best * 1e-3) * 1e-12;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  return 0;
+}

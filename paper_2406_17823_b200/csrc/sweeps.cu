@@ -1,0 +1,876 @@
+// Batched rounding sweeps of the QTT step, sequencing the kernels of
+// common.cuh.  The rounding is "Q-less": the L->R sweep keeps only the triangular factors R_k of the left
+// blocks, and the R->L sweep works in the original gauge with R_{k-1} as the metric,
+//     M = R_{k-1} (A_k C_k),  rows of J M = Sigma V^T,  core'_k = V^T[:r'],  C_{k-1} = (A_k C_k) V[:, :r'],
+// which is the same truncation as oracle O6 (QR sweep, then truncated SVDs) without ever forming a Q.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "engine.cuh"
+
+
+
+// ------------------------------------------------------------------------------------------ arena
+double* Arena::keep(size_t doubles) {
+  size_t bytes = (doubles * sizeof(double) + 255) & ~(size_t)255;
+  if (lo + bytes > hi) QTT_THROW(QTT_CAPACITY, "workspace exhausted (keep stack)");
+  double* p = reinterpret_cast<double*>(base + lo);
+  lo += bytes;
+  return p;
+}
+double* Arena::tmp(size_t doubles) {
+  size_t bytes = (doubles * sizeof(double) + 255) & ~(size_t)255;
+  if (bytes > hi || hi - bytes < lo) QTT_THROW(QTT_CAPACITY, "workspace exhausted (tmp stack)");
+  hi -= bytes;
+  return reinterpret_cast<double*>(base + hi);
+}
+
+// ------------------------------------------------------------------------------------------ shapes
+std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi) {
+  const int n = (int)r.size() - 1;
+  std::vector<int> p(n + 1), out(n + 1);
+  p[0] = 1;
+  for (int k = 1; k <= n; ++k) p[k] = std::min(4 * p[k - 1], r[k]);
+  out[n] = 1;
+  for (int k = n - 1; k >= 1; --k) out[k] = std::max(1, std::min(chi, std::min(p[k], 4 * out[k + 1])));
+  out[0] = 1;
+  return out;
+}
+
+void qtt_zip_caps(const std::vector<int>& ra, const std::vector<int>& rb, int chi, int chi_work,
+                  std::vector<int>& rwork, std::vector<int>& rout) {
+  const int n = (int)ra.size() - 1;
+  rwork.assign(n + 1, 1);
+  for (int k = 1; k < n; ++k) {
+    long long kk = (long long)ra[k] * rb[k];
+    long long m = 4ll * rwork[k - 1];
+    rwork[k] = (int)std::min<long long>(std::min(m, kk), chi_work);
+  }
+  rout.assign(n + 1, 1);
+  for (int k = n - 1; k >= 1; --k) rout[k] = std::max(1, std::min(chi, std::min(rwork[k], 4 * rout[k + 1])));
+}
+
+// ------------------------------------------------------------------------------------------ helpers
+namespace {
+
+GemmProb gemm_base(const double* A, const double* B, double* C, int M, int N, int K) {
+  GemmProb p;
+  std::memset(&p, 0, sizeof(p));
+  p.A = A; p.B = B; p.C = C;
+  p.M = M; p.N = N; p.K = K;
+  p.nbatch = 1;
+  p.alpha = 1.0; p.beta = 0.0;
+  return p;
+}
+// plain row-major C(MxN, ldc) = A(MxK, lda) * B(KxN, ldb)
+GemmProb gemm_nn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_base(A, B, C, M, N, K);
+  p.a_lo = lda; p.a_k = 1;
+  p.b_k = ldb; p.b_n = 1;
+  p.c_lo = ldc; p.c_n = 1;
+  return p;
+}
+// C = A * B^T with B stored N x K (ldb)
+GemmProb gemm_nt(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_nn(A, lda, B, 0, C, ldc, M, N, K);
+  p.b_k = 1; p.b_n = ldb;
+  return p;
+}
+// C = A^T * B with A stored K x M (lda)
+GemmProb gemm_tn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_nn(A, 0, B, ldb, C, ldc, M, N, K);
+  p.a_lo = 1; p.a_k = lda;
+  return p;
+}
+
+void run_gemms(qtt_ctx* ctx, std::vector<GemmProb>& v) {
+  if (v.empty()) return;
+  QTT_CU(qtt_launch_gemm(v.data(), (int)v.size(), ctx->stream));
+  v.clear();
+}
+
+constexpr int LQ_MAX_M = 16384;
+constexpr int LQ_CHUNK = 8192;
+
+struct LqJob {
+  double* Y;  // k x m, ld, destroyed
+  int k, m, ld;
+  double* R;  // k x k upper triangular out (ld = k)
+};
+
+// Q-less LQ of a batch; very wide matrices go through a TSQR tree over column chunks.
+void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
+  if (jobs.empty()) return;
+  std::vector<LqProb> probs;
+  std::vector<TriProb> tris;
+  std::vector<LqJob> next;  // second-level jobs of the TSQR tree
+  for (const LqJob& j : jobs) {
+    if (j.k > j.m) QTT_THROW(QTT_INVALID_ARG, "internal: LQ needs k <= m");
+    if (j.m <= LQ_MAX_M) {
+      LqProb p;
+      p.Y = j.Y; p.k = j.k; p.m = j.m; p.ld = j.ld;
+      p.V = p.TV = nullptr;
+      probs.push_back(p);
+      tris.push_back(TriProb{j.Y, j.k, j.ld, j.R, j.k});
+    } else {
+      const int chunk = std::max(LQ_CHUNK, j.k);
+      const int nch = (j.m + chunk - 1) / chunk;
+      // [L_1 | L_2 | ...] with the last chunk possibly narrower than k (then it is copied as it is)
+      std::vector<int> widths;
+      int total = 0;
+      for (int c = 0; c < nch; ++c) {
+        int mc = std::min(chunk, j.m - c * chunk);
+        widths.push_back(mc);
+        total += std::min(mc, j.k);
+      }
+      double* stack = ctx->arena.tmp((size_t)j.k * total);
+      int off = 0;
+      for (int c = 0; c < nch; ++c) {
+        int mc = widths[c];
+        double* Yc = j.Y + (size_t)c * chunk;
+        if (mc >= j.k) {
+          LqProb p;
+          p.Y = Yc; p.k = j.k; p.m = mc; p.ld = j.ld;
+          p.V = p.TV = nullptr;
+          probs.push_back(p);
+          tris.push_back(TriProb{Yc, j.k, j.ld, stack + off, total});  // mode 1 below
+          off += j.k;
+        } else {
+          QTT_CU(qtt_launch_copy2d(Yc, j.k, mc, j.ld, stack + off, total, ctx->stream));
+          off += mc;
+        }
+      }
+      next.push_back(LqJob{stack, j.k, total, total, j.R});
+    }
+  }
+  // reflector scratch: the launcher runs consecutive groups of QTT_LQ_MAX_BATCH problems one after the
+  // other on the stream, so problem i can share the scratch slot i % QTT_LQ_MAX_BATCH
+  {
+    int mmax = 0;
+    for (const LqProb& p : probs) mmax = std::max(mmax, p.m);
+    const int nslot = std::min<int>((int)probs.size(), QTT_LQ_MAX_BATCH);
+    std::vector<double*> slotV(nslot), slotTV(nslot);
+    for (int s2 = 0; s2 < nslot; ++s2) {
+      slotV[s2] = ctx->arena.tmp(qtt_lq_scratch_doubles(mmax));
+      slotTV[s2] = ctx->arena.tmp(qtt_lq_scratch_doubles(mmax));
+    }
+    for (size_t i = 0; i < probs.size(); ++i) {
+      probs[i].V = slotV[i % QTT_LQ_MAX_BATCH];
+      probs[i].TV = slotTV[i % QTT_LQ_MAX_BATCH];
+    }
+  }
+  // direct problems and chunk problems share the panel launches; their triangles are extracted separately
+  if (!probs.empty()) QTT_CU(qtt_launch_lq(probs.data(), (int)probs.size(), ctx->stream));
+  std::vector<TriProb> t0, t1;
+  {
+    size_t ti = 0;
+    for (const LqJob& j : jobs) {
+      if (j.m <= LQ_MAX_M) {
+        t0.push_back(tris[ti++]);
+      } else {
+        const int chunk = std::max(LQ_CHUNK, j.k);
+        const int nch = (j.m + chunk - 1) / chunk;
+        for (int c = 0; c < nch; ++c)
+          if (std::min(chunk, j.m - c * chunk) >= j.k) t1.push_back(tris[ti++]);
+      }
+    }
+  }
+  if (!t0.empty()) QTT_CU(qtt_launch_extract_tri(t0.data(), (int)t0.size(), 0, ctx->stream));
+  if (!t1.empty()) QTT_CU(qtt_launch_extract_tri(t1.data(), (int)t1.size(), 1, ctx->stream));
+  jobs.clear();
+  if (!next.empty()) run_lq(ctx, next);
+}
+
+struct SvdJob {
+  double* X;  // p x q (ld = q), destroyed: rows orthogonalised in place
+  int p, q;
+  double* out;  // r_cap x q
+  int r_cap, chi_max;
+  double* sigma;  // p doubles or nullptr
+  int* rank;      // device int
+  const double* delta_ptr;
+  double* delta_out;
+  double delta_scale;
+};
+
+// right singular vectors by row-Jacobi; tall inputs are first reduced to their triangular factor
+void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
+  if (jobs.empty()) return;
+  std::vector<LqJob> lq;
+  for (SvdJob& j : jobs) {
+    if (j.p > j.q && j.p >= 8) {
+      // X = Q R_X, same right singular vectors: R_X (q x q) from the LQ of X^T (q x p)
+      double* Xt = ctx->arena.tmp((size_t)j.q * j.p);
+      QTT_CU(qtt_launch_transpose(j.X, j.p, j.q, j.q, Xt, j.p, ctx->stream));
+      double* R = ctx->arena.tmp((size_t)j.q * j.q);
+      lq.push_back(LqJob{Xt, j.q, j.p, j.p, R});
+      j.X = R;
+      j.p = j.q;
+    }
+  }
+  run_lq(ctx, lq);
+  std::vector<JacProb> jp;
+  std::vector<SelProb> sp;
+  for (const SvdJob& j : jobs) {
+    JacProb a;
+    a.X = j.X; a.p = j.p; a.q = j.q; a.ld = j.q; a.status = ctx->jac_status;
+    jp.push_back(a);
+    SelProb s;
+    s.X = j.X; s.p = j.p; s.q = j.q; s.ld = j.q;
+    s.out = j.out; s.out_ld = j.q; s.r_cap = j.r_cap;
+    s.sigma = j.sigma; s.rank = j.rank;
+    s.delta_ptr = j.delta_ptr; s.delta_out = j.delta_out; s.delta_scale = j.delta_scale;
+    s.chi_max = j.chi_max;
+    sp.push_back(s);
+  }
+  QTT_CU(qtt_launch_rowjacobi(jp.data(), (int)jp.size(), ctx->stream));
+  QTT_CU(qtt_launch_select(sp.data(), (int)sp.size(), ctx->stream));
+  jobs.clear();
+}
+
+// one site tensor seen from the R->L sweep
+struct LeftCore {
+  const double* ptr;
+  int rl, rr;
+  int form;  // 0: dense [rl][4][rr]; 1: transposed isometry Qt [rr][4*rl]; 2: identity (rr == 4*rl)
+};
+struct SweepItem {
+  int n;
+  std::vector<LeftCore> core;
+  std::vector<const double*> Rf;  // bond k = 1..n-1: metric factor (pk[k] x core[k].rl), nullptr = identity
+  std::vector<int> pk;
+};
+
+// R->L truncated-SVD sweep (oracle O6 step ii) for a batch.
+void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, std::vector<OutMps>& out,
+              SigmaCapture* cap) {
+  const int nb = (int)items.size();
+  const int n = items[0].n;
+  std::vector<const double*> C(nb, ctx->ones);
+  std::vector<int> rc(nb, 1);
+  std::vector<double*> delta(nb, nullptr);
+  std::vector<int*> rank_dev(nb, nullptr);
+  std::vector<int> rank_host(nb, 0);
+  std::vector<double*> Cbuf[2];
+  Cbuf[0].assign(nb, nullptr);
+  Cbuf[1].assign(nb, nullptr);
+  for (int i = 0; i < nb; ++i) {
+    out[i].r.assign(n + 1, 1);
+    if (eps > 0.0) delta[i] = ctx->arena.tmp(1);
+    rank_dev[i] = reinterpret_cast<int*>(ctx->arena.tmp(1));
+    size_t mx = 1;
+    for (int k = 1; k < n; ++k) mx = std::max(mx, (size_t)items[i].core[k].rl * out[i].rcap[k]);
+    Cbuf[0][i] = ctx->arena.tmp(mx);
+    Cbuf[1][i] = ctx->arena.tmp(mx);
+  }
+  std::vector<GemmProb> g;
+  for (int k = n - 1; k >= 1; --k) {
+    const size_t site_mark = ctx->arena.hi;
+    std::vector<const double*> B(nb);
+    std::vector<SvdJob> svd;
+    std::vector<GemmProb> g2;
+    // B = core_k * C   (r_k x 4 rc)
+    for (int i = 0; i < nb; ++i) {
+      const LeftCore& c = items[i].core[k];
+      const int q = 4 * rc[i];
+      if (c.form == 2) {
+        B[i] = C[i];
+      } else if (c.rr == 1 && rc[i] == 1 && C[i] == ctx->ones) {
+        B[i] = c.ptr;
+      } else {
+        double* Bb = ctx->arena.tmp((size_t)c.rl * q);
+        if (c.form == 0)
+          g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], Bb, rc[i], 4 * c.rl, rc[i], c.rr));
+        else
+          g.push_back(gemm_tn(c.ptr, 4 * c.rl, C[i], rc[i], Bb, rc[i], 4 * c.rl, rc[i], c.rr));
+        B[i] = Bb;
+      }
+    }
+    run_gemms(ctx, g);
+    // M = R_{k} * B  (pk x 4 rc), or a copy of B when the left block is an isometry
+    for (int i = 0; i < nb; ++i) {
+      const LeftCore& c = items[i].core[k];
+      const int q = 4 * rc[i];
+      const int p = items[i].Rf[k] ? items[i].pk[k] : c.rl;
+      double* Mb = ctx->arena.tmp((size_t)p * q);
+      if (items[i].Rf[k])
+        g.push_back(gemm_nn(items[i].Rf[k], c.rl, B[i], q, Mb, q, p, q, c.rl));
+      else
+        QTT_CU(qtt_launch_copy2d(B[i], p, q, q, Mb, q, ctx->stream));
+      SvdJob j;
+      j.X = Mb; j.p = p; j.q = q;
+      j.out = out[i].core[k];
+      j.r_cap = out[i].rcap[k];
+      j.chi_max = std::min(chi, out[i].rcap[k]);
+      j.sigma = nullptr;
+      if (cap) {
+        j.sigma = ctx->arena.keep((size_t)p);
+        cap->sigma[i][k] = j.sigma;
+        cap->count[i][k] = std::min(p, q);
+      }
+      j.rank = rank_dev[i];
+      j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
+      if (eps > 0.0) {
+        if (k == n - 1) {
+          j.delta_out = delta[i];
+          j.delta_scale = eps / std::sqrt((double)std::max(n - 1, 1));
+        } else {
+          j.delta_ptr = delta[i];
+        }
+      }
+      svd.push_back(j);
+    }
+    run_gemms(ctx, g);
+    run_svd(ctx, svd);
+    // ranks
+    for (int i = 0; i < nb; ++i) {
+      const LeftCore& c = items[i].core[k];
+      const int p = items[i].Rf[k] ? items[i].pk[k] : c.rl;
+      rank_host[i] = std::max(1, std::min(std::min(chi, out[i].rcap[k]), std::min(p, 4 * rc[i])));
+    }
+    if (eps > 0.0) {
+      for (int i = 0; i < nb; ++i)
+        QTT_CU(cudaMemcpyAsync(&rank_host[i], rank_dev[i], sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+      QTT_CU(cudaStreamSynchronize(ctx->stream));
+    }
+    // C_{k} <- B * core'^T   (r_k x r')
+    for (int i = 0; i < nb; ++i) {
+      const LeftCore& c = items[i].core[k];
+      const int q = 4 * rc[i];
+      const int rn = rank_host[i];
+      double* Cn = Cbuf[k & 1][i];
+      g2.push_back(gemm_nt(B[i], q, out[i].core[k], q, Cn, rn, c.rl, rn, q));
+      out[i].r[k] = rn;
+      C[i] = Cn;
+      rc[i] = rn;
+    }
+    run_gemms(ctx, g2);
+    ctx->arena.hi = site_mark;
+  }
+  // first site: core'_0 = core_0 * C  (4 x rc)
+  for (int i = 0; i < nb; ++i) {
+    const LeftCore& c = items[i].core[0];
+    if (c.form == 2)
+      QTT_CU(qtt_launch_copy2d(C[i], 4, rc[i], rc[i], out[i].core[0], rc[i], ctx->stream));
+    else if (c.form == 0)
+      g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], out[i].core[0], rc[i], 4 * c.rl, rc[i], c.rr));
+    else
+      g.push_back(gemm_tn(c.ptr, 4 * c.rl, C[i], rc[i], out[i].core[0], rc[i], 4 * c.rl, rc[i], c.rr));
+  }
+  run_gemms(ctx, g);
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------ O6
+void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, double eps, std::vector<OutMps>& out,
+                           SigmaCapture* cap) {
+  const int nb = (int)in.size();
+  if (nb == 0) return;
+  const int n = in[0].n;
+  for (const View& v : in)
+    if (v.n != n) QTT_THROW(QTT_SHAPE_MISMATCH, "batched rounding needs operands with the same number of sites");
+  if (cap) {
+    cap->sigma.assign(nb, std::vector<double*>(n + 1, nullptr));
+    cap->count.assign(nb, std::vector<int>(n + 1, 0));
+  }
+  if (n == 1) {
+    for (int i = 0; i < nb; ++i) {
+      QTT_CU(qtt_launch_copy2d(in[i].core[0], 1, 4, 4, out[i].core[0], 4, ctx->stream));
+      out[i].r.assign(2, 1);
+    }
+    return;
+  }
+  std::vector<SweepItem> items(nb);
+  for (int i = 0; i < nb; ++i) {
+    SweepItem& it = items[i];
+    it.n = n;
+    it.core.resize(n);
+    for (int k = 0; k < n; ++k) it.core[k] = LeftCore{in[i].core[k], in[i].r[k], in[i].r[k + 1], 0};
+    it.Rf.assign(n + 1, nullptr);
+    it.pk.assign(n + 1, 1);
+    it.Rf[0] = ctx->ones;
+  }
+  // ---- L->R: metric factors R_k of the left blocks (oracle O6 step i, without forming Q)
+  std::vector<GemmProb> g;
+  for (int k = 0; k < n - 1; ++k) {
+    std::vector<LqJob> lq;
+    // persistent factors first, scratch after the mark
+    std::vector<double*> Rnew(nb, nullptr);
+    for (int i = 0; i < nb; ++i) {
+      SweepItem& it = items[i];
+      const int r1 = in[i].r[k + 1];
+      const int rows = 4 * it.pk[k], cols = r1;
+      if (rows <= cols) {
+        if (k > 0) Rnew[i] = ctx->arena.tmp((size_t)rows * cols);
+      } else {
+        Rnew[i] = ctx->arena.tmp((size_t)cols * cols);
+      }
+    }
+    const size_t site_mark = ctx->arena.hi;
+    for (int i = 0; i < nb; ++i) {
+      SweepItem& it = items[i];
+      const int rk = in[i].r[k], r1 = in[i].r[k + 1];
+      const int pk = it.pk[k];
+      const int rows = 4 * pk, cols = r1;
+      if (rows <= cols) {
+        if (k == 0) {
+          it.Rf[1] = in[i].core[0];
+        } else {
+          g.push_back(gemm_nn(it.Rf[k], rk, in[i].core[k], 4 * (i64)r1, Rnew[i], 4 * (i64)r1, pk, 4 * r1, rk));
+          it.Rf[k + 1] = Rnew[i];
+        }
+        it.pk[k + 1] = rows;
+      } else {
+        // Y = X^T (cols x rows), written transposed by the GEMM:  Y[b][(i,w)] = sum_a core[a,w,b] R[i,a]
+        double* Y = ctx->arena.tmp((size_t)cols * rows);
+        GemmProb p = gemm_base(in[i].core[k], it.Rf[k], Y, r1, pk, rk);
+        p.nbatch = 4;
+        p.a_lo = 1; p.a_k = 4 * (i64)r1; p.a_bs = r1;
+        p.b_k = 1; p.b_n = rk; p.b_bs = 0;
+        p.c_lo = 4 * (i64)pk; p.c_n = 4; p.c_bs = 1;
+        g.push_back(p);
+        lq.push_back(LqJob{Y, cols, rows, rows, Rnew[i]});
+        it.Rf[k + 1] = Rnew[i];
+        it.pk[k + 1] = cols;
+      }
+    }
+    run_gemms(ctx, g);
+    run_lq(ctx, lq);
+    ctx->arena.hi = site_mark;
+  }
+  sweep_rl(ctx, items, chi, eps, out, cap);
+}
+
+// ------------------------------------------------------------------------------------------ O7
+void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std::vector<View>& B, int chi, double eps,
+                             int chi_work, std::vector<OutMps>& out) {
+  const int nb = (int)A.size();
+  if (nb == 0) return;
+  const int n = A[0].n;
+  for (int i = 0; i < nb; ++i)
+    if (A[i].n != n || B[i].n != n) QTT_THROW(QTT_SHAPE_MISMATCH, "product operands differ in length");
+  std::vector<SweepItem> items(nb);
+  std::vector<const double*> R(nb, ctx->ones);
+  std::vector<int> r(nb, 1);
+  std::vector<double*> Rbuf[2];
+  Rbuf[0].assign(nb, nullptr);
+  Rbuf[1].assign(nb, nullptr);
+  for (int i = 0; i < nb; ++i) {
+    items[i].n = n;
+    items[i].core.resize(n);
+    items[i].Rf.assign(n + 1, nullptr);
+    items[i].pk.assign(n + 1, 1);
+    // carry R_l (rwork[l] x a_l b_l) ping-pongs between two buffers of the largest size
+    std::vector<int> rw, ro;
+    qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro);
+    size_t mx = 1;
+    for (int l = 1; l < n; ++l) mx = std::max(mx, (size_t)rw[l] * A[i].r[l] * B[i].r[l]);
+    Rbuf[0][i] = ctx->arena.tmp(mx);
+    Rbuf[1][i] = ctx->arena.tmp(mx);
+  }
+  std::vector<GemmProb> g;
+  for (int l = 0; l < n; ++l) {
+    const size_t site_mark = ctx->arena.hi;
+    std::vector<double*> T(nb);
+    // X[i,(w,a'),b] = sum_a A[a,(w,a')] R[i,a,b]      (first half of the site contraction, row a2)
+    std::vector<double*> X(nb);
+    for (int i = 0; i < nb; ++i) {
+      const int a = A[i].r[l], a2 = A[i].r[l + 1], b = B[i].r[l];
+      X[i] = ctx->arena.tmp((size_t)r[i] * 4 * a2 * b);
+      GemmProb p = gemm_base(A[i].core[l], R[i], X[i], 4 * a2, b, a);
+      p.nbatch = r[i];
+      p.a_lo = 1; p.a_k = 4 * (i64)a2; p.a_bs = 0;
+      p.b_k = b; p.b_n = 1; p.b_bs = (i64)a * b;
+      p.c_lo = b; p.c_n = 1; p.c_bs = 4 * (i64)a2 * b;
+      g.push_back(p);
+    }
+    run_gemms(ctx, g);
+    // T[(i,w),(a',b')] = sum_b X[i,w,a',b] B[b,w,b']   (second half)
+    for (int i = 0; i < nb; ++i) {
+      const int a2 = A[i].r[l + 1], b = B[i].r[l], b2 = B[i].r[l + 1];
+      const size_t tsz = (size_t)4 * r[i] * a2 * b2;
+      T[i] = (l == n - 1) ? ctx->arena.keep(tsz) : ctx->arena.tmp(tsz);
+      GemmProb p = gemm_base(X[i], B[i].core[l], T[i], r[i] * a2, b2, b);
+      p.nbatch = 4;
+      p.a_div = a2; p.a_hi = 4 * (i64)a2 * b; p.a_lo = b; p.a_k = 1; p.a_bs = (i64)a2 * b;
+      p.b_k = 4 * (i64)b2; p.b_n = 1; p.b_bs = b2;
+      p.c_div = a2; p.c_hi = 4 * (i64)a2 * b2; p.c_lo = b2; p.c_n = 1; p.c_bs = (i64)a2 * b2;
+      g.push_back(p);
+    }
+    run_gemms(ctx, g);
+    if (l == n - 1) {
+      for (int i = 0; i < nb; ++i) items[i].core[l] = LeftCore{T[i], r[i], 1, 0};
+      ctx->arena.hi = site_mark;
+      break;
+    }
+    // factorise T (m x kk): identity / truncated SVD keeping min(chi_work, m, kk) left singular vectors
+    std::vector<LqJob> lq;
+    std::vector<SvdJob> svd;
+    std::vector<int> keep(nb, 0);
+    std::vector<double*> Qt(nb, nullptr);
+    for (int i = 0; i < nb; ++i) {
+      const int m = 4 * r[i];
+      const i64 kk = (i64)A[i].r[l + 1] * B[i].r[l + 1];
+      if (m <= std::min<i64>(kk, chi_work)) {
+        items[i].core[l] = LeftCore{nullptr, r[i], m, 2};
+        keep[i] = 0;
+        continue;
+      }
+      keep[i] = (int)std::min<i64>(std::min<i64>(m, kk), chi_work);
+      Qt[i] = ctx->arena.keep((size_t)keep[i] * m);
+      SvdJob j;
+      if (m <= kk) {
+        double* Tc = ctx->arena.tmp((size_t)m * kk);
+        QTT_CU(cudaMemcpyAsync(Tc, T[i], sizeof(double) * (size_t)m * kk, cudaMemcpyDeviceToDevice, ctx->stream));
+        double* R1 = ctx->arena.tmp((size_t)m * m);
+        lq.push_back(LqJob{Tc, m, (int)kk, (int)kk, R1});
+        j.X = R1; j.p = m; j.q = m;
+      } else {
+        double* Y = ctx->arena.tmp((size_t)kk * m);
+        QTT_CU(qtt_launch_transpose(T[i], m, (int)kk, (int)kk, Y, m, ctx->stream));
+        j.X = Y; j.p = (int)kk; j.q = m;
+      }
+      j.out = Qt[i]; j.r_cap = keep[i]; j.chi_max = keep[i];
+      j.sigma = nullptr;
+      j.rank = reinterpret_cast<int*>(ctx->arena.tmp(1));
+      j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
+      svd.push_back(j);
+    }
+    run_lq(ctx, lq);
+    run_svd(ctx, svd);
+    // R' = Q^T T  (keep x kk), into the other carry buffer
+    for (int i = 0; i < nb; ++i) {
+      const int m = 4 * r[i];
+      const i64 kk = (i64)A[i].r[l + 1] * B[i].r[l + 1];
+      double* Rn = Rbuf[l & 1][i];
+      if (keep[i] == 0) {
+        QTT_CU(cudaMemcpyAsync(Rn, T[i], sizeof(double) * (size_t)m * kk, cudaMemcpyDeviceToDevice, ctx->stream));
+        r[i] = m;
+      } else {
+        g.push_back(gemm_nn(Qt[i], m, T[i], kk, Rn, kk, keep[i], (int)kk, m));
+        items[i].core[l] = LeftCore{Qt[i], r[i], keep[i], 1};
+        r[i] = keep[i];
+      }
+      R[i] = Rn;
+    }
+    run_gemms(ctx, g);
+    ctx->arena.hi = site_mark;
+  }
+  if (n == 1) {
+    for (int i = 0; i < nb; ++i) {
+      QTT_CU(qtt_launch_copy2d(items[i].core[0].ptr, 1, 4, 4, out[i].core[0], 4, ctx->stream));
+      out[i].r.assign(2, 1);
+    }
+    return;
+  }
+  sweep_rl(ctx, items, chi, eps, out, nullptr);
+}
+
+// ------------------------------------------------------------------------------------------ lazy kinds
+void qtt_expand_apply_batch(qtt_ctx* ctx, const std::vector<const MpoData*>& W, const std::vector<View>& x,
+                            std::vector<View>& out) {
+  const int nb = (int)x.size();
+  out.assign(nb, View());
+  if (nb == 0) return;
+  const int n = x[0].n;
+  for (int i = 0; i < nb; ++i) {
+    if (W[i]->n != x[i].n || x[i].n != n) QTT_THROW(QTT_SHAPE_MISMATCH, "MPO and MPS differ in length");
+    out[i].n = n;
+    out[i].r.resize(n + 1);
+    out[i].core.resize(n);
+    for (int k = 0; k <= n; ++k) out[i].r[k] = W[i]->D[k] * x[i].r[k];
+  }
+  for (int k = 0; k < n; ++k) {
+    std::vector<ExpandProb> e;
+    for (int i = 0; i < nb; ++i) {
+      double* o = ctx->arena.tmp((size_t)out[i].r[k] * 4 * out[i].r[k + 1]);
+      out[i].core[k] = o;
+      e.push_back(ExpandProb{W[i]->core[k], x[i].core[k], o, W[i]->D[k], W[i]->D[k + 1], x[i].r[k], x[i].r[k + 1]});
+    }
+    QTT_CU(qtt_launch_expand(e.data(), (int)e.size(), ctx->stream));
+  }
+}
+
+View qtt_expand_apply(qtt_ctx* ctx, const MpoData* W, const View& x) {
+  std::vector<View> out;
+  qtt_expand_apply_batch(ctx, {W}, {x}, out);
+  return out[0];
+}
+
+void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double, View>>>& terms,
+                      std::vector<View>& out) {
+  const int nb = (int)terms.size();
+  out.assign(nb, View());
+  if (nb == 0) return;
+  const int n = terms[0][0].second.n;
+  for (int i = 0; i < nb; ++i) {
+    if (terms[i].empty() || terms[i].size() > 5) QTT_THROW(QTT_INVALID_ARG, "a sum has 1..5 terms");
+    out[i].n = n;
+    out[i].r.assign(n + 1, 0);
+    out[i].core.resize(n);
+    for (auto& t : terms[i]) {
+      if (t.second.n != n) QTT_THROW(QTT_SHAPE_MISMATCH, "summands differ in length");
+      for (int k = 0; k <= n; ++k) out[i].r[k] += t.second.r[k];
+    }
+    out[i].r[0] = out[i].r[n] = 1;
+  }
+  for (int k = 0; k < n; ++k) {
+    std::vector<ConcatProb> c;
+    for (int i = 0; i < nb; ++i) {
+      ConcatProb p;
+      std::memset(&p, 0, sizeof(p));
+      p.nterm = (int)terms[i].size();
+      for (int t = 0; t < p.nterm; ++t) {
+        p.src[t] = terms[i][t].second.core[k];
+        p.alpha[t] = terms[i][t].first;
+        p.rl[t] = terms[i][t].second.r[k];
+        p.rr[t] = terms[i][t].second.r[k + 1];
+      }
+      p.mode = (n == 1) ? 3 : (k == 0 ? 0 : (k == n - 1 ? 2 : 1));
+      double* o = ctx->arena.tmp((size_t)out[i].r[k] * 4 * out[i].r[k + 1]);
+      out[i].core[k] = o;
+      p.out = o;
+      c.push_back(p);
+    }
+    if (n == 1) QTT_THROW(QTT_INVALID_ARG, "sums of one-site MPS are not supported");
+    QTT_CU(qtt_launch_concat(c.data(), (int)c.size(), ctx->stream));
+  }
+}
+
+View qtt_kron(qtt_ctx* ctx, const View& a, const View& b) {
+  if (a.n != b.n) QTT_THROW(QTT_SHAPE_MISMATCH, "product operands differ in length");
+  View o;
+  o.n = a.n;
+  o.r.resize(a.n + 1);
+  o.core.resize(a.n);
+  for (int k = 0; k <= a.n; ++k) o.r[k] = a.r[k] * b.r[k];
+  for (int k = 0; k < a.n; ++k) {
+    double* out = ctx->arena.tmp((size_t)o.r[k] * 4 * o.r[k + 1]);
+    KronProb p{a.core[k], b.core[k], out, a.r[k], a.r[k + 1], b.r[k], b.r[k + 1]};
+    QTT_CU(qtt_launch_kron(&p, 1, ctx->stream));
+    o.core[k] = out;
+  }
+  return o;
+}
+
+// ------------------------------------------------------------------------------------------ boundary
+void qtt_to_dense_view(qtt_ctx* ctx, const View& v, double* dense_dev_out) {
+  const int n = v.n;
+  const double* T = v.core[0];  // 4 x r_1
+  i64 rows = 4;
+  std::vector<GemmProb> g;
+  for (int k = 1; k < n; ++k) {
+    double* Tn = ctx->arena.tmp((size_t)rows * 4 * v.r[k + 1]);
+    g.push_back(gemm_nn(T, v.r[k], v.core[k], 4 * (i64)v.r[k + 1], Tn, 4 * (i64)v.r[k + 1], (int)rows, 4 * v.r[k + 1],
+                        v.r[k]));
+    run_gemms(ctx, g);
+    T = Tn;
+    rows *= 4;
+  }
+  QTT_CU(qtt_launch_interleave(T, dense_dev_out, n, 1, ctx->stream));
+}
+
+void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, double eps, OutMps& out) {
+  const int n = nbits;
+  const i64 total = 1ll << (2 * n);
+  double* carry = ctx->arena.tmp((size_t)total);
+  QTT_CU(qtt_launch_interleave(dense_dev, carry, n, 0, ctx->stream));
+  out.r.assign(n + 1, 1);
+  if (n == 1) {
+    QTT_CU(qtt_launch_copy2d(carry, 1, 4, 4, out.core[0], 4, ctx->stream));
+    return;
+  }
+  int rc = 1;
+  double* delta = eps > 0.0 ? ctx->arena.tmp(1) : nullptr;
+  int* rank_dev = reinterpret_cast<int*>(ctx->arena.tmp(1));
+  std::vector<GemmProb> g;
+  for (int k = n - 1; k >= 1; --k) {
+    // unfolding M: 4^k x (4 rc)
+    const i64 rows = 1ll << (2 * k);
+    const int q = 4 * rc;
+    if (rows > 2147483647ll / std::max(q, 1)) QTT_THROW(QTT_CAPACITY, "grid too large");
+    std::vector<SvdJob> svd;
+    SvdJob j;
+    if (rows <= q || rows < 8) {
+      double* Mc = ctx->arena.tmp((size_t)rows * q);
+      QTT_CU(qtt_launch_copy2d(carry, (int)rows, q, q, Mc, q, ctx->stream));
+      j.X = Mc; j.p = (int)rows; j.q = q;
+    } else {
+      // same right singular vectors as its triangular factor: LQ of M^T (q x rows)
+      double* Mt = ctx->arena.tmp((size_t)rows * q);
+      QTT_CU(qtt_launch_transpose(carry, (int)rows, q, q, Mt, (int)rows, ctx->stream));
+      double* R = ctx->arena.tmp((size_t)q * q);
+      std::vector<LqJob> lq{LqJob{Mt, q, (int)rows, (int)rows, R}};
+      run_lq(ctx, lq);
+      j.X = R; j.p = q; j.q = q;
+    }
+    j.out = out.core[k];
+    j.r_cap = out.rcap[k];
+    j.chi_max = std::min(chi, out.rcap[k]);
+    j.sigma = nullptr;
+    j.rank = rank_dev;
+    j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
+    if (eps > 0.0) {
+      if (k == n - 1) {
+        j.delta_out = delta;
+        j.delta_scale = eps / std::sqrt((double)std::max(n - 1, 1));
+      } else {
+        j.delta_ptr = delta;
+      }
+    }
+    svd.push_back(j);
+    run_svd(ctx, svd);
+    int rn = (int)std::max<i64>(1, std::min<i64>(std::min(chi, out.rcap[k]), std::min<i64>(rows, q)));
+    if (eps > 0.0) {
+      QTT_CU(cudaMemcpyAsync(&rn, rank_dev, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+      QTT_CU(cudaStreamSynchronize(ctx->stream));
+    }
+    // carry <- M * core'^T  (4^k x r')
+    double* Cn = ctx->arena.tmp((size_t)rows * rn);
+    g.push_back(gemm_nt(carry, q, out.core[k], q, Cn, rn, (int)rows, rn, q));
+    run_gemms(ctx, g);
+    carry = Cn;
+    rc = rn;
+    out.r[k] = rn;
+  }
+  QTT_CU(qtt_launch_copy2d(carry, 4, rc, rc, out.core[0], rc, ctx->stream));
+}
+
+double* qtt_dot_view(qtt_ctx* ctx, const View& a, const View& b) {
+  if (a.n != b.n) QTT_THROW(QTT_SHAPE_MISMATCH, "operands differ in length");
+  const double* E = ctx->ones;  // ra x rb
+  std::vector<GemmProb> g;
+  for (int k = 0; k < a.n; ++k) {
+    const int ra = a.r[k], rb = b.r[k], a2 = a.r[k + 1], b2 = b.r[k + 1];
+    // G[b,(w,a')] = sum_a E[a,b] A[a,(w,a')]
+    double* G = ctx->arena.tmp((size_t)rb * 4 * a2);
+    g.push_back(gemm_tn(E, rb, a.core[k], 4 * (i64)a2, G, 4 * (i64)a2, rb, 4 * a2, ra));
+    run_gemms(ctx, g);
+    // E'[a',b'] = sum_{(b,w)} G[(b,w),a'] B[(b,w),b']
+    double* En = ctx->arena.tmp((size_t)a2 * b2);
+    g.push_back(gemm_tn(G, a2, b.core[k], b2, En, b2, a2, b2, 4 * rb));
+    run_gemms(ctx, g);
+    E = En;
+  }
+  return const_cast<double*>(E);
+}
+
+// ------------------------------------------------------------------------------------------ O8 / O9
+namespace {
+
+std::vector<OutMps> alloc_outs_keep(qtt_ctx* ctx, const std::vector<std::vector<int>>& caps) {
+  std::vector<OutMps> out(caps.size());
+  for (size_t i = 0; i < caps.size(); ++i) {
+    const int n = (int)caps[i].size() - 1;
+    out[i].n = n;
+    out[i].rcap = caps[i];
+    out[i].core.resize(n);
+    for (int k = 0; k < n; ++k) out[i].core[k] = ctx->arena.keep((size_t)caps[i][k] * 4 * caps[i][k + 1]);
+  }
+  return out;
+}
+View view_of(const OutMps& o) {
+  View v;
+  v.n = o.n;
+  v.r = o.r;
+  v.core.assign(o.core.begin(), o.core.end());
+  return v;
+}
+
+// f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i   (oracle O8)
+void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap, double Re, int chi, double eps,
+         int chi_work, View f[2]) {
+  // level 1: six applies + roundings in one batch: (D1 u_i, D2 u_i, Lap u_i) for i = 0, 1
+  std::vector<View> g(6);
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<const MpoData*> W{Dj[0], Dj[1], Lap, Dj[0], Dj[1], Lap};
+    std::vector<View> X{u[0], u[0], u[0], u[1], u[1], u[1]};
+    std::vector<View> ex;
+    qtt_expand_apply_batch(ctx, W, X, ex);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : ex) caps.push_back(qtt_round_caps(e.r, chi));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, ex, chi, eps, out);
+    for (int i = 0; i < 6; ++i) g[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+  // level 2: four products c_ij = u_j (.) g_ij
+  std::vector<View> c(4);
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<View> A{u[0], u[1], u[0], u[1]};
+    std::vector<View> B{g[0], g[1], g[3], g[4]};
+    std::vector<std::vector<int>> caps;
+    for (int i = 0; i < 4; ++i) {
+      std::vector<int> rw, ro;
+      qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro);
+      caps.push_back(ro);
+    }
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_product_batch(ctx, A, B, chi, eps, chi_work, out);
+    for (int i = 0; i < 4; ++i) c[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+  // level 3: f_i = -c_i1 - c_i2 + lap_i / Re, one rounding each
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<std::vector<std::pair<double, View>>> terms(2);
+    for (int i = 0; i < 2; ++i) terms[i] = {{-1.0, c[2 * i]}, {-1.0, c[2 * i + 1]}, {1.0 / Re, g[3 * i + 2]}};
+    std::vector<View> s;
+    qtt_concat_batch(ctx, terms, s);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : s) caps.push_back(qtt_round_caps(e.r, chi));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, s, chi, eps, out);
+    for (int i = 0; i < 2; ++i) f[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+}
+
+void lincomb_round(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double, View>>>& terms, int chi, double eps,
+                   std::vector<OutMps>& out) {
+  const size_t mark = ctx->arena.hi;
+  std::vector<View> s;
+  qtt_concat_batch(ctx, terms, s);
+  qtt_round_dense_batch(ctx, s, chi, eps, out);
+  ctx->arena.hi = mark;
+}
+
+}  // namespace
+
+void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
+                   double dt, int chi, double eps, int chi_work, OutMps out[2]) {
+  const MpoData* Dj[2] = {Dx, Dy};
+  View k1[2], k2[2], k3[2], k4[2], us[2];
+  auto stage = [&](const View kk[2], double h, View dst[2]) {
+    std::vector<std::vector<std::pair<double, View>>> terms(2);
+    std::vector<std::vector<int>> caps;
+    for (int i = 0; i < 2; ++i) {
+      terms[i] = {{1.0, u[i]}, {h, kk[i]}};
+      std::vector<int> rs(u[i].r.size());
+      for (size_t b = 0; b < rs.size(); ++b) rs[b] = u[i].r[b] + kk[i].r[b];
+      rs.front() = rs.back() = 1;
+      caps.push_back(qtt_round_caps(rs, chi));
+    }
+    std::vector<OutMps> o = alloc_outs_keep(ctx, caps);
+    lincomb_round(ctx, terms, chi, eps, o);
+    for (int i = 0; i < 2; ++i) dst[i] = view_of(o[i]);
+  };
+  rhs(ctx, u, Dj, Lap, Re, chi, eps, chi_work, k1);
+  stage(k1, dt / 2, us);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k2);
+  stage(k2, dt / 2, us);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k3);
+  stage(k3, dt, us);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k4);
+  std::vector<std::vector<std::pair<double, View>>> terms(2);
+  for (int i = 0; i < 2; ++i)
+    terms[i] = {{1.0, u[i]}, {dt / 6, k1[i]}, {dt / 3, k2[i]}, {dt / 3, k3[i]}, {dt / 6, k4[i]}};
+  std::vector<OutMps> o{out[0], out[1]};
+  lincomb_round(ctx, terms, chi, eps, o);
+  out[0] = o[0];
+  out[1] = o[1];
+}
