@@ -86,6 +86,14 @@ qtt_status qtt_to_dense(qtt_ctx* ctx, const qtt_mps* x, double* dense_dev_out);
  * entries with both ends 1. */
 qtt_status qtt_mpo_create(qtt_ctx* ctx, int n_sites, const int* bonds, const double* const* cores_host,
                           qtt_mpo** out);
+/* PAPER.md:391-424 App. A (Eq. A1-A3, Table II): the periodic central-difference MPO
+ * (F[i+1] - F[i-1]) / (2 dx) along direction 1 (x) or 2 (y), bond 3, boundary vectors L = (1,1,1) on the
+ * most-significant site and R = (0, 1, -1)/(2 dx) on the least-significant site folded into the end cores.
+ * Index convention: w = output, w' = contracted with the MPS (reading 1).  n_sites >= 2. */
+qtt_status qtt_mpo_central_difference(qtt_ctx* ctx, int n_sites, int direction, double dx, qtt_mpo** out);
+/* Compact periodic 5-point Laplacian MPO, bond 5 (reading 3): channels identity, x+1, x-1, y+1, y-1;
+ * L = (1,1,1,1,1), R = (-4,1,1,1,1)/dx^2.  n_sites >= 2. */
+qtt_status qtt_mpo_laplacian(qtt_ctx* ctx, int n_sites, double dx, qtt_mpo** out);
 void qtt_mpo_free(qtt_mpo* w);
 
 /* y = W x, exact, bond D*chi, composite bond index = alpha*chi + a (lazy). */

@@ -1,0 +1,269 @@
+"""Thin Python binding of the C ABI in include/qtt.h: argument marshalling only.
+
+PyTorch is used for device memory (the alloc/release callbacks hand out torch-owned blocks) and for
+the CUDA stream; every numerical step runs in the kernels of libqtt_b200.so.  Function names follow
+the C ABI (``qtt_mps_from_dense`` ...).  Errors raise :class:`QttError` with the library's message.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Sequence
+
+import numpy as np
+import torch
+
+from . import _lib
+
+
+class QttError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_lib.STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+class Context:
+    """qtt_ctx: one CUDA device, one stream, one workspace.  Owns the torch blocks the library asks for."""
+
+    def __init__(self, device: int = 0, workspace_bytes: int = 1 << 30, stream: "torch.cuda.Stream | None" = None):
+        self.lib = _lib.load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: libqtt_b200 has no CPU fallback")
+        self.device = torch.device("cuda", device)
+        # stream capture (CUDA graphs) is not allowed on the legacy default stream
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+        self._blocks: dict[int, torch.Tensor] = {}
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device=self.device)
+            except Exception:
+                return None
+            self._blocks[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _release(ptr, _user):
+            self._blocks.pop(ptr, None)
+
+        self._alloc_cb = _lib.ALLOC_FN(_alloc)
+        self._release_cb = _lib.RELEASE_FN(_release)
+        h = C.c_void_p()
+        st = self.lib.qtt_ctx_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream), self._alloc_cb,
+                                     self._release_cb, None, workspace_bytes)
+        if st != _lib.QTT_OK:
+            raise QttError(st, "qtt_ctx_create failed")
+        self.h = h
+
+    def check(self, st: int):
+        if st != _lib.QTT_OK:
+            raise QttError(st, self.lib.qtt_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.qtt_ctx_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+
+class Mps:
+    def __init__(self, ctx: Context, h):
+        self.ctx, self.h = ctx, h
+
+    def free(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.qtt_mps_free(self.h)
+        self.h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Mpo:
+    def __init__(self, ctx: Context, h):
+        self.ctx, self.h = ctx, h
+
+    def free(self):
+        if self.h and self.ctx.h:
+            self.ctx.lib.qtt_mpo_free(self.h)
+        self.h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def _cores_args(cores: Sequence[np.ndarray], ndim: int):
+    arrs = [np.ascontiguousarray(c, dtype=np.float64) for c in cores]
+    for a in arrs:
+        if a.ndim != ndim:
+            raise ValueError(f"cores must have {ndim} dimensions")
+    n = len(arrs)
+    bonds = (C.c_int * (n + 1))(*([a.shape[0] for a in arrs] + [arrs[-1].shape[-1]]))
+    ptrs = (C.POINTER(C.c_double) * n)(*[a.ctypes.data_as(C.POINTER(C.c_double)) for a in arrs])
+    return arrs, n, bonds, ptrs
+
+
+# ------------------------------------------------------------------ the calls of include/qtt.h
+def qtt_mps_from_dense(ctx: Context, dense: torch.Tensor, chi_max: int, eps: float = 0.0) -> Mps:
+    """dense: N x N fp64 CUDA tensor F[x][y]."""
+    if dense.dtype != torch.float64 or not dense.is_cuda or dense.dim() != 2 or dense.shape[0] != dense.shape[1]:
+        raise ValueError("dense must be a square fp64 CUDA tensor")
+    dense = dense.contiguous()
+    n = int(dense.shape[0]).bit_length() - 1
+    if (1 << n) != dense.shape[0]:
+        raise ValueError("N must be a power of two")
+    ctx.stream.wait_stream(torch.cuda.current_stream(ctx.device))
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mps_from_dense(ctx.h, C.c_void_p(dense.data_ptr()), n, int(chi_max), float(eps), C.byref(h)))
+    dense.record_stream(ctx.stream)
+    return Mps(ctx, h)
+
+
+def qtt_mps_from_cores(ctx: Context, cores: Sequence[np.ndarray]) -> Mps:
+    arrs, n, bonds, ptrs = _cores_args(cores, 3)
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mps_from_cores(ctx.h, n, bonds, ptrs, C.byref(h)))
+    return Mps(ctx, h)
+
+
+def qtt_to_dense(ctx: Context, x: Mps) -> torch.Tensor:
+    n = ctx.lib.qtt_mps_num_sites(x.h)
+    N = 1 << n
+    out = torch.empty((N, N), dtype=torch.float64, device=ctx.device)
+    ctx.stream.wait_stream(torch.cuda.current_stream(ctx.device))
+    ctx.check(ctx.lib.qtt_to_dense(ctx.h, x.h, C.c_void_p(out.data_ptr())))
+    out.record_stream(ctx.stream)
+    torch.cuda.current_stream(ctx.device).wait_stream(ctx.stream)
+    return out
+
+
+def qtt_mpo_create(ctx: Context, cores: Sequence[np.ndarray]) -> Mpo:
+    arrs, n, bonds, ptrs = _cores_args(cores, 4)
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mpo_create(ctx.h, n, bonds, ptrs, C.byref(h)))
+    return Mpo(ctx, h)
+
+
+def qtt_mpo_central_difference(ctx: Context, n_sites: int, direction: int, dx: float) -> Mpo:
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mpo_central_difference(ctx.h, n_sites, direction, float(dx), C.byref(h)))
+    return Mpo(ctx, h)
+
+
+def qtt_mpo_laplacian(ctx: Context, n_sites: int, dx: float) -> Mpo:
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mpo_laplacian(ctx.h, n_sites, float(dx), C.byref(h)))
+    return Mpo(ctx, h)
+
+
+def qtt_apply_mpo(ctx: Context, w: Mpo, x: Mps) -> Mps:
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_apply_mpo(ctx.h, w.h, x.h, C.byref(h)))
+    return Mps(ctx, h)
+
+
+def qtt_hadamard(ctx: Context, a: Mps, b: Mps) -> Mps:
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_hadamard(ctx.h, a.h, b.h, C.byref(h)))
+    return Mps(ctx, h)
+
+
+def qtt_axpy(ctx: Context, alpha: float, x: Mps, y: Mps) -> None:
+    ctx.check(ctx.lib.qtt_axpy(ctx.h, float(alpha), x.h, y.h))
+
+
+def qtt_round(ctx: Context, x: Mps, chi_max: int, eps: float = 0.0) -> None:
+    ctx.check(ctx.lib.qtt_round(ctx.h, x.h, int(chi_max), float(eps)))
+
+
+def qtt_round_batch(ctx: Context, xs: Sequence[Mps], chi_max: int, eps: float = 0.0) -> None:
+    arr = (C.c_void_p * len(xs))(*[x.h for x in xs])
+    ctx.check(ctx.lib.qtt_round_batch(ctx.h, len(xs), arr, int(chi_max), float(eps)))
+
+
+def qtt_rk4_step(ctx: Context, u: Sequence[Mps], Dx: Mpo, Dy: Mpo, Lap: Mpo, Re: float, dt: float, chi_max: int,
+                 eps: float = 0.0) -> None:
+    arr = (C.c_void_p * 2)(u[0].h, u[1].h)
+    ctx.check(ctx.lib.qtt_rk4_step(ctx.h, arr, Dx.h, Dy.h, Lap.h, float(Re), float(dt), int(chi_max), float(eps)))
+
+
+# ------------------------------------------------------------------ inspection
+def qtt_mps_bonds(x: Mps) -> list[int]:
+    n = x.ctx.lib.qtt_mps_num_sites(x.h)
+    b = (C.c_int * (n + 1))()
+    x.ctx.check(x.ctx.lib.qtt_mps_bonds(x.h, b))
+    return list(b)
+
+
+def qtt_mps_get_core(ctx: Context, x: Mps, k: int) -> np.ndarray:
+    r = qtt_mps_bonds(x)
+    out = np.empty((r[k], 4, r[k + 1]), dtype=np.float64)
+    ctx.check(ctx.lib.qtt_mps_get_core(ctx.h, x.h, k, out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
+def qtt_mps_get_cores(ctx: Context, x: Mps) -> list[np.ndarray]:
+    return [qtt_mps_get_core(ctx, x, k) for k in range(ctx.lib.qtt_mps_num_sites(x.h))]
+
+
+def qtt_mps_dot(ctx: Context, a: Mps, b: Mps) -> float:
+    v = C.c_double()
+    ctx.check(ctx.lib.qtt_mps_dot(ctx.h, a.h, b.h, C.byref(v)))
+    return v.value
+
+
+def qtt_mps_norm(ctx: Context, x: Mps) -> float:
+    v = C.c_double()
+    ctx.check(ctx.lib.qtt_mps_norm(ctx.h, x.h, C.byref(v)))
+    return v.value
+
+
+def qtt_mps_schmidt(ctx: Context, x: Mps) -> list:
+    """Schmidt values per bond (index 1..n-1; entries 0 and n are None)."""
+    r = qtt_mps_bonds(x)
+    n = len(r) - 1
+    cap = max(max(r), 1) * 4
+    buf = np.zeros((n + 1, cap), dtype=np.float64)
+    counts = (C.c_int * (n + 1))()
+    ctx.check(ctx.lib.qtt_mps_schmidt(ctx.h, x.h, buf.ctypes.data_as(C.POINTER(C.c_double)), cap, counts))
+    return [None] + [buf[k, : counts[k]].copy() for k in range(1, n)] + [None]
+
+
+def qtt_mps_clone(ctx: Context, x: Mps) -> Mps:
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mps_clone(ctx.h, x.h, C.byref(h)))
+    return Mps(ctx, h)
+
+
+def qtt_ctx_set_chi_work(ctx: Context, chi_work: int) -> None:
+    ctx.check(ctx.lib.qtt_ctx_set_chi_work(ctx.h, int(chi_work)))
+
+
+def qtt_ctx_set_graphs(ctx: Context, enabled: bool) -> None:
+    ctx.check(ctx.lib.qtt_ctx_set_graphs(ctx.h, 1 if enabled else 0))
+
+
+def qtt_ctx_set_materialize_limit(ctx: Context, nbytes: int) -> None:
+    ctx.check(ctx.lib.qtt_ctx_set_materialize_limit(ctx.h, int(nbytes)))
+
+
+def qtt_ctx_jacobi_stats(ctx: Context) -> tuple[int, int]:
+    a, b = C.c_int(), C.c_int()
+    ctx.check(ctx.lib.qtt_ctx_jacobi_stats(ctx.h, C.byref(a), C.byref(b)))
+    return a.value, b.value
+
+
+def qtt_ctx_launch_count(ctx: Context) -> int:
+    return int(ctx.lib.qtt_ctx_launch_count(ctx.h))

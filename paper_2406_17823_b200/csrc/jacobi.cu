@@ -37,6 +37,9 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
   double* part = sm + (g.use_smem ? (size_t)pmax * wp : 0);
   double* rot = part + 2 * MAXC * 3 * np2_max;
   int* flags = reinterpret_cast<int*>(rot + 2 * np2_max);  // [0] rotations this sweep
+  // Largest squared row norm seen so far, identical in every CTA of the cluster (it is derived from the
+  // exchanged totals only): [0] accumulates during phase B1, [1] is the value phase B1 reads.
+  unsigned long long* nmax = reinterpret_cast<unsigned long long*>(flags + 2);
 
   const int w = g.wslice;
   const int cs = rank * w;
@@ -54,7 +57,10 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
     S = P.X + cs;
     rs = P.ld;
   }
-  if (tid == 0) flags[0] = 0;
+  if (tid == 0) {
+    flags[0] = 0;
+    nmax[0] = nmax[1] = 0ull;
+  }
   __syncthreads();
 
   // threads per pair: power of two, chosen so one pass covers all pairs when possible
@@ -122,7 +128,12 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
         }
         double c = 1.0, s = 0.0;
         const double lim = tol * sqrt(aa) * sqrt(bb);
-        if (fabs(ab) > lim && lim > 0.0) {
+        // rows below eps * (largest row norm) are zero to working accuracy: rotating them against each
+        // other never terminates when p > rank (they cannot all be mutually orthogonal); the selection
+        // step writes such rows out as exact zeros
+        const double floor2 = 4.930380657631324e-32 * __longlong_as_double((long long)nmax[1]);
+        atomicMax(&nmax[0], (unsigned long long)__double_as_longlong(fmax(aa, bb)));
+        if (fabs(ab) > lim && lim > 0.0 && aa > floor2 && bb > floor2) {
           const double zeta = (bb - aa) / (2.0 * ab);
           const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
           c = 1.0 / sqrt(1.0 + t * t);
@@ -154,6 +165,7 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
         }
       }
       par ^= 1u;
+      if (tid == 0) nmax[1] = nmax[0];
       __syncthreads();
     }
     const int nrot = flags[0];
@@ -265,7 +277,8 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
     if (j < r) {
       src = idx[j];
       double s2 = key[j];
-      inv = (s2 > 1e-290) ? rsqrt(s2) : 0.0;
+      // rows below 4 eps sigma_1 were not orthogonalised (see the row-Jacobi floor): exact zeros
+      inv = (s2 > 1e-290 && s2 > 7.888609052210118e-31 * key[0]) ? rsqrt(s2) : 0.0;
       // one Newton step: rsqrt() is accurate to ~1 ulp in fp64, keep the normalisation at full precision
       inv = inv * (1.5 - 0.5 * s2 * inv * inv);
     }

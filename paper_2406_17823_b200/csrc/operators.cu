@@ -1,0 +1,88 @@
+// Finite-difference MPO builders of the C ABI (include/qtt.h: qtt_mpo_central_difference,
+// qtt_mpo_laplacian).  Host code: the cores are tiny 0/1 tensors, built once and uploaded through
+// qtt_mpo_create.
+//
+// Construction (App. A): a periodic shift x -> x + s, s = +-1, is a ripple-carry adder
+// running from the least-significant site to the most-significant one.  The MPO bond carries the
+// "request" still to be served: channel 0 = nothing to add (identity on the site), channel c > 0 = add
+// s_c to the bit b_c of this site.  out[w] takes in[w'] with  bit(w') = bit(w) + s (mod 2)  and the
+// request travels on to the more significant neighbour iff that addition wrapped.  The periodic
+// boundary drops the request that leaves the most-significant site (L = all ones); the stencil
+// weights sit on the least-significant end (R).  Index convention W[alpha_m][w (out)][w' (in)][alpha_{m+1}].
+#include <vector>
+
+#include "../../include/qtt.h"
+
+namespace {
+
+struct Channel {
+  int bit;    // which bit of w = 2*x_bit + y_bit is shifted: 1 = x, 0 = y; -1 = identity channel
+  int shift;  // +1: out[i] = in[i+1];  -1: out[i] = in[i-1]
+};
+
+// Bulk core for a list of channels (channel 0 must be the identity), D = channels.size().
+std::vector<double> bulk_core(const std::vector<Channel>& ch) {
+  const int D = (int)ch.size();
+  std::vector<double> C((size_t)D * 16 * D, 0.0);
+  auto at = [&](int am, int w, int wp, int am1) -> double& { return C[(((size_t)am * 4 + w) * 4 + wp) * D + am1]; };
+  for (int w = 0; w < 4; ++w) at(0, w, w, 0) = 1.0;
+  for (int c = 1; c < D; ++c) {
+    const int mask = 1 << ch[c].bit;
+    for (int w = 0; w < 4; ++w) {
+      const int out_bit = (w & mask) ? 1 : 0;
+      const int wp = w ^ mask;  // the shifted bit always flips
+      // in = out + 1: wraps when out_bit == 1;  in = out - 1: borrows when out_bit == 0
+      const bool onward = (ch[c].shift > 0) ? (out_bit == 1) : (out_bit == 0);
+      at(onward ? c : 0, w, wp, c) = 1.0;
+    }
+  }
+  return C;
+}
+
+qtt_status build(qtt_ctx* ctx, int n, const std::vector<Channel>& ch, const std::vector<double>& Rvec, qtt_mpo** out) {
+  if (!ctx || !out || n < 2) return QTT_INVALID_ARG;
+  const int D = (int)ch.size();
+  const std::vector<double> C = bulk_core(ch);
+  // first core: L = ones contracted into alpha_m  -> [1][4][4][D]
+  std::vector<double> first((size_t)16 * D, 0.0);
+  for (int am = 0; am < D; ++am)
+    for (int e = 0; e < 16; ++e)
+      for (int a1 = 0; a1 < D; ++a1) first[(size_t)e * D + a1] += C[((size_t)am * 16 + e) * D + a1];
+  // last core: R contracted into alpha_{m+1} -> [D][4][4][1]
+  std::vector<double> last((size_t)D * 16, 0.0);
+  for (int am = 0; am < D; ++am)
+    for (int e = 0; e < 16; ++e) {
+      double s = 0.0;
+      for (int a1 = 0; a1 < D; ++a1) s += C[((size_t)am * 16 + e) * D + a1] * Rvec[a1];
+      last[(size_t)am * 16 + e] = s;
+    }
+  std::vector<int> bonds(n + 1, D);
+  bonds[0] = bonds[n] = 1;
+  std::vector<const double*> cores(n, C.data());
+  cores[0] = first.data();
+  cores[n - 1] = last.data();
+  return qtt_mpo_create(ctx, n, bonds.data(), cores.data(), out);
+}
+
+}  // namespace
+
+extern "C" {
+
+qtt_status qtt_mpo_central_difference(qtt_ctx* ctx, int n_sites, int direction, double dx, qtt_mpo** out) {
+  if (direction != 1 && direction != 2) return QTT_INVALID_ARG;
+  if (!(dx > 0.0)) return QTT_INVALID_ARG;
+  const int bit = (direction == 1) ? 1 : 0;
+  std::vector<Channel> ch{{-1, 0}, {bit, +1}, {bit, -1}};
+  std::vector<double> R{0.0, 1.0 / (2.0 * dx), -1.0 / (2.0 * dx)};
+  return build(ctx, n_sites, ch, R, out);
+}
+
+qtt_status qtt_mpo_laplacian(qtt_ctx* ctx, int n_sites, double dx, qtt_mpo** out) {
+  if (!(dx > 0.0)) return QTT_INVALID_ARG;
+  std::vector<Channel> ch{{-1, 0}, {1, +1}, {1, -1}, {0, +1}, {0, -1}};
+  const double h = 1.0 / (dx * dx);
+  std::vector<double> R{-4.0 * h, h, h, h, h};
+  return build(ctx, n_sites, ch, R, out);
+}
+
+}  // extern "C"

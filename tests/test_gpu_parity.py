@@ -1,0 +1,293 @@
+"""GPU parity proper: the qtt_* C ABI (through the ctypes binding) against the CPU oracle on the
+same seeded host inputs.  Bar (BASELINE.json north_star): relative Frobenius error <= 1e-10 on dense
+reconstructions, Schmidt spectra within 1e-9 * sigma_1; integer results (bonds, ranks) exact."""
+import numpy as np
+import pytest
+
+import qtt_inputs as I
+from oracle import qtt_oracle as O
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def Q():
+    import paper_2406_17823_b200 as q
+    return q
+
+
+@pytest.fixture(scope="module")
+def ctx(Q):
+    c = Q.Context(device=0, workspace_bytes=2 << 30)
+    yield c
+    c.close()
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def gpu_dense(Q, ctx, x):
+    t = Q.qtt_to_dense(ctx, x)
+    ctx.synchronize()
+    return t.cpu().numpy()
+
+
+def smooth_field(n, seed):
+    N = 1 << n
+    rng = np.random.default_rng(seed)
+    X, Y = I.grid(n)
+    F = np.zeros((N, N))
+    for kx in range(-3, 4):
+        for ky in range(-3, 4):
+            a, p = rng.standard_normal(), rng.uniform(0, 2 * np.pi)
+            F += a / (1 + kx * kx + ky * ky) * np.cos(2 * np.pi * (kx * X + ky * Y) + p)
+    return F + np.tanh((Y - 0.5) / 0.1)
+
+
+def ops(Q, ctx, n):
+    dx = 1.0 / (1 << n)
+    g = (Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx),
+         Q.qtt_mpo_laplacian(ctx, n, dx))
+    o = (O.mpo_d1(n, dx), O.mpo_d2(n, dx), O.mpo_laplacian(n, dx))
+    return g, o
+
+
+# ---------------------------------------------------------------- boundary: encode / decode
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 7])
+def test_from_cores_to_dense_matches_oracle(Q, ctx, n):
+    cores = I.random_cores(n, 6, seed=n)
+    x = Q.qtt_mps_from_cores(ctx, cores)
+    assert Q.qtt_mps_bonds(x) == O.bonds(cores)
+    assert rel(gpu_dense(Q, ctx, x), O.to_dense(cores)) < 1e-13
+
+
+@pytest.mark.parametrize("n,chi", [(2, 100), (4, 1000), (5, 8), (6, 7), (8, 32)])
+def test_from_dense_matches_oracle(Q, ctx, n, chi):
+    import torch
+    F = smooth_field(n, 3) + 1e-3 * np.random.default_rng(n).standard_normal((1 << n, 1 << n))
+    want = O.from_dense(F, chi)
+    x = Q.qtt_mps_from_dense(ctx, torch.from_numpy(F).cuda(), chi)
+    assert Q.qtt_mps_bonds(x) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, x), O.to_dense(want)) < TOL
+
+
+def test_from_dense_eps_rule_matches_oracle_ranks(Q, ctx):
+    import torch
+    F = smooth_field(6, 9)
+    for eps in (1e-2, 1e-5):
+        want = O.from_dense(F, 1 << 20, eps)
+        x = Q.qtt_mps_from_dense(ctx, torch.from_numpy(F).cuda(), 1 << 20, eps)
+        assert Q.qtt_mps_bonds(x) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, x), O.to_dense(want)) < TOL
+
+
+# ---------------------------------------------------------------- operators (native builders)
+@pytest.mark.parametrize("n", [2, 4, 6])
+def test_native_mpo_builders_match_oracle_operators(Q, ctx, n):
+    g, o = ops(Q, ctx, n)
+    cores = I.random_cores(n, 5, seed=1)
+    x = Q.qtt_mps_from_cores(ctx, cores)
+    for Wg, Wo in zip(g, o):
+        y = Q.qtt_apply_mpo(ctx, Wg, x)
+        want = O.apply_mpo(Wo, cores)
+        assert Q.qtt_mps_bonds(y) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, y), O.to_dense(want)) < 1e-13
+        # element-wise equality of the exact expanded cores
+        for k in range(n):
+            assert np.allclose(Q.qtt_mps_get_core(ctx, y, k), want[k], rtol=1e-14, atol=0)
+
+
+def test_mpo_create_from_host_cores(Q, ctx):
+    n = 5
+    dx = 1.0 / 32
+    Wo = O.mpo_laplacian(n, dx)
+    W = Q.qtt_mpo_create(ctx, Wo)
+    cores = I.random_cores(n, 4, seed=2)
+    x = Q.qtt_mps_from_cores(ctx, cores)
+    y = Q.qtt_apply_mpo(ctx, W, x)
+    assert rel(gpu_dense(Q, ctx, y), O.to_dense(O.apply_mpo(Wo, cores))) < 1e-13
+
+
+# ---------------------------------------------------------------- exact lazy algebra
+def test_hadamard_and_axpy_exact(Q, ctx):
+    n = 5
+    A, B, Cc = (I.random_cores(n, c, seed=s) for c, s in ((4, 1), (3, 2), (5, 3)))
+    a, b, c = (Q.qtt_mps_from_cores(ctx, t) for t in (A, B, Cc))
+    h = Q.qtt_hadamard(ctx, a, b)
+    assert Q.qtt_mps_bonds(h) == O.bonds(O.hadamard(A, B))
+    assert rel(gpu_dense(Q, ctx, h), O.to_dense(A) * O.to_dense(B)) < 1e-13
+    y = Q.qtt_mps_clone(ctx, c)
+    Q.qtt_axpy(ctx, -2.5, a, y)
+    Q.qtt_axpy(ctx, 0.125, b, y)
+    want = O.lincomb([(0.125, B), (-2.5, A), (1.0, Cc)])
+    assert Q.qtt_mps_bonds(y) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, y), O.to_dense(want)) < 1e-13
+    assert abs(Q.qtt_mps_dot(ctx, a, b) - O.dot(A, B)) <= 1e-12 * O.norm(A) * O.norm(B)
+    assert abs(Q.qtt_mps_norm(ctx, c) - O.norm(Cc)) <= 1e-12 * O.norm(Cc)
+
+
+# ---------------------------------------------------------------- rounding
+@pytest.mark.parametrize("n,chi0,chi", [(4, 16, 3), (5, 12, 8), (6, 20, 6), (8, 24, 16), (8, 40, 32)])
+def test_round_dense_matches_oracle(Q, ctx, n, chi0, chi):
+    F = smooth_field(n, n) + 1e-2 * np.random.default_rng(n).standard_normal((1 << n, 1 << n))
+    A = O.from_dense(F, chi0)
+    # scramble the gauge so that the input is not already canonical
+    rng = np.random.default_rng(7)
+    for k in range(n - 1):
+        r = A[k].shape[2]
+        G = rng.standard_normal((r, r)) + 2 * np.eye(r)
+        A[k] = np.einsum("awb,bc->awc", A[k], G)
+        A[k + 1] = np.einsum("ab,bwc->awc", np.linalg.inv(G), A[k + 1])
+    want = O.round_mps(A, chi)
+    x = Q.qtt_mps_from_cores(ctx, A)
+    Q.qtt_round(ctx, x, chi)
+    assert Q.qtt_mps_bonds(x) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, x), O.to_dense(want)) < TOL
+    sg, so = Q.qtt_mps_schmidt(ctx, x), O.schmidt_values(want)
+    for k in range(1, n):
+        m = min(len(sg[k]), len(so[k]))
+        assert np.max(np.abs(sg[k][:m] - so[k][:m])) <= 1e-9 * so[k][0]
+    ms, hits = Q.qtt_ctx_jacobi_stats(ctx)
+    assert hits == 0
+
+
+@pytest.mark.parametrize("which", [0, 1, 2])
+def test_apply_then_round_matches_oracle(Q, ctx, which):
+    n, chi = 7, 12
+    g, o = ops(Q, ctx, n)
+    F = smooth_field(n, 21)
+    A = O.from_dense(F, chi)
+    want = O.round_mps(O.apply_mpo(o[which], A), chi)
+    x = Q.qtt_mps_from_cores(ctx, A)
+    y = Q.qtt_apply_mpo(ctx, g[which], x)
+    Q.qtt_round(ctx, y, chi)
+    assert Q.qtt_mps_bonds(y) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, y), O.to_dense(want)) < TOL
+
+
+def test_round_eps_rule_matches_oracle(Q, ctx):
+    n = 6
+    F = smooth_field(n, 5)
+    A = O.lincomb([(1.0, O.from_dense(F, 20)), (0.5, O.from_dense(F.T.copy(), 20))])
+    for eps in (1e-1, 1e-3, 1e-6):
+        want = O.round_mps(A, 1 << 20, eps)
+        x = Q.qtt_mps_from_cores(ctx, A)
+        Q.qtt_round(ctx, x, 1 << 20, eps)
+        assert Q.qtt_mps_bonds(x) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, x), O.to_dense(want)) < TOL
+
+
+def test_round_batch_mixed_operands(Q, ctx):
+    n, chi = 6, 8
+    g, o = ops(Q, ctx, n)
+    A = O.from_dense(smooth_field(n, 1), chi)
+    B = O.from_dense(smooth_field(n, 2), chi)
+    a, b = Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B)
+    xs = [Q.qtt_apply_mpo(ctx, g[0], a), Q.qtt_hadamard(ctx, a, b), Q.qtt_apply_mpo(ctx, g[2], b)]
+    s = Q.qtt_mps_clone(ctx, a)
+    Q.qtt_axpy(ctx, 3.0, b, s)
+    xs.append(s)
+    Q.qtt_round_batch(ctx, xs, chi)
+    wants = [O.round_mps(O.apply_mpo(o[0], A), chi), O.round_product(A, B, chi),
+             O.round_mps(O.apply_mpo(o[2], B), chi), O.round_mps(O.lincomb([(3.0, B), (1.0, A)]), chi)]
+    for x, w in zip(xs, wants):
+        assert Q.qtt_mps_bonds(x) == O.bonds(w)
+        assert rel(gpu_dense(Q, ctx, x), O.to_dense(w)) < TOL
+
+
+# ---------------------------------------------------------------- zip-up (fused Hadamard + round)
+@pytest.mark.parametrize("n,ca,cb,chi,cw", [(4, 3, 3, 4, 0), (5, 4, 3, 6, 0), (6, 6, 6, 8, 0), (6, 6, 6, 8, 8),
+                                            (7, 8, 8, 8, 12), (8, 16, 16, 16, 0)])
+def test_round_product_matches_oracle(Q, ctx, n, ca, cb, chi, cw):
+    A = O.from_dense(smooth_field(n, 31), ca)
+    B = O.from_dense(smooth_field(n, 32), cb)
+    want = O.round_product(A, B, chi, 0.0, cw if cw else None)
+    Q.qtt_ctx_set_chi_work(ctx, cw)
+    try:
+        a, b = Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B)
+        h = Q.qtt_hadamard(ctx, a, b)
+        Q.qtt_round(ctx, h, chi)
+    finally:
+        Q.qtt_ctx_set_chi_work(ctx, 0)
+    assert Q.qtt_mps_bonds(h) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, h), O.to_dense(want)) < TOL
+
+
+def test_config1_chain_matches_oracle_and_dense(Q, ctx):
+    """BASELINE config 1: 2^5 x 2^5, chi 8: from_dense -> apply d/dx -> Hadamard -> one round to 8."""
+    import torch
+    n, chi = 5, 8
+    F = I.config1_field(n, 0)
+    g, o = ops(Q, ctx, n)
+    A = O.from_dense(F, chi)
+    want = O.round_product(A, O.apply_mpo(o[0], A), chi, 0.0, 1 << 20)
+    u = Q.qtt_mps_from_dense(ctx, torch.from_numpy(F).cuda(), chi)
+    du = Q.qtt_apply_mpo(ctx, g[0], u)
+    w = Q.qtt_hadamard(ctx, u, du)
+    # exact product (bond 192) against the dense 32 x 32 brute force
+    u8 = O.to_dense(A)
+    dx = 1.0 / 32
+    dense = u8 * (np.roll(u8, -1, 0) - np.roll(u8, 1, 0)) / (2 * dx)
+    # noise-dominated result: d/dx of the tanh(y) part cancels, so rounding is amplified by
+    # ||u|| * (1/2dx) / ||w|| ~ 1e3 above machine epsilon
+    assert rel(gpu_dense(Q, ctx, w), dense) < 1e-11
+    Q.qtt_ctx_set_chi_work(ctx, 1 << 20)
+    try:
+        Q.qtt_round(ctx, w, chi)
+    finally:
+        Q.qtt_ctx_set_chi_work(ctx, 0)
+    assert Q.qtt_mps_bonds(w) == O.bonds(want)
+    assert rel(gpu_dense(Q, ctx, w), O.to_dense(want)) < TOL
+
+
+# ---------------------------------------------------------------- RK4
+@pytest.mark.parametrize("graphs", [False, True])
+def test_rk4_step_small_matches_oracle(Q, ctx, graphs):
+    n, chi, Re, dt = 6, 12, 100.0, 1e-3
+    g, o = ops(Q, ctx, n)
+    X, Y = I.grid(n)
+    ux = np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y) + 0.3 * smooth_field(n, 4)
+    uy = -np.cos(2 * np.pi * X) * np.sin(2 * np.pi * Y) + 0.3 * smooth_field(n, 5)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    Q.qtt_ctx_set_graphs(ctx, graphs)
+    u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+    for step in range(2):
+        U = O.rk4_step(U, o[0], o[1], o[2], Re, dt, chi)
+        Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], Re, dt, chi)
+        for i in range(2):
+            assert Q.qtt_mps_bonds(u[i]) == O.bonds(U[i])
+            assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U[i])) < TOL
+    Q.qtt_ctx_set_graphs(ctx, True)
+    assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+
+
+def test_rk4_config2_matches_oracle(Q, ctx):
+    """BASELINE config 2: 2^8 x 2^8 double shear layer, chi 32, Re 1e4, dt 1e-4, one step."""
+    import torch
+    cfg = I.CONFIGS[2]
+    n, chi = cfg["n"], cfg["chi"]
+    ux, uy = I.config_fields(2)
+    g, o = ops(Q, ctx, n)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
+    for i in range(2):
+        assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U[i])) < TOL
+    U1 = O.rk4_step(U, o[0], o[1], o[2], cfg["Re"], cfg["dt"], chi)
+    Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+    for i in range(2):
+        assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+        assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < TOL
+    assert Q.qtt_ctx_launch_count(ctx) > 0
+
+
+# ---------------------------------------------------------------- error behaviour
+def test_errors_are_status_codes(Q, ctx):
+    a = Q.qtt_mps_from_cores(ctx, I.random_cores(4, 3, seed=1))
+    b = Q.qtt_mps_from_cores(ctx, I.random_cores(5, 3, seed=1))
+    with pytest.raises(Q.QttError) as e:
+        Q.qtt_hadamard(ctx, a, b)
+    assert e.value.status == -2
+    with pytest.raises(Q.QttError):
+        Q.qtt_round(ctx, a, 0)
