@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- RK4 steps/s of the QTT/MPS time-step algebra on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one qtt_rk4_step (the whole hot path: 24 apply+round, 16 hadamard+round, 8+6+2 sum+round)
+on the synthetic decaying-jet workload of BASELINE.json configs[2] (2^10 x 2^10, chi = 64), the
+configuration the metric is quoted on.  One process per GPU; the path does not shard ("replicas only",
+DESIGN.md): with N > 1 every rank advances its own replica and value = N * K / max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the host cores on a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import qtt_inputs as I  # noqa: E402
+
+METRIC = "QTT RK4 steps/sec at 2^10x2^10, chi=64 fp64"
+UNIT = "steps/s"
+
+
+def workload(cfg: int):
+    c = I.CONFIGS[cfg]
+    name = {2: "config2 double shear layer", 3: "config3 decaying jet", 4: "config4 decaying turbulence"}[cfg]
+    desc = (f"{name}: 2^{c['n']}x2^{c['n']} grid ({c['n']} sites, d=4), chi_max={c['chi']}, chi_work={2 * c['chi']}, "
+            f"Re={c['Re']:g}, dt={c['dt']:g}, eps=0, one qtt_rk4_step per step")
+    return c, desc
+
+
+# ------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200", "-i",
+                 str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------- CPU oracle leg
+def oracle_sample_seconds(cfg: int, state=None):
+    """Times a bounded sample of one RK4 step with the oracle as it stands: ONE of the four rhs evaluations
+    (6 apply+round, 4 hadamard+round, 2 three-term sums) plus ONE of the four stage combinations, and
+    extrapolates one step as 4 x that sample.  Returns (seconds per extrapolated step, description, state)."""
+    from oracle import qtt_oracle as O
+    c, _ = workload(cfg)
+    n, chi = c["n"], c["chi"]
+    if state is None:
+        ux, uy = I.config_fields(cfg)
+        dx = 1.0 / (1 << n)
+        state = dict(U=[O.from_dense(ux, chi), O.from_dense(uy, chi)], Dx=O.mpo_d1(n, dx), Dy=O.mpo_d2(n, dx),
+                     Lap=O.mpo_laplacian(n, dx))
+    U = state["U"]
+    t0 = time.perf_counter()
+    k1 = O.rhs(U, state["Dx"], state["Dy"], state["Lap"], c["Re"], chi)
+    U2 = [O.round_mps(O.lincomb([(1.0, U[i]), (c["dt"] / 2, k1[i])]), chi) for i in range(2)]
+    t = time.perf_counter() - t0
+    state["U"] = U2  # the next sample continues from the half-step state
+    return 4.0 * t, "1 of the 4 rhs evaluations + 1 of the 4 stage combinations of one RK4 step, x4", state
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    c, desc = workload(args.config)
+    state = None
+    for _ in range(args.warmup):
+        _, _, state = oracle_sample_seconds(args.config, state)
+    tot, sample = 0.0, ""
+    for _ in range(args.steps):
+        s, sample, state = oracle_sample_seconds(args.config, state)
+        tot += s
+    sec = tot / max(args.steps, 1)
+    val = 1.0 / sec
+    cores = blas_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc, "note": "CPU oracle (NumPy fp64 + LAPACK) on the host cores; each step is a "
+                   "bounded sample extrapolated to one RK4 step"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def fp64_peaks(Q, ctx):
+    """Measured fp64 issue rates of this GPU (TFLOP/s): the DMMA.8x8x4 tensor pipe and the DFMA pipe."""
+    import ctypes as C
+    out = {}
+    for kind, name in ((0, "dmma"), (1, "dfma")):
+        t = C.c_double()
+        rc = ctx.lib.qtt_diag_fp64_probe(C.c_void_p(ctx.stream.cuda_stream), kind, 148 * 8, 2000, C.byref(t))
+        out[name] = t.value if rc == 0 else None
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2406_17823_b200 as Q
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    c, desc = workload(args.config)
+    n, chi = c["n"], c["chi"]
+    ctx = Q.Context(device=local, workspace_bytes=int(args.workspace_gib * (1 << 30)))
+    dx = 1.0 / (1 << n)
+    Dx, Dy = Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx)
+    Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
+    ux, uy = I.config_fields(args.config, seed=rank)
+    u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
+    ctx.synchronize()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    def step():
+        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    launches0 = Q.qtt_ctx_launch_count(ctx)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    with torch.cuda.stream(ctx.stream):
+        for e0, e1 in ev:
+            flush.zero_()  # L2 flush between timed iterations, outside the per-step event pair
+            e0.record(ctx.stream)
+            step()
+            e1.record(ctx.stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
+    launches = Q.qtt_ctx_launch_count(ctx) - launches0
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = world * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: cores in pinned host memory -> device, step, cores back
+    host = [Q.qtt_mps_get_cores(ctx, x) for x in u]
+    h2d = sum(a.nbytes for cs in host for a in cs)
+    e2e_steps = max(1, min(args.steps, 5))
+    barrier()
+    t0 = time.perf_counter()
+    d2h = 0
+    for _ in range(e2e_steps):
+        v = [Q.qtt_mps_from_cores(ctx, cs) for cs in host]
+        Q.qtt_rk4_step(ctx, v, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+        host = [Q.qtt_mps_get_cores(ctx, x) for x in v]
+        d2h = sum(a.nbytes for cs in host for a in cs)
+    torch.cuda.synchronize()
+    e2e_sec = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_sec], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_sec = float(t.item())
+    e2e = {"value": world / e2e_sec, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+           "steps": e2e_steps}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc, "l2": "256 MiB buffer zeroed between timed steps, outside the per-step CUDA "
+                   "event pairs; ms_per_step = sum of the per-step event times / steps",
+                   "graph": "whole RK4 step replayed as one CUDA graph", "parallelism": "replicas only"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+    }
+    if rank == 0:
+        line.update(roofline_and_baseline(Q, ctx, u, (Dx, Dy, Lap), c, chi, args, ms_per_step))
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
+    """Per-kernel-family device times of one more (eagerly launched, event-bracketed) step -> roofline of the
+    dominant family; the site-contraction TFLOP/s; and the CPU oracle timed on a bounded sample."""
+    Dx, Dy, Lap = ops
+    peaks = fp64_peaks(Q, ctx)
+    Q.qtt_ctx_profile(ctx, True)
+    Q.qtt_ctx_profile_report(ctx)  # clear
+    nprof = 2
+    for _ in range(nprof):
+        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+    rep = Q.qtt_ctx_profile_report(ctx)
+    Q.qtt_ctx_profile(ctx, False)
+    tot_ms = sum(v["ms"] for v in rep.values()) or 1.0
+    fams = {}
+    for k, v in rep.items():
+        fams[k] = {"ms_per_step": v["ms"] / nprof, "launches_per_step": v["launches"] // nprof,
+                   "share": v["ms"] / tot_ms,
+                   "work_per_step": v["work"] / nprof}
+    dom = max(rep, key=lambda k: rep[k]["ms"])
+    d = rep[dom]
+    bound = {"gemm": "tensor", "lq_panel": "alu", "lq_update": "alu", "rowjacobi": "alu", "select": "hbm",
+             "move": "hbm"}[dom]
+    if bound == "hbm":
+        try:
+            peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+            src = "MEASURED_PEAKS.json hbm_gbs (of measured)"
+        except Exception:
+            peak, src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
+        achieved = d["work"] / (d["ms"] * 1e-3) * 1e-9
+        unit = "GB/s"
+    else:
+        peak = peaks["dmma"] if bound == "tensor" else peaks["dfma"]
+        src = ("qtt_diag_fp64_probe, measured in this run: register-only " +
+               ("DMMA.8x8x4" if bound == "tensor" else "DFMA") + " issue rate (MEASURED_PEAKS.json has no fp64 figure)")
+        achieved = d["work"] / (d["ms"] * 1e-3) * 1e-12
+        unit = "TFLOP/s"
+    roof = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
+            "frac": achieved / peak if peak else None, "traffic": None, "peak_source": src,
+            "launches_per_step": d["launches"] // nprof, "avg_launch_ms": d["ms"] / max(d["launches"], 1),
+            "share_of_step_kernel_time": d["ms"] / tot_ms,
+            "algorithmic_work": "nominal SVD count 6ab^2+20b^3 per matrix (DESIGN.md)" if dom == "rowjacobi" else
+            "DESIGN.md per-family formulas"}
+    g = rep["gemm"]
+    out = {"roofline": roof, "families": fams,
+           "contraction": {"tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],
+                           "frac": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,
+                           "what": "sum 2MNK of all DMMA site-contraction GEMMs of a step / their summed kernel time"},
+           "fp64_peaks_tflops": peaks,
+           "step_flop_model": {"kernel_time_sum_ms": tot_ms / nprof, "graph_ms_per_step": ms_per_step}}
+    if int(os.environ.get("WORLD_SIZE", "1")) == 1 and not args.no_cpu_baseline:
+        sec, sample, _ = oracle_sample_seconds(args.config)
+        out["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                               "sample": sample, "seconds_per_step_extrapolated": sec}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=(2, 3, 4))
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--workspace-gib", type=float, default=8.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -37,6 +37,8 @@ PROTOTYPES = {
     "qtt_ctx_set_graphs": (C.c_int, [_P, C.c_int]),
     "qtt_ctx_jacobi_stats": (C.c_int, [_P, _IP, _IP]),
     "qtt_ctx_launch_count": (C.c_longlong, [_P]),
+    "qtt_ctx_profile": (C.c_int, [_P, C.c_int]),
+    "qtt_ctx_profile_report": (C.c_int, [_P, _DP, _DP, C.POINTER(C.c_longlong)]),
     "qtt_mps_from_dense": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_double, _PP]),
     "qtt_mps_from_cores": (C.c_int, [_P, C.c_int, _IP, _DPP, _PP]),
     "qtt_to_dense": (C.c_int, [_P, _P, _P]),

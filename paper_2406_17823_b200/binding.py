@@ -267,3 +267,18 @@ def qtt_ctx_jacobi_stats(ctx: Context) -> tuple[int, int]:
 
 def qtt_ctx_launch_count(ctx: Context) -> int:
     return int(ctx.lib.qtt_ctx_launch_count(ctx.h))
+
+
+PROF_FAMILIES = ("gemm", "lq_panel", "lq_update", "rowjacobi", "select", "move")
+
+
+def qtt_ctx_profile(ctx: Context, enabled: bool) -> None:
+    ctx.check(ctx.lib.qtt_ctx_profile(ctx.h, 1 if enabled else 0))
+
+
+def qtt_ctx_profile_report(ctx: Context) -> dict:
+    """{family: {"ms": kernel milliseconds, "work": flops or bytes, "launches": count}} since the last report."""
+    n = len(PROF_FAMILIES)
+    ms, work, cnt = (C.c_double * n)(), (C.c_double * n)(), (C.c_longlong * n)()
+    ctx.check(ctx.lib.qtt_ctx_profile_report(ctx.h, ms, work, cnt))
+    return {f: {"ms": ms[i], "work": work[i], "launches": int(cnt[i])} for i, f in enumerate(PROF_FAMILIES)}

@@ -318,6 +318,20 @@ qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits) 
   if (h[1] > 0) QTT_THROW(QTT_NUMERIC, "Jacobi sweep limit hit");
   QTT_API_END(ctx)
 }
+qtt_status qtt_ctx_profile(qtt_ctx* ctx, int enabled) {
+  if (!ctx) return QTT_INVALID_ARG;
+  ctx->profiling = enabled ? 1 : 0;
+  qtt_prof_enable(enabled != 0);
+  return QTT_OK;
+}
+qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_host, long long* launches_host) {
+  if (!ctx || !ms_host || !work_host || !launches_host) return QTT_INVALID_ARG;
+  static_assert(QK_COUNT == QTT_PROF_FAMILIES, "family count");
+  QTT_API_BEGIN
+  set_device(ctx);
+  QTT_CU(qtt_prof_collect(ms_host, work_host, launches_host));
+  QTT_API_END(ctx)
+}
 long long qtt_ctx_launch_count(const qtt_ctx* ctx) { return g_qtt_launch_count + (ctx ? ctx->graph_launches : 0); }
 
 // ------------------------------------------------------------------------------------------ MPS / MPO
@@ -598,7 +612,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
   const int cw = ctx->chi_work > 0 ? ctx->chi_work : 2 * chi_max;
   ArenaScope scope(ctx);
 
-  if (eps > 0.0 || !ctx->graphs) {
+  if (eps > 0.0 || !ctx->graphs || ctx->profiling) {
     // eager path (eps > 0 synchronises once per bond)
     View uv[2] = {materialize(ctx, u[0]->body), materialize(ctx, u[1]->body)};
     std::vector<int> rin[2] = {uv[0].r, uv[1].r}, rout[2];

@@ -142,3 +142,18 @@ cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t strea
 // Number of kernels enqueued by the launchers above (qtt_ctx_launch_count).
 extern long long g_qtt_launch_count;
 void qtt_kernels_init();
+
+// Per-family kernel timing (qtt_ctx_profile_*): when enabled, every launch is bracketed by a CUDA event
+// pair on its stream.  Must be off while a stream is being captured.
+enum QttKernelFamily { QK_GEMM = 0, QK_LQ_PANEL, QK_LQ_UPDATE, QK_JACOBI, QK_SELECT, QK_MOVE, QK_COUNT };
+struct QttProf {
+  int fam;
+  cudaStream_t st;
+  bool live;
+  // work: algorithmic flops (GEMM, LQ, Jacobi) or bytes (select, move) of this launch
+  QttProf(int family, cudaStream_t stream, double work);
+  ~QttProf();
+};
+void qtt_prof_enable(bool on);
+// Synchronises the device, sums the event pairs recorded so far and clears them.
+cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]);

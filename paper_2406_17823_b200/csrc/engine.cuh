@@ -86,6 +86,7 @@ struct qtt_ctx {
   int chi_work = 0;
   size_t mat_limit = (size_t)2 << 30;
   int graphs = 1;
+  int profiling = 0;
   double* ones = nullptr;   // device: 1.0
   int* jac_status = nullptr;  // device: [max sweeps, limit hits]
   long long graph_launches = 0;

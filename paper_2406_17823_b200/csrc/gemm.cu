@@ -242,8 +242,12 @@ cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream) {
   }
   grp.total_tiles = t;
   if (t == 0) return cudaSuccess;
-  qtt_gemm_dmma_kernel<BM, BN, WM, WN><<<t, NT, SMEM, stream>>>(grp);
-  ++g_qtt_launch_count;
+  double flops = 0.0;
+  for (int i = 0; i < grp.nprob; ++i) flops += 2.0 * grp.p[i].M * grp.p[i].N * (double)grp.p[i].K * grp.p[i].nbatch;
+  {
+    QttProf prof(QK_GEMM, stream, flops);
+    qtt_gemm_dmma_kernel<BM, BN, WM, WN><<<t, NT, SMEM, stream>>>(grp);
+  }
   return cudaGetLastError();
 }
 

@@ -193,6 +193,287 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
 }
 
 // ------------------------------------------------------------------------------------------------
+// Two-level block Jacobi, the production path for every matrix whose row blocks fit in a cluster's
+// shared memory.  The p rows are cut into 2C blocks of b rows; every CTA of the cluster (C CTAs) holds
+// two blocks with their FULL rows, so a rotation needs no cross-CTA reduction at all:
+//   sweep = intra-block pairs of the two resident blocks (b-1 rounds)
+//         + 2C-1 outer rounds of a round-robin tournament over the blocks; in each, the CTA meets
+//           every row of its "top" block with every row of its "bot" block (b inner rounds of b
+//           disjoint pairs, one lane group per pair, the top row kept in registers), then the blocks
+//           move one seat through distributed shared memory (pull into a spare slot, two
+//           cluster.syncs, relabel the slots -- no copy inside a CTA).
+// Every pair of rows meets exactly once per sweep, as in the cyclic one-sided Jacobi method.
+constexpr int BJ_NT = 512;
+
+template <int G, int EPL>
+struct PairOps {
+  // reduce (aa, bb, ab) over the G lanes of a group
+  static __device__ __forceinline__ void reduce(double& aa, double& bb, double& ab) {
+#pragma unroll
+    for (int o = G >> 1; o > 0; o >>= 1) {
+      aa += __shfl_xor_sync(0xffffffffu, aa, o);
+      bb += __shfl_xor_sync(0xffffffffu, bb, o);
+      ab += __shfl_xor_sync(0xffffffffu, ab, o);
+    }
+  }
+  // rotation (c, s) that orthogonalises two rows with Gram entries (aa, bb, ab); returns false if none is needed
+  static __device__ __forceinline__ bool rotation(double aa, double bb, double ab, double tol2, double floor2,
+                                                  double& c, double& s) {
+    c = 1.0;
+    s = 0.0;
+    if (!(ab * ab > tol2 * aa * bb) || !(aa > floor2) || !(bb > floor2)) return false;
+    const double zeta = (bb - aa) / (2.0 * ab);
+    const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+    c = rsqrt(1.0 + t * t);
+    c = c * (1.5 - 0.5 * (1.0 + t * t) * c * c);  // one Newton step: full fp64 accuracy
+    s = c * t;
+    return s != 0.0;
+  }
+};
+
+template <int G, int EPL>
+__global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_constant__ JacGroup g, int b, int pitch) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = g.cluster;
+  const int rank = (C > 1) ? (int)cluster.block_rank() : 0;
+  const JacProb& P = g.p[blockIdx.x / C];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int p = P.p, q = P.q;
+  constexpr int NGRP = BJ_NT / G;
+  const int grp = tid / G, gl = tid % G;
+  const int ne = pitch / G;  // elements per lane actually used (<= EPL)
+
+  extern __shared__ __align__(16) double sm[];
+  const size_t slot_sz = (size_t)b * pitch;
+  double* xch = sm + 3 * slot_sz;                              // [MAXC] partial sums / rotation counts from peers
+  int* cnt = reinterpret_cast<int*>(xch + 2 * MAXC);           // [0] rotations of this CTA in this sweep
+  int top_s = 0, bot_s = 1, spare_s = 2;
+  auto slot = [&](int sidx) { return sm + (size_t)sidx * slot_sz; };
+
+  // ---- load: block k holds rows [k b, (k+1) b); CTA c starts with top = block c, bot = block 2C-1-c
+  double fro = 0.0;
+  for (int which = 0; which < 2; ++which) {
+    const int blk = which == 0 ? rank : 2 * C - 1 - rank;
+    double* S = slot(which == 0 ? top_s : bot_s);
+    for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
+      const int r = idx / pitch, x = idx - r * pitch;
+      const int gr = blk * b + r;
+      double v = 0.0;
+      if (gr < p && x < q) v = P.X[(i64)gr * P.ld + x];
+      S[idx] = v;
+      fro += v * v;
+    }
+  }
+  // Frobenius norm^2 over the cluster -> noise floor (rows below eps * ||X||_F / sqrt(p) are zero to
+  // working accuracy; they cannot all be made mutually orthogonal when p > rank)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) fro += __shfl_xor_sync(0xffffffffu, fro, o);
+  if (tid == 0) cnt[0] = 0;
+  if (tid < 2 * MAXC) xch[tid] = 0.0;
+  __syncthreads();
+  if (lane == 0) atomicAdd(&xch[MAXC + rank], fro);  // own partial, slot [MAXC + rank]
+  __syncthreads();
+  if (C > 1) {
+    cluster.sync();  // peers have zeroed their xch
+    if (tid < C && tid != rank) {
+      double* remote = cluster.map_shared_rank(xch, tid);
+      remote[MAXC + rank] = xch[MAXC + rank];
+    }
+    cluster.sync();
+  }
+  double fro2 = 0.0;
+  for (int c2 = 0; c2 < C; ++c2) fro2 += xch[MAXC + c2];
+  const double floor2 = 4.930380657631324e-32 * fro2 / (double)p;
+  const double tol = 2.220446049250313e-16 * sqrt((double)q);
+  const double tol2 = tol * tol;
+  __syncthreads();
+
+  const int be = b + (b & 1);  // players of the intra-block tournament
+  int sweep = 0, hit_limit = 0;
+  int myrot = 0;
+  for (; sweep < g.max_sweeps; ++sweep) {
+    // ---- intra-block pairs of both resident blocks
+    for (int round = 0; round < be - 1; ++round) {
+      for (int k0 = 0; k0 < be; k0 += NGRP) {  // be pairs in all: be/2 per block
+        const int kk = k0 + grp;
+        int ia = b, ib = b;
+        double* S = slot(top_s);
+        if (kk < be) {
+          const int k = kk % (be / 2);
+          S = slot(kk < be / 2 ? top_s : bot_s);
+          if (k == 0) {
+            ia = be - 1;
+            ib = round;
+          } else {
+            ia = (round + k) % (be - 1);
+            ib = (round - k + (be - 1)) % (be - 1);
+          }
+        }
+        const bool live = ia < b && ib < b;
+        double a[EPL], v[EPL];
+        double aa = 0.0, bb = 0.0, ab = 0.0;
+        if (live) {
+          const double* ra = S + (size_t)ia * pitch + gl;
+          const double* rb = S + (size_t)ib * pitch + gl;
+#pragma unroll
+          for (int e = 0; e < EPL; ++e)
+            if (e < ne) {
+              a[e] = ra[e * G];
+              v[e] = rb[e * G];
+              aa += a[e] * a[e];
+              bb += v[e] * v[e];
+              ab += a[e] * v[e];
+            }
+        }
+        PairOps<G, EPL>::reduce(aa, bb, ab);
+        double c, s;
+        if (live && PairOps<G, EPL>::rotation(aa, bb, ab, tol2, floor2, c, s)) {
+          double* ra = S + (size_t)ia * pitch + gl;
+          double* rb = S + (size_t)ib * pitch + gl;
+#pragma unroll
+          for (int e = 0; e < EPL; ++e)
+            if (e < ne) {
+              ra[e * G] = c * a[e] - s * v[e];
+              rb[e * G] = s * a[e] + c * v[e];
+            }
+          if (gl == 0) ++myrot;
+        }
+      }
+      __syncthreads();
+    }
+    // ---- tournament over the 2C blocks
+    for (int t = 0; t < 2 * C - 1; ++t) {
+      double* T = slot(top_s);
+      double* B = slot(bot_s);
+      for (int i0 = 0; i0 < b; i0 += NGRP) {
+        const int i = i0 + grp;
+        const bool have = i < b;
+        double a[EPL];
+        if (have) {
+#pragma unroll
+          for (int e = 0; e < EPL; ++e)
+            if (e < ne) a[e] = T[(size_t)i * pitch + gl + e * G];
+        }
+        for (int r = 0; r < b; ++r) {
+          const int j = have ? (i + r) % b : 0;
+          double v[EPL];
+          double aa = 0.0, bb = 0.0, ab = 0.0;
+          if (have) {
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+              if (e < ne) {
+                v[e] = B[(size_t)j * pitch + gl + e * G];
+                aa += a[e] * a[e];
+                bb += v[e] * v[e];
+                ab += a[e] * v[e];
+              }
+          }
+          PairOps<G, EPL>::reduce(aa, bb, ab);
+          double c, s;
+          if (have && PairOps<G, EPL>::rotation(aa, bb, ab, tol2, floor2, c, s)) {
+#pragma unroll
+            for (int e = 0; e < EPL; ++e)
+              if (e < ne) {
+                const double an = c * a[e] - s * v[e];
+                B[(size_t)j * pitch + gl + e * G] = s * a[e] + c * v[e];
+                a[e] = an;
+              }
+            if (gl == 0) ++myrot;
+          }
+          __syncthreads();
+        }
+        if (have) {
+#pragma unroll
+          for (int e = 0; e < EPL; ++e)
+            if (e < ne) T[(size_t)i * pitch + gl + e * G] = a[e];
+        }
+      }
+      __syncthreads();
+      if (C == 1) break;
+      // ---- move the blocks one seat (labels of every peer are a function of the round number only)
+      const int tt = sweep * (2 * C - 1) + t;  // exchanges done so far
+      // peer labelling after tt relabels: CTA 0: top fixed at slot 0, (bot, spare) = tt even ? (1, 2) : (2, 1);
+      // CTA c >= 1: (top, bot, spare) = cyclic shifts of (0, 1, 2): top = (3 - tt % 3) % 3 ... computed below
+      auto peer_top = [&](int c2) { return c2 == 0 ? 0 : (2 * tt) % 3; };
+      auto peer_bot = [&](int c2) { return c2 == 0 ? ((tt & 1) ? 2 : 1) : (2 * tt + 1) % 3; };
+      cluster.sync();  // every CTA has finished rotating its blocks
+      // phase 1: new top <- old top of the left neighbour (CTA 1: old bot of CTA 0) into my spare slot
+      if (rank >= 1) {
+        const int src = rank - 1;
+        const int ss = (rank == 1) ? peer_bot(0) : peer_top(src);
+        const double* remote = cluster.map_shared_rank(sm + (size_t)ss * slot_sz, src);
+        double* dst = slot(spare_s);
+        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
+          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
+      }
+      cluster.sync();
+      // phase 2: new bot <- old bot of the right neighbour (last CTA: its own old top, a relabel)
+      if (rank <= C - 2) {
+        const int src = rank + 1;
+        const double* remote = cluster.map_shared_rank(sm + (size_t)peer_bot(src) * slot_sz, src);
+        double* dst = slot(rank == 0 ? spare_s : top_s);
+        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
+          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
+      }
+      cluster.sync();
+      if (rank == 0) {
+        const int ob = bot_s;
+        bot_s = spare_s;
+        spare_s = ob;
+      } else {
+        const int ot = top_s, ob = bot_s;
+        top_s = spare_s;
+        bot_s = ot;
+        spare_s = ob;
+      }
+    }
+    // ---- rotations of this sweep over the whole cluster
+    {
+      int r2 = myrot;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+      if (lane == 0 && r2) atomicAdd(&cnt[0], r2);
+      myrot = 0;
+    }
+    __syncthreads();
+    int total = cnt[0];
+    if (C > 1) {
+      const int par = sweep & 1;
+      if (tid < C) {
+        double* remote = cluster.map_shared_rank(xch, tid);
+        remote[par * MAXC + rank] = (double)cnt[0];
+      }
+      cluster.sync();
+      total = 0;
+      for (int c2 = 0; c2 < C; ++c2) total += (int)xch[par * MAXC + c2];
+    }
+    __syncthreads();
+    if (tid == 0) cnt[0] = 0;
+    __syncthreads();
+    if (total == 0) {
+      ++sweep;
+      break;
+    }
+    if (sweep + 1 == g.max_sweeps) hit_limit = 1;
+  }
+  // ---- after whole sweeps every block is back in its first seat
+  for (int which = 0; which < 2; ++which) {
+    const int blk = which == 0 ? rank : 2 * C - 1 - rank;
+    const double* S = slot(which == 0 ? top_s : bot_s);
+    for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
+      const int r = idx / pitch, x = idx - r * pitch;
+      const int gr = blk * b + r;
+      if (gr < p && x < q) P.X[(i64)gr * P.ld + x] = S[idx];
+    }
+  }
+  if (rank == 0 && tid == 0 && P.status) {
+    atomicMax(&P.status[0], sweep);
+    if (hit_limit) atomicAdd(&P.status[1], 1);
+  }
+  if (C > 1) cluster.sync();
+}
+
+// ------------------------------------------------------------------------------------------------
 // select: sort rows by norm (bitonic in shared memory), rank rule, normalised top rows.
 constexpr int SNT = 256;
 constexpr int SEL_MAXP = 2048;
@@ -289,7 +570,98 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
 
 }  // namespace
 
+namespace {
+template <int G, int EPL>
+cudaError_t launch_blockjacobi(JacGroup& grp, int b, int pitch, size_t smem, double flops, cudaStream_t stream) {
+  static bool attr_done = false;
+  if (!attr_done) {
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<G, EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        224 * 1024));
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<G, EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    attr_done = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grp.cluster * grp.nprob);
+  cfg.blockDim = dim3(BJ_NT);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = grp.cluster;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  QttProf prof(QK_JACOBI, stream, flops);
+  return cudaLaunchKernelEx(&cfg, qtt_blockjacobi_kernel<G, EPL>, grp, b, pitch);
+}
+
+// Block-Jacobi configuration for a group with largest shape pmax x qmax; false if it does not fit.
+bool blockjacobi_config(int pmax, int qmax, int& G, int& EPL, int& C, int& b, int& pitch, size_t& smem) {
+  if (qmax <= 128) { G = 16; EPL = 8; }
+  else if (qmax <= 256) { G = 16; EPL = 16; }
+  else if (qmax <= 512) { G = 32; EPL = 16; }
+  else return false;
+  pitch = ((qmax + G - 1) / G) * G;
+  C = pmax / 16;
+  C = C < 1 ? 1 : (C > MAXC ? MAXC : C);
+  for (;;) {
+    b = (pmax + 2 * C - 1) / (2 * C);
+    smem = ((size_t)3 * b * pitch + 2 * MAXC + 2) * sizeof(double);
+    if (smem <= 220 * 1024) return true;
+    if (C == MAXC) return false;
+    C = C * 2 > MAXC ? MAXC : C * 2;
+  }
+}
+}  // namespace
+
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream) {
+  // production path: two-level block Jacobi, problems grouped as they come (same-site operands share a shape)
+  {
+    int done = 0;
+    bool all_fit = true;
+    for (int i = 0; i < n && all_fit; ++i) {
+      int G, EPL, C, b, pitch;
+      size_t smem;
+      if (probs[i].p >= 2 && probs[i].q >= 1 && !blockjacobi_config(probs[i].p, probs[i].q, G, EPL, C, b, pitch, smem))
+        all_fit = false;
+    }
+    if (all_fit) {
+      while (done < n) {
+        JacGroup grp;
+        grp.nprob = 0;
+        int pmax = 0, qmax = 0;
+        double flops = 0.0;
+        while (done < n && grp.nprob < QTT_JAC_MAX_BATCH) {
+          const JacProb& pr = probs[done];
+          if (pr.p >= 2 && pr.q >= 1) {
+            // keep a group to one (G, EPL) class and similar row counts so that padding stays small
+            if (grp.nprob > 0 && (pr.p != pmax || pr.q != qmax)) break;
+            grp.p[grp.nprob++] = pr;
+            pmax = pr.p;
+            qmax = pr.q;
+            double a = pr.p > pr.q ? pr.p : pr.q, bb = pr.p > pr.q ? pr.q : pr.p;
+            flops += 6.0 * a * bb * bb + 20.0 * bb * bb * bb;
+          }
+          ++done;
+        }
+        if (grp.nprob == 0) continue;
+        int G, EPL, C, b, pitch;
+        size_t smem;
+        blockjacobi_config(pmax, qmax, G, EPL, C, b, pitch, smem);
+        grp.cluster = C;
+        grp.use_smem = 1;
+        grp.wslice = 0;
+        grp.max_sweeps = 60;
+        cudaError_t e;
+        if (G == 16 && EPL == 8) e = launch_blockjacobi<16, 8>(grp, b, pitch, smem, flops, stream);
+        else if (G == 16) e = launch_blockjacobi<16, 16>(grp, b, pitch, smem, flops, stream);
+        else e = launch_blockjacobi<32, 16>(grp, b, pitch, smem, flops, stream);
+        if (e != cudaSuccess) return e;
+      }
+      return cudaSuccess;
+    }
+  }
   static bool attr_done = false;
   if (!attr_done) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_rowjacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
@@ -354,8 +726,15 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
     at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_rowjacobi_kernel, grp, pmax, wp));
-    ++g_qtt_launch_count;
+    double flops = 0.0;  // nominal SVD count 6 a b^2 + 20 b^3, a >= b (kernels)
+    for (int i = 0; i < grp.nprob; ++i) {
+      double a = grp.p[i].p > grp.p[i].q ? grp.p[i].p : grp.p[i].q, b = grp.p[i].p > grp.p[i].q ? grp.p[i].q : grp.p[i].p;
+      flops += 6.0 * a * b * b + 20.0 * b * b * b;
+    }
+    {
+      QttProf prof(QK_JACOBI, stream, flops);
+      QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_rowjacobi_kernel, grp, pmax, wp));
+    }
   }
   return cudaSuccess;
 }
@@ -368,8 +747,12 @@ cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream) 
       g.p[i] = probs[b0 + i];
       if (g.p[i].p > SEL_MAXP) return cudaErrorInvalidValue;
     }
-    qtt_select_kernel<<<g.nprob, SNT, 0, stream>>>(g);
-    ++g_qtt_launch_count;
+    double bytes = 0.0;
+    for (int i = 0; i < g.nprob; ++i) bytes += 8.0 * ((double)g.p[i].p * g.p[i].q + (double)g.p[i].r_cap * g.p[i].q);
+    {
+      QttProf prof(QK_SELECT, stream, bytes);
+      qtt_select_kernel<<<g.nprob, SNT, 0, stream>>>(g);
+    }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;

@@ -343,11 +343,20 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
       at[0].val.clusterDim.z = 1;
       cfg.attrs = at;
       cfg.numAttrs = 1;
-      QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
-      ++g_qtt_launch_count;
+      // Householder count of this panel step: panel 2 nb^2 mw, trailing update 4 nb mw rows_below
+      double fp = 0.0, fu = 0.0;
+      for (int i = 0; i < grp.nprob; ++i) {
+        const double mw = grp.p[i].m - p0, nbp = (grp.p[i].k - p0 < NB) ? grp.p[i].k - p0 : NB;
+        fp += 2.0 * nbp * nbp * mw;
+        fu += 4.0 * nbp * mw * (grp.p[i].k - p0 - nbp);
+      }
+      {
+        QttProf prof(QK_LQ_PANEL, stream, fp);
+        QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
+      }
       if (ctas > 0) {
+        QttProf prof(QK_LQ_UPDATE, stream, fu);
         qtt_lq_update_kernel<<<ctas, UPD_NT, 0, stream>>>(ug);
-        ++g_qtt_launch_count;
         QTT_CHECK_CUDA(cudaGetLastError());
       }
     }
@@ -367,8 +376,10 @@ cudaError_t qtt_launch_extract_tri(const TriProb* probs, int n, int mode, cudaSt
     }
     int bx = (int)(((i64)kmax * kmax + 255) / 256);
     bx = bx > 256 ? 256 : bx;
-    qtt_extract_tri_kernel<<<dim3(bx, g.nprob), 256, 0, stream>>>(g);
-    ++g_qtt_launch_count;
+    {
+      QttProf prof(QK_MOVE, stream, 16.0 * kmax * kmax * g.nprob);
+      qtt_extract_tri_kernel<<<dim3(bx, g.nprob), 256, 0, stream>>>(g);
+    }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;

@@ -159,8 +159,10 @@ cudaError_t qtt_launch_expand(const ExpandProb* probs, int n, cudaStream_t strea
       i64 sz = (i64)g.p[i].Dl * g.p[i].a * 4 * g.p[i].Dr * g.p[i].b;
       mx = sz > mx ? sz : mx;
     }
-    qtt_expand_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
-    ++g_qtt_launch_count;
+    {
+      QttProf prof(QK_MOVE, stream, 16.0 * (double)mx * g.nprob);
+      qtt_expand_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;
@@ -181,8 +183,10 @@ cudaError_t qtt_launch_concat(const ConcatProb* probs, int n, cudaStream_t strea
       i64 sz = RL * 4 * RR;
       mx = sz > mx ? sz : mx;
     }
-    qtt_concat_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
-    ++g_qtt_launch_count;
+    {
+      QttProf prof(QK_MOVE, stream, 16.0 * (double)mx * g.nprob);
+      qtt_concat_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;
@@ -198,16 +202,20 @@ cudaError_t qtt_launch_kron(const KronProb* probs, int n, cudaStream_t stream) {
       i64 sz = (i64)g.p[i].a * g.p[i].b * 4 * g.p[i].a2 * g.p[i].b2;
       mx = sz > mx ? sz : mx;
     }
-    qtt_kron_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
-    ++g_qtt_launch_count;
+    {
+      QttProf prof(QK_MOVE, stream, 8.0 * (double)mx * g.nprob);
+      qtt_kron_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+    }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;
 }
 
 cudaError_t qtt_launch_interleave(const double* src, double* dst, int nbits, int inverse, cudaStream_t stream) {
-  qtt_interleave_kernel<<<grid_for(1ll << (2 * nbits)), NT, 0, stream>>>(src, dst, nbits, inverse);
-  ++g_qtt_launch_count;
+  {
+    QttProf prof(QK_MOVE, stream, 16.0 * (double)(1ll << (2 * nbits)));
+    qtt_interleave_kernel<<<grid_for(1ll << (2 * nbits)), NT, 0, stream>>>(src, dst, nbits, inverse);
+  }
   return cudaGetLastError();
 }
 
@@ -216,22 +224,28 @@ cudaError_t qtt_launch_transpose(const double* src, int rows, int cols, int lds,
   if (rows <= 0 || cols <= 0) return cudaSuccess;
   dim3 grid((rows + 31) / 32, (cols + 31) / 32);
   if (grid.y > 65535) return cudaErrorInvalidValue;
-  qtt_transpose_kernel<<<grid, dim3(32, 8), 0, stream>>>(src, rows, cols, lds, dst, ldd);
-  ++g_qtt_launch_count;
+  {
+    QttProf prof(QK_MOVE, stream, 16.0 * (double)rows * cols);
+    qtt_transpose_kernel<<<grid, dim3(32, 8), 0, stream>>>(src, rows, cols, lds, dst, ldd);
+  }
   return cudaGetLastError();
 }
 
 cudaError_t qtt_launch_copy2d(const double* src, int rows, int cols, int lds, double* dst, int ldd,
                               cudaStream_t stream) {
   if (rows <= 0 || cols <= 0) return cudaSuccess;
-  qtt_copy2d_kernel<<<grid_for((i64)rows * cols), NT, 0, stream>>>(src, rows, cols, lds, dst, ldd);
-  ++g_qtt_launch_count;
+  {
+    QttProf prof(QK_MOVE, stream, 16.0 * (double)rows * cols);
+    qtt_copy2d_kernel<<<grid_for((i64)rows * cols), NT, 0, stream>>>(src, rows, cols, lds, dst, ldd);
+  }
   return cudaGetLastError();
 }
 
 cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t stream) {
   if (n <= 0) return cudaSuccess;
-  qtt_fill_kernel<<<grid_for(n), NT, 0, stream>>>(dst, n, value);
-  ++g_qtt_launch_count;
+  {
+    QttProf prof(QK_MOVE, stream, 8.0 * (double)n);
+    qtt_fill_kernel<<<grid_for(n), NT, 0, stream>>>(dst, n, value);
+  }
   return cudaGetLastError();
 }

@@ -2,6 +2,7 @@
 // fp64 roofline (MEASURED_PEAKS.json carries no fp64 figure), and the one-time
 // kernel attribute setup.
 #include <cstdio>
+#include <vector>
 
 #include "../../include/qtt_diag.h"
 #include "common.cuh"
@@ -50,6 +51,47 @@ __global__ void __launch_bounds__(256) qtt_probe_dfma_kernel(int iters, double* 
 }  // namespace
 
 long long g_qtt_launch_count = 0;
+
+// ------------------------------------------------------------------------------------------ profiler
+namespace {
+struct ProfRec { int fam; cudaEvent_t e0, e1; double work; };
+bool g_prof_on = false;
+std::vector<ProfRec> g_prof;
+}  // namespace
+
+QttProf::QttProf(int family, cudaStream_t stream, double work) : fam(family), st(stream), live(g_prof_on) {
+  ++g_qtt_launch_count;
+  if (!live) return;
+  ProfRec r;
+  r.fam = fam;
+  r.work = work;
+  if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) {
+    live = false;
+    return;
+  }
+  cudaEventRecord(r.e0, st);
+  g_prof.push_back(r);
+}
+QttProf::~QttProf() {
+  if (live) cudaEventRecord(g_prof.back().e1, st);
+}
+void qtt_prof_enable(bool on) { g_prof_on = on; }
+cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]) {
+  for (int i = 0; i < QK_COUNT; ++i) ms[i] = work[i] = 0.0, launches[i] = 0;
+  cudaError_t e = cudaDeviceSynchronize();
+  for (ProfRec& r : g_prof) {
+    float t = 0.f;
+    if (e == cudaSuccess && cudaEventElapsedTime(&t, r.e0, r.e1) == cudaSuccess) {
+      ms[r.fam] += t;
+      work[r.fam] += r.work;
+      launches[r.fam] += 1;
+    }
+    cudaEventDestroy(r.e0);
+    cudaEventDestroy(r.e1);
+  }
+  g_prof.clear();
+  return e;
+}
 
 void qtt_kernels_init() {}
 

@@ -141,7 +141,7 @@ def test_rowjacobi_gives_singular_values_and_orthogonal_rows(env, p, q, batch):
     stream.synchronize()
     Z = dX.cpu().numpy()
     stt = status.cpu().numpy()
-    assert stt[1] == 0 and 1 <= stt[0] <= 40
+    assert stt[1] == 0 and 1 <= stt[0] <= 60
     for b in range(batch):
         s = np.sort(np.linalg.norm(Z[b], axis=1))[::-1]
         want = np.linalg.svd(X[b], compute_uv=False)
