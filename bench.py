@@ -279,7 +279,7 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     dom = max(rep, key=lambda k: rep[k]["ms"])
     d = rep[dom]
     bound = {"gemm": "tensor", "lq_panel": "alu", "lq_update": "alu", "rowjacobi": "alu", "select": "hbm",
-             "move": "hbm"}[dom]
+             "move": "hbm", "qrcp": "alu"}[dom]
     if bound == "hbm":
         try:
             peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]

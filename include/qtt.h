@@ -72,10 +72,11 @@ qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits);
 /* Per-kernel-family device timing for bench.py's roofline.  While enabled, every kernel launch is bracketed
  * by a CUDA event pair on the stream and qtt_rk4_step runs eagerly (no graph replay).  qtt_ctx_profile_report
  * synchronises, then writes, for the QTT_PROF_FAMILIES families
- *   0 gemm (DMMA site contractions)  1 lq_panel  2 lq_update  3 rowjacobi  4 select  5 data movement,
- * the summed kernel milliseconds, the summed algorithmic work (flops for 0-3, bytes for 4-5; the per-launch
+ *   0 gemm (DMMA site contractions)  1 lq_panel  2 lq_update  3 rowjacobi  4 select  5 data movement
+ *   6 qrcp (pivoted-QR preconditioner of the Jacobi SVD),
+ * the summed kernel milliseconds, the summed algorithmic work (flops for 0-3 and 6, bytes for 4-5; the per-launch
  * formulas are stated in DESIGN.md) and the number of launches since the last report (host arrays). */
-#define QTT_PROF_FAMILIES 6
+#define QTT_PROF_FAMILIES 7
 qtt_status qtt_ctx_profile(qtt_ctx* ctx, int enabled);
 qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_host, long long* launches_host);
 /* Number of kernels launched (or graph nodes replayed) by this context so far. */

@@ -24,6 +24,13 @@ int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, do
  * [1] += matrices that hit the sweep limit.  SURVEY.md section 8 row a5. */
 int qtt_diag_rowjacobi(void* stream, double* X_dev, int batch, int p, int q, int ld, int* status_dev);
 
+/* The production SVD front end on `batch` matrices X_i (p x q, ld, stride p*ld), in place: rank-revealing
+ * Householder QR with column pivoting X <- Q^T X (columns stay in place, rows from the numerical rank on are
+ * exact zeros, rank_dev[i] <- rank), then -- unless status_dev is NULL -- one-sided Jacobi on the first
+ * rank rows.  Right singular vectors and singular values of X are those of the result's rows.  Needs the
+ * column slices to fit a cluster's shared memory (else cudaErrorInvalidConfiguration).  SURVEY.md section 8 row a5. */
+int qtt_diag_svd_rows(void* stream, double* X_dev, int batch, int p, int q, int ld, int* rank_dev, int* status_dev);
+
 /* Sort rows by norm, apply the rank rule (delta < 0: r = min(chi_max, p, q); else smallest r whose discarded
  * tail is <= delta, clamped to [1, chi_max]), write sigma (p), rank (1 int) and the normalised top rows
  * (r_cap x q) to out_dev. */
@@ -34,6 +41,13 @@ int qtt_diag_select(void* stream, const double* X_dev, int p, int q, int ld, dou
  * `ctas` CTAs of 256 threads, `iters` iterations of 64 independent instructions per warp / thread chain set.
  * *tflops_out <- achieved TFLOP/s (host pointer).  Synchronous. */
 int qtt_diag_fp64_probe(void* stream, int kind, int ctas, int iters, double* tflops_out);
+
+/* While qtt_ctx_profile (qtt.h) is enabled: synchronises the device and writes one CSV line per kernel launch
+ * recorded since the last qtt_ctx_profile_report -- family, shape tag d0..d3, kernel milliseconds, algorithmic
+ * work -- to the host path; the records are kept (the next report still sums them).  Shape tags:
+ * gemm (M, N, K of the first problem, problems); lq_panel / lq_update (k, m, problems, first panel row);
+ * rowjacobi (p, q, problems, CTAs per matrix); select (p, q, problems, 0); move (0). */
+int qtt_diag_profile_dump(const char* path_host);
 
 #ifdef __cplusplus
 }

@@ -66,8 +66,10 @@ PROTOTYPES = {
                                 C.c_longlong, C.c_longlong]),
     "qtt_diag_lq": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
     "qtt_diag_rowjacobi": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P]),
+    "qtt_diag_svd_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
     "qtt_diag_select": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, _P, C.c_int, _P, _P, C.c_int, C.c_double]),
     "qtt_diag_fp64_probe": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, _DP]),
+    "qtt_diag_profile_dump": (C.c_int, [C.c_char_p]),
 }
 
 _lib = None

@@ -269,7 +269,7 @@ def qtt_ctx_launch_count(ctx: Context) -> int:
     return int(ctx.lib.qtt_ctx_launch_count(ctx.h))
 
 
-PROF_FAMILIES = ("gemm", "lq_panel", "lq_update", "rowjacobi", "select", "move")
+PROF_FAMILIES = ("gemm", "lq_panel", "lq_update", "rowjacobi", "select", "move", "qrcp")
 
 
 def qtt_ctx_profile(ctx: Context, enabled: bool) -> None:

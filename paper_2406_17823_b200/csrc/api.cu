@@ -831,9 +831,28 @@ int qtt_diag_rowjacobi(void* stream, double* X, int batch, int p, int q, int ld,
   for (int i = 0; i < batch; ++i) {
     probs[i].X = X + (size_t)i * p * ld;
     probs[i].p = p; probs[i].q = q; probs[i].ld = ld;
+    probs[i].p_dev = nullptr;
     probs[i].status = status;
   }
   return (int)qtt_launch_rowjacobi(probs.data(), batch, static_cast<cudaStream_t>(stream));
+}
+
+int qtt_diag_svd_rows(void* stream, double* X, int batch, int p, int q, int ld, int* rank_dev, int* status) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (!qtt_qrcp_fits(p, q)) return (int)cudaErrorInvalidConfiguration;
+  std::vector<QrcpProb> qp(batch);
+  std::vector<JacProb> probs(batch);
+  for (int i = 0; i < batch; ++i) {
+    qp[i] = QrcpProb{X + (size_t)i * p * ld, p, q, ld, rank_dev + i};
+    probs[i].X = qp[i].X;
+    probs[i].p = p < q ? p : q; probs[i].q = q; probs[i].ld = ld;
+    probs[i].p_dev = rank_dev + i;
+    probs[i].status = status;
+  }
+  cudaError_t e = qtt_launch_qrcp(qp.data(), batch, st);
+  if (e != cudaSuccess) return (int)e;
+  if (!status) return 0;  // status == NULL: preconditioner only
+  return (int)qtt_launch_rowjacobi(probs.data(), batch, st);
 }
 
 int qtt_diag_select(void* stream, const double* X, int p, int q, int ld, double* out, int r_cap, double* sigma,

@@ -77,6 +77,7 @@ cudaError_t qtt_launch_extract_tri(const TriProb* probs, int n, int mode, cudaSt
 struct JacProb {
   double* X;
   int p, q, ld;
+  const int* p_dev;  // if non-null: number of rows to rotate (<= p), read on the device (numerical rank from qrcp)
   int* status;  // device ints, may be shared by all problems: [0] <- max(sweeps used), [1] += 1 if the sweep limit was hit
 };
 #define QTT_JAC_MAX_BATCH 16
@@ -89,6 +90,25 @@ struct JacGroup {
   JacProb p[QTT_JAC_MAX_BATCH];
 };
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream);
+
+// Rank-revealing preconditioner of the row-Jacobi SVD: X (p x q, rows contiguous, ld) <- Q^T X by Householder QR
+// with column pivoting (columns stay in place); rows from the numerical rank on are written as zeros and the
+// rank goes to rank_out (device int, may be null).  One cluster per matrix, column slices in shared memory.
+struct QrcpProb {
+  double* X;
+  int p, q, ld;
+  int* rank_out;
+};
+#define QTT_QRCP_MAX_BATCH 16
+struct QrcpGroup {
+  int nprob;
+  int cluster;  // CTAs per matrix
+  int w;        // columns per CTA (largest problem)
+  int pp;       // column pitch in shared memory
+  QrcpProb p[QTT_QRCP_MAX_BATCH];
+};
+cudaError_t qtt_launch_qrcp(const QrcpProb* probs, int n, cudaStream_t stream);
+bool qtt_qrcp_fits(int p, int q);  // the column slices of a p x q matrix fit in a cluster's shared memory
 
 // After rowjacobi: sort the rows by norm, pick the rank, write normalised rows.
 //   sigma[0..p) <- row norms, descending;  rank[0] <- r' ;  out (r_cap x q, ld = q) <- top rows / sigma.
@@ -145,13 +165,14 @@ void qtt_kernels_init();
 
 // Per-family kernel timing (qtt_ctx_profile_*): when enabled, every launch is bracketed by a CUDA event
 // pair on its stream.  Must be off while a stream is being captured.
-enum QttKernelFamily { QK_GEMM = 0, QK_LQ_PANEL, QK_LQ_UPDATE, QK_JACOBI, QK_SELECT, QK_MOVE, QK_COUNT };
+enum QttKernelFamily { QK_GEMM = 0, QK_LQ_PANEL, QK_LQ_UPDATE, QK_JACOBI, QK_SELECT, QK_MOVE, QK_QRCP, QK_COUNT };
 struct QttProf {
   int fam;
   cudaStream_t st;
   bool live;
   // work: algorithmic flops (GEMM, LQ, Jacobi) or bytes (select, move) of this launch
-  QttProf(int family, cudaStream_t stream, double work);
+  // d0..d3: shape tag of the launch (per family, see qtt_diag_profile_dump in include/qtt_diag.h)
+  QttProf(int family, cudaStream_t stream, double work, int d0 = 0, int d1 = 0, int d2 = 0, int d3 = 0);
   ~QttProf();
 };
 void qtt_prof_enable(bool on);

@@ -245,7 +245,7 @@ cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream) {
   double flops = 0.0;
   for (int i = 0; i < grp.nprob; ++i) flops += 2.0 * grp.p[i].M * grp.p[i].N * (double)grp.p[i].K * grp.p[i].nbatch;
   {
-    QttProf prof(QK_GEMM, stream, flops);
+    QttProf prof(QK_GEMM, stream, flops, grp.p[0].M, grp.p[0].N, grp.p[0].K, grp.nprob);
     qtt_gemm_dmma_kernel<BM, BN, WM, WN><<<t, NT, SMEM, stream>>>(grp);
   }
   return cudaGetLastError();

@@ -27,7 +27,10 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
   const int rank = cluster.block_rank();
   const JacProb& P = g.p[blockIdx.x / C];
   const int tid = threadIdx.x;
-  const int p = P.p, q = P.q;
+  int p = P.p;
+  if (P.p_dev) p = min(p, P.p_dev[0]);
+  if (p < 2) return;  // uniform over the cluster
+  const int q = P.q;
   const int pe = (p + 1) & ~1;  // players in the tournament (one bye if p is odd)
   const int np2 = pe / 2;
   const int pe_max = (pmax + 1) & ~1, np2_max = pe_max / 2;
@@ -232,19 +235,26 @@ struct PairOps {
 };
 
 template <int G, int EPL>
-__global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_constant__ JacGroup g, int b, int pitch) {
+__global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_constant__ JacGroup g, int bmax,
+                                                                 int pitchmax) {
   cg::cluster_group cluster = cg::this_cluster();
   const int C = g.cluster;
   const int rank = (C > 1) ? (int)cluster.block_rank() : 0;
   const JacProb& P = g.p[blockIdx.x / C];
   const int tid = threadIdx.x, lane = tid & 31;
-  const int p = P.p, q = P.q;
+  // rows to rotate: the numerical rank found by the pivoted-QR preconditioner, if there is one
+  int p = P.p;
+  if (P.p_dev) p = min(p, P.p_dev[0]);
+  if (p < 2) return;  // uniform over the cluster: nothing to orthogonalise
+  const int q = P.q;
   constexpr int NGRP = BJ_NT / G;
   const int grp = tid / G, gl = tid % G;
-  const int ne = pitch / G;  // elements per lane actually used (<= EPL)
+  const int pitch = ((q + G - 1) / G) * G;  // <= pitchmax
+  const int b = (p + 2 * C - 1) / (2 * C);  // <= bmax
+  const int ne = pitch / G;                 // elements per lane actually used (<= EPL)
 
   extern __shared__ __align__(16) double sm[];
-  const size_t slot_sz = (size_t)b * pitch;
+  const size_t slot_sz = (size_t)bmax * pitchmax;
   double* xch = sm + 3 * slot_sz;                              // [MAXC] partial sums / rotation counts from peers
   int* cnt = reinterpret_cast<int*>(xch + 2 * MAXC);           // [0] rotations of this CTA in this sweep
   int top_s = 0, bot_s = 1, spare_s = 2;
@@ -572,7 +582,8 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
 
 namespace {
 template <int G, int EPL>
-cudaError_t launch_blockjacobi(JacGroup& grp, int b, int pitch, size_t smem, double flops, cudaStream_t stream) {
+cudaError_t launch_blockjacobi(JacGroup& grp, int pmax, int qmax, int b, int pitch, size_t smem, double flops,
+                               cudaStream_t stream) {
   static bool attr_done = false;
   if (!attr_done) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<G, EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -592,7 +603,7 @@ cudaError_t launch_blockjacobi(JacGroup& grp, int b, int pitch, size_t smem, dou
   at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  QttProf prof(QK_JACOBI, stream, flops);
+  QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, grp.nprob, grp.cluster);
   return cudaLaunchKernelEx(&cfg, qtt_blockjacobi_kernel<G, EPL>, grp, b, pitch);
 }
 
@@ -616,7 +627,8 @@ bool blockjacobi_config(int pmax, int qmax, int& G, int& EPL, int& C, int& b, in
 }  // namespace
 
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream) {
-  // production path: two-level block Jacobi, problems grouped as they come (same-site operands share a shape)
+  // production path: two-level block Jacobi; problems of one call (the operands of one site, similar shapes)
+  // share launches as long as the largest shape of the group fits a cluster's shared memory
   {
     int done = 0;
     bool all_fit = true;
@@ -635,11 +647,13 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
         while (done < n && grp.nprob < QTT_JAC_MAX_BATCH) {
           const JacProb& pr = probs[done];
           if (pr.p >= 2 && pr.q >= 1) {
-            // keep a group to one (G, EPL) class and similar row counts so that padding stays small
-            if (grp.nprob > 0 && (pr.p != pmax || pr.q != qmax)) break;
+            const int pm = pr.p > pmax ? pr.p : pmax, qm = pr.q > qmax ? pr.q : qmax;
+            int G, EPL, C, b, pitch;
+            size_t smem;
+            if (grp.nprob > 0 && !blockjacobi_config(pm, qm, G, EPL, C, b, pitch, smem)) break;
             grp.p[grp.nprob++] = pr;
-            pmax = pr.p;
-            qmax = pr.q;
+            pmax = pm;
+            qmax = qm;
             double a = pr.p > pr.q ? pr.p : pr.q, bb = pr.p > pr.q ? pr.q : pr.p;
             flops += 6.0 * a * bb * bb + 20.0 * bb * bb * bb;
           }
@@ -654,9 +668,9 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
         grp.wslice = 0;
         grp.max_sweeps = 60;
         cudaError_t e;
-        if (G == 16 && EPL == 8) e = launch_blockjacobi<16, 8>(grp, b, pitch, smem, flops, stream);
-        else if (G == 16) e = launch_blockjacobi<16, 16>(grp, b, pitch, smem, flops, stream);
-        else e = launch_blockjacobi<32, 16>(grp, b, pitch, smem, flops, stream);
+        if (G == 16 && EPL == 8) e = launch_blockjacobi<16, 8>(grp, pmax, qmax, b, pitch, smem, flops, stream);
+        else if (G == 16) e = launch_blockjacobi<16, 16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
+        else e = launch_blockjacobi<32, 16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
         if (e != cudaSuccess) return e;
       }
       return cudaSuccess;
@@ -732,7 +746,7 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
       flops += 6.0 * a * b * b + 20.0 * b * b * b;
     }
     {
-      QttProf prof(QK_JACOBI, stream, flops);
+      QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, grp.nprob, -C);
       QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_rowjacobi_kernel, grp, pmax, wp));
     }
   }
@@ -750,7 +764,7 @@ cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream) 
     double bytes = 0.0;
     for (int i = 0; i < g.nprob; ++i) bytes += 8.0 * ((double)g.p[i].p * g.p[i].q + (double)g.p[i].r_cap * g.p[i].q);
     {
-      QttProf prof(QK_SELECT, stream, bytes);
+      QttProf prof(QK_SELECT, stream, bytes, g.p[0].p, g.p[0].q, g.nprob, 0);
       qtt_select_kernel<<<g.nprob, SNT, 0, stream>>>(g);
     }
     QTT_CHECK_CUDA(cudaGetLastError());

@@ -351,11 +351,11 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
         fu += 4.0 * nbp * mw * (grp.p[i].k - p0 - nbp);
       }
       {
-        QttProf prof(QK_LQ_PANEL, stream, fp);
+        QttProf prof(QK_LQ_PANEL, stream, fp, grp.p[0].k, grp.p[0].m, grp.nprob, p0);
         QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
       }
       if (ctas > 0) {
-        QttProf prof(QK_LQ_UPDATE, stream, fu);
+        QttProf prof(QK_LQ_UPDATE, stream, fu, ug.p[0].k, ug.p[0].m, ug.nprob, p0);
         qtt_lq_update_kernel<<<ctas, UPD_NT, 0, stream>>>(ug);
         QTT_CHECK_CUDA(cudaGetLastError());
       }

@@ -54,17 +54,19 @@ long long g_qtt_launch_count = 0;
 
 // ------------------------------------------------------------------------------------------ profiler
 namespace {
-struct ProfRec { int fam; cudaEvent_t e0, e1; double work; };
+struct ProfRec { int fam; cudaEvent_t e0, e1; double work; int d[4]; };
 bool g_prof_on = false;
 std::vector<ProfRec> g_prof;
 }  // namespace
 
-QttProf::QttProf(int family, cudaStream_t stream, double work) : fam(family), st(stream), live(g_prof_on) {
+QttProf::QttProf(int family, cudaStream_t stream, double work, int d0, int d1, int d2, int d3)
+    : fam(family), st(stream), live(g_prof_on) {
   ++g_qtt_launch_count;
   if (!live) return;
   ProfRec r;
   r.fam = fam;
   r.work = work;
+  r.d[0] = d0; r.d[1] = d1; r.d[2] = d2; r.d[3] = d3;
   if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) {
     live = false;
     return;
@@ -94,6 +96,23 @@ cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long lo
 }
 
 void qtt_kernels_init() {}
+
+extern "C" int qtt_diag_profile_dump(const char* path_host) {
+  if (!path_host) return (int)cudaErrorInvalidValue;
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) return (int)e;
+  FILE* f = fopen(path_host, "w");
+  if (!f) return (int)cudaErrorInvalidValue;
+  static const char* names[QK_COUNT] = {"gemm", "lq_panel", "lq_update", "rowjacobi", "select", "move", "qrcp"};
+  fprintf(f, "family,d0,d1,d2,d3,ms,work\n");
+  for (ProfRec& r : g_prof) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.e0, r.e1) != cudaSuccess) continue;
+    fprintf(f, "%s,%d,%d,%d,%d,%.6f,%.6g\n", names[r.fam], r.d[0], r.d[1], r.d[2], r.d[3], (double)t, r.work);
+  }
+  fclose(f);
+  return 0;
+}
 
 extern "C" int qtt_diag_fp64_probe(void* stream, int kind, int ctas, int iters, double* tflops_out) {
   cudaStream_t st = static_cast<cudaStream_t>(stream);

@@ -194,12 +194,15 @@ struct SvdJob {
   double delta_scale;
 };
 
-// right singular vectors by row-Jacobi; tall inputs are first reduced to their triangular factor
+// right singular vectors by row-Jacobi, preconditioned by a rank-revealing pivoted QR (qrcp.cu): X <- Q^T X has
+// graded rows (7-9 Jacobi sweeps instead of 20-45) and only its first rank(X) rows are non-zero, so the Jacobi
+// kernel rotates rank(X) rows.  Inputs too large for the cluster-resident QR are first reduced to their
+// triangular factor by the blocked LQ.
 void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
   if (jobs.empty()) return;
   std::vector<LqJob> lq;
   for (SvdJob& j : jobs) {
-    if (j.p > j.q && j.p >= 8) {
+    if (!qtt_qrcp_fits(j.p, j.q) && j.p > j.q && j.p >= 8) {
       // X = Q R_X, same right singular vectors: R_X (q x q) from the LQ of X^T (q x p)
       double* Xt = ctx->arena.tmp((size_t)j.q * j.p);
       QTT_CU(qtt_launch_transpose(j.X, j.p, j.q, j.q, Xt, j.p, ctx->stream));
@@ -210,20 +213,30 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
     }
   }
   run_lq(ctx, lq);
+  std::vector<QrcpProb> qp;
   std::vector<JacProb> jp;
   std::vector<SelProb> sp;
   for (const SvdJob& j : jobs) {
+    int prow = j.p;
+    const int* rank_dev = nullptr;
+    if (j.p >= 2 && qtt_qrcp_fits(j.p, j.q)) {
+      int* rk = reinterpret_cast<int*>(ctx->arena.tmp(1));
+      qp.push_back(QrcpProb{j.X, j.p, j.q, j.q, rk});
+      rank_dev = rk;
+      prow = std::min(j.p, j.q);  // the rows below are exact zeros after the QR
+    }
     JacProb a;
-    a.X = j.X; a.p = j.p; a.q = j.q; a.ld = j.q; a.status = ctx->jac_status;
+    a.X = j.X; a.p = prow; a.q = j.q; a.ld = j.q; a.p_dev = rank_dev; a.status = ctx->jac_status;
     jp.push_back(a);
     SelProb s;
-    s.X = j.X; s.p = j.p; s.q = j.q; s.ld = j.q;
+    s.X = j.X; s.p = prow; s.q = j.q; s.ld = j.q;
     s.out = j.out; s.out_ld = j.q; s.r_cap = j.r_cap;
     s.sigma = j.sigma; s.rank = j.rank;
     s.delta_ptr = j.delta_ptr; s.delta_out = j.delta_out; s.delta_scale = j.delta_scale;
     s.chi_max = j.chi_max;
     sp.push_back(s);
   }
+  if (!qp.empty()) QTT_CU(qtt_launch_qrcp(qp.data(), (int)qp.size(), ctx->stream));
   QTT_CU(qtt_launch_rowjacobi(jp.data(), (int)jp.size(), ctx->stream));
   QTT_CU(qtt_launch_select(sp.data(), (int)sp.size(), ctx->stream));
   jobs.clear();

@@ -195,3 +195,59 @@ def test_fp64_probes_report_plausible_rates(env):
         t = C.c_double()
         assert lib.qtt_diag_fp64_probe(C.c_void_p(stream.cuda_stream), kind, 148 * 4, 2000, C.byref(t)) == 0
         assert 1.0 < t.value < 200.0
+
+
+SVD_CASES = [
+    # p, q, batch, true rank (0 = full)
+    (1, 4, 1, 0), (2, 4, 2, 0), (12, 4, 3, 0), (16, 64, 2, 0), (48, 16, 1, 0), (64, 256, 2, 20), (192, 256, 3, 70),
+    (320, 256, 2, 100), (100, 37, 2, 0), (256, 256, 1, 0), (512, 512, 1, 150),
+]
+
+
+@pytest.mark.parametrize("p,q,batch,rk", SVD_CASES)
+def test_pivoted_qr_preconditioner_then_jacobi(env, p, q, batch, rk):
+    """qtt_diag_svd_rows: X <- Q^T X keeps X^T X (row space, singular values), reveals the numerical rank, zeroes the
+    rows below it; Jacobi on the graded rows then reproduces LAPACK's singular values in few sweeps."""
+    lib, torch, stream = env
+    rng = np.random.default_rng(p * 7 + q + rk)
+    mn = min(p, q)
+    if rk:
+        X = (rng.standard_normal((batch, p, rk)) * np.logspace(0, -9, rk)[None, None, :]) @ rng.standard_normal((batch, rk, q))
+    else:
+        X = rng.standard_normal((batch, p, q)) * np.logspace(0, -7, q)[None, None, :]
+    want = [np.linalg.svd(X[b], compute_uv=False) for b in range(batch)]
+    # preconditioner only
+    dX = dev(torch, X)
+    rank = torch.zeros(batch, dtype=torch.int32, device="cuda")
+    torch.cuda.synchronize()
+    assert lib.qtt_diag_svd_rows(C.c_void_p(stream.cuda_stream), ptr(dX), batch, p, q, q, ptr(rank), None) == 0
+    stream.synchronize()
+    R = dX.cpu().numpy()
+    rr = rank.cpu().numpy()
+    for b in range(batch):
+        nx = np.linalg.norm(X[b])
+        assert 1 <= rr[b] <= mn
+        if rk:
+            assert rk <= rr[b] <= rk + 2  # exact rank rk plus at most a couple of noise rows above 8 eps ||X||
+        assert np.all(R[b][rr[b]:] == 0.0)
+        assert np.linalg.norm(R[b].T @ R[b] - X[b].T @ X[b]) <= 1e-13 * nx * nx
+        # graded rows: norms of the rows decrease up to the usual pivoted-QR slack
+        rn = np.linalg.norm(R[b][: rr[b]], axis=1)
+        assert np.all(rn[1:] <= rn[:-1] * np.sqrt(q) * 1.0001)
+    # preconditioner + Jacobi
+    dX = dev(torch, X)
+    status = torch.zeros(2, dtype=torch.int32, device="cuda")
+    torch.cuda.synchronize()
+    assert lib.qtt_diag_svd_rows(C.c_void_p(stream.cuda_stream), ptr(dX), batch, p, q, q, ptr(rank), ptr(status)) == 0
+    stream.synchronize()
+    Z = dX.cpu().numpy()
+    stt = status.cpu().numpy()
+    assert stt[1] == 0 and stt[0] <= 16, stt
+    for b in range(batch):
+        s = np.sort(np.linalg.norm(Z[b], axis=1))[::-1]
+        assert np.max(np.abs(s[:mn] - want[b])) <= 1e-12 * want[b][0]
+        G = Z[b] @ Z[b].T
+        d = np.sqrt(np.maximum(np.diag(G), 1e-300))
+        big = d > 1e-9 * d.max()
+        off = (G - np.diag(np.diag(G))) / np.outer(d, d)
+        assert np.max(np.abs(off[np.ix_(big, big)])) < 1e-13 * np.sqrt(q) * 4
