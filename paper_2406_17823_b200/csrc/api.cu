@@ -817,8 +817,9 @@ int qtt_diag_lq(void* stream, double* Y, int batch, int k, int m, int ld, double
   for (int i = 0; i < batch; ++i) {
     probs[i].Y = Y + (size_t)i * k * ld;
     probs[i].k = k; probs[i].m = m; probs[i].ld = ld;
-    probs[i].V = scratch + (size_t)i * 2 * s;
+    probs[i].V = scratch + (size_t)i * 3 * s;
     probs[i].TV = probs[i].V + s;
+    probs[i].W = probs[i].TV + s;
     tris[i] = TriProb{probs[i].Y, k, ld, R + (size_t)i * k * k, k};
   }
   cudaError_t e = qtt_launch_lq(probs.data(), batch, static_cast<cudaStream_t>(stream));

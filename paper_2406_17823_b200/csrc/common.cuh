@@ -41,7 +41,8 @@ struct GemmGroup {
   GemmProb p[QTT_GEMM_MAX_GROUP];
 };
 // Launch as many kernels as needed for `n` problems (any n).  Returns cudaSuccess or the error.
-cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream);
+// `family`: profiler family the launches are booked under (QK_GEMM unless the GEMM is a step of another family).
+cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream, int family = 0);
 
 // ----------------------------------------------------------------------------------------------
 // Batched Q-less LQ (blocked Householder by rows).  Y is k x m (k <= m), rows contiguous with
@@ -52,6 +53,7 @@ struct LqProb {
   int k, m, ld;
   double* V;   // scratch  nb x m : clean reflector rows of the current panel
   double* TV;  // scratch  nb x m : T * V of the current panel
+  double* W;   // scratch  nb x m : (rows below the panel) x nb product Y2 V^T of the trailing update
 };
 #define QTT_LQ_MAX_BATCH 16
 #define QTT_LQ_NB 16
@@ -61,7 +63,7 @@ struct LqGroup {
   LqProb p[QTT_LQ_MAX_BATCH];
 };
 cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream);
-size_t qtt_lq_scratch_doubles(int m);  // per problem, for V and for TV (each)
+size_t qtt_lq_scratch_doubles(int m);  // per problem, for each of V, TV and W
 
 // Copy the triangular factor out of a factored Y:  mode 0: R = L^T (k x k upper, row-major, ld = ldr),
 // mode 1: L itself (k x k lower) into dst with leading dimension ldr.

@@ -223,7 +223,7 @@ qtt_gemm_dmma_kernel(const __grid_constant__ GemmGroup g) {
 }
 
 template <int BM, int BN, int WM, int WN>
-cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream) {
+cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream, int family) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
   constexpr size_t SMEM = (size_t)STAGES * (BM + BN) * KPITCH * sizeof(double);
   static bool attr_done = false;
@@ -245,7 +245,7 @@ cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream) {
   double flops = 0.0;
   for (int i = 0; i < grp.nprob; ++i) flops += 2.0 * grp.p[i].M * grp.p[i].N * (double)grp.p[i].K * grp.p[i].nbatch;
   {
-    QttProf prof(QK_GEMM, stream, flops, grp.p[0].M, grp.p[0].N, grp.p[0].K, grp.nprob);
+    QttProf prof(family, stream, flops, grp.p[0].M, grp.p[0].N, grp.p[0].K, grp.nprob);
     qtt_gemm_dmma_kernel<BM, BN, WM, WN><<<t, NT, SMEM, stream>>>(grp);
   }
   return cudaGetLastError();
@@ -256,7 +256,7 @@ inline bool al16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 
 }  // namespace
 
-cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream) {
+cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream, int family) {
   int done = 0;
   while (done < n) {
     GemmGroup grp;
@@ -287,11 +287,11 @@ cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream) {
     if (grp.nprob == 0) continue;
     cudaError_t e;
     if (big_tiles >= 120 && minMN >= 96)
-      e = launch_cfg<128, 128, 64, 32>(grp, stream);
+      e = launch_cfg<128, 128, 64, 32>(grp, stream, family);
     else if (mid_tiles >= 32 && minMN >= 48)
-      e = launch_cfg<64, 64, 32, 32>(grp, stream);
+      e = launch_cfg<64, 64, 32, 32>(grp, stream, family);
     else
-      e = launch_cfg<32, 32, 16, 16>(grp, stream);
+      e = launch_cfg<32, 32, 16, 16>(grp, stream, family);
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;

@@ -9,6 +9,7 @@
 // warp shuffles inside a CTA and all-to-all through distributed shared memory between CTAs.
 // Trailing update: a separate grid, one warp per pair of rows, Y2 <- Y2 - (Y2 V^T) (T V), compact WY.
 #include <cooperative_groups.h>
+#include <cstring>
 
 #include "common.cuh"
 namespace cg = cooperative_groups;
@@ -355,9 +356,34 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
         QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
       }
       if (ctas > 0) {
-        QttProf prof(QK_LQ_UPDATE, stream, fu, ug.p[0].k, ug.p[0].m, ug.nprob, p0);
-        qtt_lq_update_kernel<<<ctas, UPD_NT, 0, stream>>>(ug);
-        QTT_CHECK_CUDA(cudaGetLastError());
+        // trailing update of the rows below the panel, Y2 <- Y2 - (Y2 V^T)(T V), as two grouped DMMA GEMMs
+        GemmProb g1[QTT_LQ_MAX_BATCH], g2[QTT_LQ_MAX_BATCH];
+        for (int i = 0; i < ug.nprob; ++i) {
+          const LqProb& p = ug.p[i];
+          const int nbp = (p.k - p0 < NB) ? p.k - p0 : NB;
+          const int r0 = p0 + nbp, rem = p.k - r0, mw = p.m - p0;
+          GemmProb a;
+          memset(&a, 0, sizeof(a));
+          a.nbatch = 1;
+          a.alpha = 1.0; a.beta = 0.0;
+          a.A = p.Y + (i64)r0 * p.ld + p0; a.a_lo = p.ld; a.a_k = 1;
+          a.B = p.V + p0; a.b_k = 1; a.b_n = p.m;
+          a.C = p.W; a.c_lo = NB; a.c_n = 1;
+          a.M = rem; a.N = nbp; a.K = mw;
+          g1[i] = a;
+          GemmProb b;
+          memset(&b, 0, sizeof(b));
+          b.nbatch = 1;
+          b.alpha = -1.0; b.beta = 1.0;
+          b.A = p.W; b.a_lo = NB; b.a_k = 1;
+          b.B = p.TV + p0; b.b_k = p.m; b.b_n = 1;
+          b.C = p.Y + (i64)r0 * p.ld + p0; b.c_lo = p.ld; b.c_n = 1;
+          b.M = rem; b.N = mw; b.K = nbp;
+          g2[i] = b;
+        }
+        QTT_CHECK_CUDA(qtt_launch_gemm(g1, ug.nprob, stream, QK_LQ_UPDATE));
+        QTT_CHECK_CUDA(qtt_launch_gemm(g2, ug.nprob, stream, QK_LQ_UPDATE));
+        (void)fu;
       }
     }
   }

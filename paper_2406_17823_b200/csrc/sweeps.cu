@@ -110,7 +110,7 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
     if (j.m <= LQ_MAX_M) {
       LqProb p;
       p.Y = j.Y; p.k = j.k; p.m = j.m; p.ld = j.ld;
-      p.V = p.TV = nullptr;
+      p.V = p.TV = p.W = nullptr;
       probs.push_back(p);
       tris.push_back(TriProb{j.Y, j.k, j.ld, j.R, j.k});
     } else {
@@ -132,7 +132,7 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
         if (mc >= j.k) {
           LqProb p;
           p.Y = Yc; p.k = j.k; p.m = mc; p.ld = j.ld;
-          p.V = p.TV = nullptr;
+          p.V = p.TV = p.W = nullptr;
           probs.push_back(p);
           tris.push_back(TriProb{Yc, j.k, j.ld, stack + off, total});  // mode 1 below
           off += j.k;
@@ -150,14 +150,16 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
     int mmax = 0;
     for (const LqProb& p : probs) mmax = std::max(mmax, p.m);
     const int nslot = std::min<int>((int)probs.size(), QTT_LQ_MAX_BATCH);
-    std::vector<double*> slotV(nslot), slotTV(nslot);
+    std::vector<double*> slotV(nslot), slotTV(nslot), slotW(nslot);
     for (int s2 = 0; s2 < nslot; ++s2) {
       slotV[s2] = ctx->arena.tmp(qtt_lq_scratch_doubles(mmax));
       slotTV[s2] = ctx->arena.tmp(qtt_lq_scratch_doubles(mmax));
+      slotW[s2] = ctx->arena.tmp(qtt_lq_scratch_doubles(mmax));
     }
     for (size_t i = 0; i < probs.size(); ++i) {
       probs[i].V = slotV[i % QTT_LQ_MAX_BATCH];
       probs[i].TV = slotTV[i % QTT_LQ_MAX_BATCH];
+      probs[i].W = slotW[i % QTT_LQ_MAX_BATCH];
     }
   }
   // direct problems and chunk problems share the panel launches; their triangles are extracted separately

@@ -92,7 +92,7 @@ def test_lq_triangular_factor(env, k, m, batch):
     Y = rng.standard_normal((batch, k, m))
     dY = dev(torch, Y)
     dR = torch.zeros((batch, k, k), dtype=torch.float64, device="cuda")
-    scratch = torch.zeros(batch * 2 * 16 * m, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(batch * 3 * 16 * m, dtype=torch.float64, device="cuda")
     torch.cuda.synchronize()
     st = lib.qtt_diag_lq(C.c_void_p(stream.cuda_stream), ptr(dY), batch, k, m, m, ptr(dR), ptr(scratch))
     assert st == 0
@@ -114,7 +114,7 @@ def test_lq_rank_deficient(env):
     Y[10] = 0.0
     dY = dev(torch, Y)
     dR = torch.zeros((k, k), dtype=torch.float64, device="cuda")
-    scratch = torch.zeros(2 * 16 * m, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(3 * 16 * m, dtype=torch.float64, device="cuda")
     torch.cuda.synchronize()
     assert lib.qtt_diag_lq(C.c_void_p(stream.cuda_stream), ptr(dY), 1, k, m, m, ptr(dR), ptr(scratch)) == 0
     stream.synchronize()
