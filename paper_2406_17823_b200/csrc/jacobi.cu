@@ -196,74 +196,93 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
 }
 
 // ------------------------------------------------------------------------------------------------
-// Two-level block Jacobi, the production path for every matrix whose row blocks fit in a cluster's
-// shared memory.  The p rows are cut into 2C blocks of b rows; every CTA of the cluster (C CTAs) holds
-// two blocks with their FULL rows, so a rotation needs no cross-CTA reduction at all:
+// Two-level block Jacobi, the production path for every matrix whose row blocks fit in a cluster's shared
+// memory.  The p rows are cut into 2C blocks of b rows; every CTA of the cluster (C CTAs) holds two blocks
+// with their FULL rows, so a rotation needs no cross-CTA reduction at all:
 //   sweep = intra-block pairs of the two resident blocks (b-1 rounds)
 //         + 2C-1 outer rounds of a round-robin tournament over the blocks; in each, the CTA meets
 //           every row of its "top" block with every row of its "bot" block (b inner rounds of b
-//           disjoint pairs, one lane group per pair, the top row kept in registers), then the blocks
+//           disjoint pairs, one warp per pair, the top row kept in registers), then the blocks
 //           move one seat through distributed shared memory (pull into a spare slot, two
 //           cluster.syncs, relabel the slots -- no copy inside a CTA).
 // Every pair of rows meets exactly once per sweep, as in the cyclic one-sided Jacobi method.
+//  * Squared row norms travel with the rows and are updated in closed form after a rotation
+//    (aa' = aa - t ab, bb' = bb + t ab), so a pair costs ONE inner product (a.b) and one warp reduction; they
+//    are recomputed from the data once per sweep.
+//  * The number of rows is read on the device (numerical rank from the pivoted-QR preconditioner); only
+//    Ce = ceil(p / (2 bmax)) CTAs of the cluster take part, the others exit at once (cluster barriers wait
+//    for non-exited threads only).
+//  * Convergence: a sweep in which no pair had cos^2 > 1e-15 ends the iteration -- Jacobi converges
+//    quadratically, so after such a sweep the remaining cosines are O(1e-15).
 constexpr int BJ_NT = 512;
+constexpr int BJ_G = 32;
+constexpr int BJ_NGRP = BJ_NT / BJ_G;
 
-template <int G, int EPL>
-struct PairOps {
-  // reduce (aa, bb, ab) over the G lanes of a group
-  static __device__ __forceinline__ void reduce(double& aa, double& bb, double& ab) {
-#pragma unroll
-    for (int o = G >> 1; o > 0; o >>= 1) {
-      aa += __shfl_xor_sync(0xffffffffu, aa, o);
-      bb += __shfl_xor_sync(0xffffffffu, bb, o);
-      ab += __shfl_xor_sync(0xffffffffu, ab, o);
-    }
-  }
-  // rotation (c, s) that orthogonalises two rows with Gram entries (aa, bb, ab); returns false if none is needed
-  static __device__ __forceinline__ bool rotation(double aa, double bb, double ab, double tol2, double floor2,
-                                                  double& c, double& s) {
-    c = 1.0;
-    s = 0.0;
-    if (!(ab * ab > tol2 * aa * bb) || !(aa > floor2) || !(bb > floor2)) return false;
-    const double zeta = (bb - aa) / (2.0 * ab);
-    const double t = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-    c = rsqrt(1.0 + t * t);
-    c = c * (1.5 - 0.5 * (1.0 + t * t) * c * c);  // one Newton step: full fp64 accuracy
-    s = c * t;
-    return s != 0.0;
-  }
+struct Rot {
+  double c, s, t;
+  bool apply, big;
 };
+// rotation that orthogonalises two rows with Gram entries (aa, bb, ab):  a' = c a - s b,  b' = s a + c b
+__device__ __forceinline__ Rot jacobi_rotation(double aa, double bb, double ab, double tol2, double floor2) {
+  Rot r;
+  r.c = 1.0; r.s = 0.0; r.t = 0.0;
+  r.apply = false; r.big = false;
+  const double ab2 = ab * ab, nn = aa * bb;
+  if (!(ab2 > tol2 * nn) || !(aa > floor2) || !(bb > floor2)) return r;
+  const double d = bb - aa;
+  // t = sign(zeta) / (|zeta| + sqrt(1 + zeta^2)),  zeta = d / (2 ab)
+  const double t = copysign(2.0, d) * ab / (fabs(d) + sqrt(d * d + 4.0 * ab2));
+  if (!(t == t)) return r;
+  const double w = 1.0 + t * t;
+  double c = rsqrt(w);
+  c = c * (1.5 - 0.5 * w * c * c);  // one Newton step: full fp64 accuracy
+  r.c = c;
+  r.s = c * t;
+  r.t = t;
+  r.apply = r.s != 0.0;
+  r.big = ab2 > 1e-15 * nn;
+  return r;
+}
+__device__ __forceinline__ double warp_sum1(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
 
-template <int G, int EPL>
+// shared memory: 3 slots of [bmax * pitchmax data | bme norms] | xch [2][MAXC] counts | fro [MAXC] | ints
+template <int EPL>
 __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_constant__ JacGroup g, int bmax,
                                                                  int pitchmax) {
   cg::cluster_group cluster = cg::this_cluster();
   const int C = g.cluster;
   const int rank = (C > 1) ? (int)cluster.block_rank() : 0;
   const JacProb& P = g.p[blockIdx.x / C];
-  const int tid = threadIdx.x, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
   // rows to rotate: the numerical rank found by the pivoted-QR preconditioner, if there is one
   int p = P.p;
   if (P.p_dev) p = min(p, P.p_dev[0]);
   if (p < 2) return;  // uniform over the cluster: nothing to orthogonalise
+  const int Ce = max(1, (p + 2 * bmax - 1) / (2 * bmax));  // CTAs that take part (<= C)
+  if (rank >= Ce) return;
   const int q = P.q;
-  constexpr int NGRP = BJ_NT / G;
-  const int grp = tid / G, gl = tid % G;
-  const int pitch = ((q + G - 1) / G) * G;  // <= pitchmax
-  const int b = (p + 2 * C - 1) / (2 * C);  // <= bmax
-  const int ne = pitch / G;                 // elements per lane actually used (<= EPL)
+  const int pitch = ((q + BJ_G - 1) / BJ_G) * BJ_G;  // <= pitchmax
+  const int b = (p + 2 * Ce - 1) / (2 * Ce);         // <= bmax
+  const int ne = pitch / BJ_G;                       // elements per lane actually used (<= EPL)
 
   extern __shared__ __align__(16) double sm[];
-  const size_t slot_sz = (size_t)bmax * pitchmax;
-  double* xch = sm + 3 * slot_sz;                              // [MAXC] partial sums / rotation counts from peers
-  int* cnt = reinterpret_cast<int*>(xch + 2 * MAXC);           // [0] rotations of this CTA in this sweep
+  const int bme = (bmax + 1) & ~1;
+  const size_t data_sz = (size_t)bmax * pitchmax;
+  const size_t slot_sz = data_sz + bme;
+  double* xch = sm + 3 * slot_sz;  // [2][MAXC] "big rotation" counts from peers
+  double* xfro = xch + 2 * MAXC;   // [MAXC]
+  int* cnt = reinterpret_cast<int*>(xfro + MAXC);
   int top_s = 0, bot_s = 1, spare_s = 2;
   auto slot = [&](int sidx) { return sm + (size_t)sidx * slot_sz; };
 
-  // ---- load: block k holds rows [k b, (k+1) b); CTA c starts with top = block c, bot = block 2C-1-c
+  // ---- load: block k holds rows [k b, (k+1) b); CTA c starts with top = block c, bot = block 2Ce-1-c
   double fro = 0.0;
   for (int which = 0; which < 2; ++which) {
-    const int blk = which == 0 ? rank : 2 * C - 1 - rank;
+    const int blk = which == 0 ? rank : 2 * Ce - 1 - rank;
     double* S = slot(which == 0 ? top_s : bot_s);
     for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
       const int r = idx / pitch, x = idx - r * pitch;
@@ -276,23 +295,22 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
   }
   // Frobenius norm^2 over the cluster -> noise floor (rows below eps * ||X||_F / sqrt(p) are zero to
   // working accuracy; they cannot all be made mutually orthogonal when p > rank)
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) fro += __shfl_xor_sync(0xffffffffu, fro, o);
+  fro = warp_sum1(fro);
   if (tid == 0) cnt[0] = 0;
-  if (tid < 2 * MAXC) xch[tid] = 0.0;
+  if (tid < MAXC) xfro[tid] = 0.0;
   __syncthreads();
-  if (lane == 0) atomicAdd(&xch[MAXC + rank], fro);  // own partial, slot [MAXC + rank]
+  if (lane == 0) atomicAdd(&xfro[rank], fro);
   __syncthreads();
-  if (C > 1) {
-    cluster.sync();  // peers have zeroed their xch
-    if (tid < C && tid != rank) {
-      double* remote = cluster.map_shared_rank(xch, tid);
-      remote[MAXC + rank] = xch[MAXC + rank];
+  if (Ce > 1) {
+    cluster.sync();  // peers have zeroed their xfro
+    if (tid < Ce && tid != rank) {
+      double* remote = cluster.map_shared_rank(xfro, tid);
+      remote[rank] = xfro[rank];
     }
     cluster.sync();
   }
   double fro2 = 0.0;
-  for (int c2 = 0; c2 < C; ++c2) fro2 += xch[MAXC + c2];
+  for (int c2 = 0; c2 < Ce; ++c2) fro2 += xfro[c2];
   const double floor2 = 4.930380657631324e-32 * fro2 / (double)p;
   const double tol = 2.220446049250313e-16 * sqrt((double)q);
   const double tol2 = tol * tol;
@@ -300,11 +318,25 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
 
   const int be = b + (b & 1);  // players of the intra-block tournament
   int sweep = 0, hit_limit = 0;
-  int myrot = 0;
+  int mybig = 0;
   for (; sweep < g.max_sweeps; ++sweep) {
+    // ---- fresh squared norms of the resident rows
+    for (int which = 0; which < 2; ++which) {
+      double* S = slot(which == 0 ? top_s : bot_s);
+      for (int r = grp; r < b; r += BJ_NGRP) {
+        const double* row = S + (size_t)r * pitch + lane;
+        double sq = 0.0;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e)
+          if (e < ne) sq += row[e * BJ_G] * row[e * BJ_G];
+        sq = warp_sum1(sq);
+        if (lane == 0) S[data_sz + r] = sq;
+      }
+    }
+    __syncthreads();
     // ---- intra-block pairs of both resident blocks
     for (int round = 0; round < be - 1; ++round) {
-      for (int k0 = 0; k0 < be; k0 += NGRP) {  // be pairs in all: be/2 per block
+      for (int k0 = 0; k0 < be; k0 += BJ_NGRP) {  // be pairs in all: be/2 per block
         const int kk = k0 + grp;
         int ia = b, ib = b;
         double* S = slot(top_s);
@@ -321,109 +353,122 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         }
         const bool live = ia < b && ib < b;
         double a[EPL], v[EPL];
-        double aa = 0.0, bb = 0.0, ab = 0.0;
+        double ab = 0.0;
+        double* ra = S + (size_t)(live ? ia : 0) * pitch + lane;
+        double* rb = S + (size_t)(live ? ib : 0) * pitch + lane;
         if (live) {
-          const double* ra = S + (size_t)ia * pitch + gl;
-          const double* rb = S + (size_t)ib * pitch + gl;
 #pragma unroll
           for (int e = 0; e < EPL; ++e)
             if (e < ne) {
-              a[e] = ra[e * G];
-              v[e] = rb[e * G];
-              aa += a[e] * a[e];
-              bb += v[e] * v[e];
+              a[e] = ra[e * BJ_G];
+              v[e] = rb[e * BJ_G];
               ab += a[e] * v[e];
             }
         }
-        PairOps<G, EPL>::reduce(aa, bb, ab);
-        double c, s;
-        if (live && PairOps<G, EPL>::rotation(aa, bb, ab, tol2, floor2, c, s)) {
-          double* ra = S + (size_t)ia * pitch + gl;
-          double* rb = S + (size_t)ib * pitch + gl;
+        ab = warp_sum1(ab);
+        if (live) {
+          const double aa = S[data_sz + ia], bb = S[data_sz + ib];
+          const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
+          if (R.apply) {
 #pragma unroll
-          for (int e = 0; e < EPL; ++e)
-            if (e < ne) {
-              ra[e * G] = c * a[e] - s * v[e];
-              rb[e * G] = s * a[e] + c * v[e];
+            for (int e = 0; e < EPL; ++e)
+              if (e < ne) {
+                ra[e * BJ_G] = R.c * a[e] - R.s * v[e];
+                rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
+              }
+            if (lane == 0) {
+              S[data_sz + ia] = fmax(aa - R.t * ab, 0.0);
+              S[data_sz + ib] = fmax(bb + R.t * ab, 0.0);
+              if (R.big) ++mybig;
             }
-          if (gl == 0) ++myrot;
+          }
         }
       }
       __syncthreads();
     }
-    // ---- tournament over the 2C blocks
-    for (int t = 0; t < 2 * C - 1; ++t) {
+    // ---- tournament over the 2Ce blocks
+    for (int t = 0; t < 2 * Ce - 1; ++t) {
       double* T = slot(top_s);
       double* B = slot(bot_s);
-      for (int i0 = 0; i0 < b; i0 += NGRP) {
+      for (int i0 = 0; i0 < b; i0 += BJ_NGRP) {
         const int i = i0 + grp;
         const bool have = i < b;
         double a[EPL];
+        double aa = 0.0;
+        double* rt = T + (size_t)(have ? i : 0) * pitch + lane;
         if (have) {
 #pragma unroll
           for (int e = 0; e < EPL; ++e)
-            if (e < ne) a[e] = T[(size_t)i * pitch + gl + e * G];
+            if (e < ne) a[e] = rt[e * BJ_G];
+          aa = T[data_sz + i];
         }
+        int j = have ? i : 0;
         for (int r = 0; r < b; ++r) {
-          const int j = have ? (i + r) % b : 0;
           double v[EPL];
-          double aa = 0.0, bb = 0.0, ab = 0.0;
+          double ab = 0.0;
+          double* rb = B + (size_t)j * pitch + lane;
           if (have) {
 #pragma unroll
             for (int e = 0; e < EPL; ++e)
               if (e < ne) {
-                v[e] = B[(size_t)j * pitch + gl + e * G];
-                aa += a[e] * a[e];
-                bb += v[e] * v[e];
+                v[e] = rb[e * BJ_G];
                 ab += a[e] * v[e];
               }
           }
-          PairOps<G, EPL>::reduce(aa, bb, ab);
-          double c, s;
-          if (have && PairOps<G, EPL>::rotation(aa, bb, ab, tol2, floor2, c, s)) {
+          ab = warp_sum1(ab);
+          if (have) {
+            const double bb = B[data_sz + j];
+            const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
+            if (R.apply) {
 #pragma unroll
-            for (int e = 0; e < EPL; ++e)
-              if (e < ne) {
-                const double an = c * a[e] - s * v[e];
-                B[(size_t)j * pitch + gl + e * G] = s * a[e] + c * v[e];
-                a[e] = an;
+              for (int e = 0; e < EPL; ++e)
+                if (e < ne) {
+                  const double an = R.c * a[e] - R.s * v[e];
+                  rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
+                  a[e] = an;
+                }
+              aa = fmax(aa - R.t * ab, 0.0);
+              if (lane == 0) {
+                B[data_sz + j] = fmax(bb + R.t * ab, 0.0);
+                if (R.big) ++mybig;
               }
-            if (gl == 0) ++myrot;
+            }
           }
+          j = (j + 1 == b) ? 0 : j + 1;
           __syncthreads();
         }
         if (have) {
 #pragma unroll
           for (int e = 0; e < EPL; ++e)
-            if (e < ne) T[(size_t)i * pitch + gl + e * G] = a[e];
+            if (e < ne) rt[e * BJ_G] = a[e];
+          if (lane == 0) T[data_sz + i] = aa;
         }
       }
       __syncthreads();
-      if (C == 1) break;
+      if (Ce == 1) break;
       // ---- move the blocks one seat (labels of every peer are a function of the round number only)
-      const int tt = sweep * (2 * C - 1) + t;  // exchanges done so far
+      const int tt = sweep * (2 * Ce - 1) + t;  // exchanges done so far
       // peer labelling after tt relabels: CTA 0: top fixed at slot 0, (bot, spare) = tt even ? (1, 2) : (2, 1);
-      // CTA c >= 1: (top, bot, spare) = cyclic shifts of (0, 1, 2): top = (3 - tt % 3) % 3 ... computed below
+      // CTA c >= 1: (top, bot, spare) = cyclic shifts of (0, 1, 2)
       auto peer_top = [&](int c2) { return c2 == 0 ? 0 : (2 * tt) % 3; };
       auto peer_bot = [&](int c2) { return c2 == 0 ? ((tt & 1) ? 2 : 1) : (2 * tt + 1) % 3; };
+      auto pull = [&](double* dst, const double* remote) {
+        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
+          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
+        for (int idx = tid; idx < b; idx += BJ_NT) dst[data_sz + idx] = remote[data_sz + idx];
+      };
       cluster.sync();  // every CTA has finished rotating its blocks
       // phase 1: new top <- old top of the left neighbour (CTA 1: old bot of CTA 0) into my spare slot
       if (rank >= 1) {
         const int src = rank - 1;
         const int ss = (rank == 1) ? peer_bot(0) : peer_top(src);
-        const double* remote = cluster.map_shared_rank(sm + (size_t)ss * slot_sz, src);
-        double* dst = slot(spare_s);
-        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
-          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
+        pull(slot(spare_s), cluster.map_shared_rank(sm + (size_t)ss * slot_sz, src));
       }
       cluster.sync();
       // phase 2: new bot <- old bot of the right neighbour (last CTA: its own old top, a relabel)
-      if (rank <= C - 2) {
+      if (rank <= Ce - 2) {
         const int src = rank + 1;
-        const double* remote = cluster.map_shared_rank(sm + (size_t)peer_bot(src) * slot_sz, src);
-        double* dst = slot(rank == 0 ? spare_s : top_s);
-        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
-          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
+        pull(slot(rank == 0 ? spare_s : top_s), cluster.map_shared_rank(sm + (size_t)peer_bot(src) * slot_sz, src));
       }
       cluster.sync();
       if (rank == 0) {
@@ -437,25 +482,20 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         spare_s = ob;
       }
     }
-    // ---- rotations of this sweep over the whole cluster
-    {
-      int r2 = myrot;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) r2 += __shfl_xor_sync(0xffffffffu, r2, o);
-      if (lane == 0 && r2) atomicAdd(&cnt[0], r2);
-      myrot = 0;
-    }
+    // ---- "big" rotations of this sweep over the whole cluster
+    if (lane == 0 && mybig) atomicAdd(&cnt[0], mybig);
+    mybig = 0;
     __syncthreads();
     int total = cnt[0];
-    if (C > 1) {
+    if (Ce > 1) {
       const int par = sweep & 1;
-      if (tid < C) {
+      if (tid < Ce) {
         double* remote = cluster.map_shared_rank(xch, tid);
         remote[par * MAXC + rank] = (double)cnt[0];
       }
       cluster.sync();
       total = 0;
-      for (int c2 = 0; c2 < C; ++c2) total += (int)xch[par * MAXC + c2];
+      for (int c2 = 0; c2 < Ce; ++c2) total += (int)xch[par * MAXC + c2];
     }
     __syncthreads();
     if (tid == 0) cnt[0] = 0;
@@ -468,7 +508,7 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
   }
   // ---- after whole sweeps every block is back in its first seat
   for (int which = 0; which < 2; ++which) {
-    const int blk = which == 0 ? rank : 2 * C - 1 - rank;
+    const int blk = which == 0 ? rank : 2 * Ce - 1 - rank;
     const double* S = slot(which == 0 ? top_s : bot_s);
     for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
       const int r = idx / pitch, x = idx - r * pitch;
@@ -480,7 +520,7 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
     atomicMax(&P.status[0], sweep);
     if (hit_limit) atomicAdd(&P.status[1], 1);
   }
-  if (C > 1) cluster.sync();
+  if (Ce > 1) cluster.sync();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -581,14 +621,14 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
 }  // namespace
 
 namespace {
-template <int G, int EPL>
+template <int EPL>
 cudaError_t launch_blockjacobi(JacGroup& grp, int pmax, int qmax, int b, int pitch, size_t smem, double flops,
                                cudaStream_t stream) {
   static bool attr_done = false;
   if (!attr_done) {
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<G, EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         224 * 1024));
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<G, EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     attr_done = true;
   }
   cudaLaunchConfig_t cfg = {};
@@ -604,25 +644,23 @@ cudaError_t launch_blockjacobi(JacGroup& grp, int pmax, int qmax, int b, int pit
   cfg.attrs = at;
   cfg.numAttrs = 1;
   QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, grp.nprob, grp.cluster);
-  return cudaLaunchKernelEx(&cfg, qtt_blockjacobi_kernel<G, EPL>, grp, b, pitch);
+  return cudaLaunchKernelEx(&cfg, qtt_blockjacobi_kernel<EPL>, grp, b, pitch);
 }
 
 // Block-Jacobi configuration for a group with largest shape pmax x qmax; false if it does not fit.
-bool blockjacobi_config(int pmax, int qmax, int& G, int& EPL, int& C, int& b, int& pitch, size_t& smem) {
-  if (qmax <= 128) { G = 16; EPL = 8; }
-  else if (qmax <= 256) { G = 16; EPL = 16; }
-  else if (qmax <= 512) { G = 32; EPL = 16; }
+// One warp per row pair (EPL = elements per lane); C = ceil(p / 32) CTAs of two blocks of <= 16 rows each, so
+// that the 16 warps of a CTA are all busy in the tournament phase.
+bool blockjacobi_config(int pmax, int qmax, int& EPL, int& C, int& b, int& pitch, size_t& smem) {
+  if (qmax <= 128) EPL = 4;
+  else if (qmax <= 256) EPL = 8;
+  else if (qmax <= 512) EPL = 16;
   else return false;
-  pitch = ((qmax + G - 1) / G) * G;
-  C = pmax / 16;
+  pitch = ((qmax + BJ_G - 1) / BJ_G) * BJ_G;
+  C = (pmax + 31) / 32;
   C = C < 1 ? 1 : (C > MAXC ? MAXC : C);
-  for (;;) {
-    b = (pmax + 2 * C - 1) / (2 * C);
-    smem = ((size_t)3 * b * pitch + 2 * MAXC + 2) * sizeof(double);
-    if (smem <= 220 * 1024) return true;
-    if (C == MAXC) return false;
-    C = C * 2 > MAXC ? MAXC : C * 2;
-  }
+  b = (pmax + 2 * C - 1) / (2 * C);
+  smem = ((size_t)3 * ((size_t)b * pitch + ((b + 1) & ~1)) + 3 * MAXC + 2) * sizeof(double);
+  return smem <= 220 * 1024;
 }
 }  // namespace
 
@@ -633,9 +671,9 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
     int done = 0;
     bool all_fit = true;
     for (int i = 0; i < n && all_fit; ++i) {
-      int G, EPL, C, b, pitch;
+      int EPL, C, b, pitch;
       size_t smem;
-      if (probs[i].p >= 2 && probs[i].q >= 1 && !blockjacobi_config(probs[i].p, probs[i].q, G, EPL, C, b, pitch, smem))
+      if (probs[i].p >= 2 && probs[i].q >= 1 && !blockjacobi_config(probs[i].p, probs[i].q, EPL, C, b, pitch, smem))
         all_fit = false;
     }
     if (all_fit) {
@@ -648,9 +686,9 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
           const JacProb& pr = probs[done];
           if (pr.p >= 2 && pr.q >= 1) {
             const int pm = pr.p > pmax ? pr.p : pmax, qm = pr.q > qmax ? pr.q : qmax;
-            int G, EPL, C, b, pitch;
+            int EPL, C, b, pitch;
             size_t smem;
-            if (grp.nprob > 0 && !blockjacobi_config(pm, qm, G, EPL, C, b, pitch, smem)) break;
+            if (grp.nprob > 0 && !blockjacobi_config(pm, qm, EPL, C, b, pitch, smem)) break;
             grp.p[grp.nprob++] = pr;
             pmax = pm;
             qmax = qm;
@@ -660,17 +698,17 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
           ++done;
         }
         if (grp.nprob == 0) continue;
-        int G, EPL, C, b, pitch;
+        int EPL, C, b, pitch;
         size_t smem;
-        blockjacobi_config(pmax, qmax, G, EPL, C, b, pitch, smem);
+        blockjacobi_config(pmax, qmax, EPL, C, b, pitch, smem);
         grp.cluster = C;
         grp.use_smem = 1;
         grp.wslice = 0;
         grp.max_sweeps = 60;
         cudaError_t e;
-        if (G == 16 && EPL == 8) e = launch_blockjacobi<16, 8>(grp, pmax, qmax, b, pitch, smem, flops, stream);
-        else if (G == 16) e = launch_blockjacobi<16, 16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
-        else e = launch_blockjacobi<32, 16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
+        if (EPL == 4) e = launch_blockjacobi<4>(grp, pmax, qmax, b, pitch, smem, flops, stream);
+        else if (EPL == 8) e = launch_blockjacobi<8>(grp, pmax, qmax, b, pitch, smem, flops, stream);
+        else e = launch_blockjacobi<16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
         if (e != cudaSuccess) return e;
       }
       return cudaSuccess;
