@@ -15,7 +15,9 @@ int qtt_diag_gemm(void* stream, const double* A_dev, const double* B_dev, double
                   int nbatch, long long strideA, long long strideB, long long strideC);
 
 /* Q-less LQ of `batch` matrices Y_i (k x m, k <= m <= 16384, leading dimension ld, consecutive with stride
- * k*ld, DESTROYED); R_i = L_i^T (k x k upper triangular, row-major, consecutive) with Y = L Q.
+ * k*ld, DESTROYED unless small); R_i = L_i^T (k x k upper triangular, row-major, consecutive) with Y = L Q.
+ * Matrices whose slices fit a cluster's shared memory go through the cluster-resident Householder kernel (and
+ * are left alone), larger ones through the blocked panel + DMMA trailing-update path.
  * scratch_dev: batch * 3 * 16 * m doubles.  SURVEY.md section 8 row a4. */
 int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, double* R_dev, double* scratch_dev);
 

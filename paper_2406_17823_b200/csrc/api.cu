@@ -811,6 +811,11 @@ int qtt_diag_gemm(void* stream, const double* A, const double* B, double* C, int
 }
 
 int qtt_diag_lq(void* stream, double* Y, int batch, int k, int m, int ld, double* R, double* scratch) {
+  if (k <= m && qtt_qrcp_fits(m, k)) {  // the cluster-resident Householder kernel, as in the sweeps
+    std::vector<QrcpProb> qp(batch);
+    for (int i = 0; i < batch; ++i) qp[i] = QrcpProb{Y + (size_t)i * k * ld, m, k, ld, nullptr, 1, R + (size_t)i * k * k};
+    return (int)qtt_launch_qrcp(qp.data(), batch, 0, static_cast<cudaStream_t>(stream));
+  }
   std::vector<LqProb> probs(batch);
   std::vector<TriProb> tris(batch);
   const size_t s = qtt_lq_scratch_doubles(m);
@@ -844,13 +849,13 @@ int qtt_diag_svd_rows(void* stream, double* X, int batch, int p, int q, int ld, 
   std::vector<QrcpProb> qp(batch);
   std::vector<JacProb> probs(batch);
   for (int i = 0; i < batch; ++i) {
-    qp[i] = QrcpProb{X + (size_t)i * p * ld, p, q, ld, rank_dev + i};
+    qp[i] = QrcpProb{X + (size_t)i * p * ld, p, q, ld, rank_dev + i, 0, nullptr};
     probs[i].X = qp[i].X;
     probs[i].p = p < q ? p : q; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = rank_dev + i;
     probs[i].status = status;
   }
-  cudaError_t e = qtt_launch_qrcp(qp.data(), batch, st);
+  cudaError_t e = qtt_launch_qrcp(qp.data(), batch, 1, st);
   if (e != cudaSuccess) return (int)e;
   if (!status) return 0;  // status == NULL: preconditioner only
   return (int)qtt_launch_rowjacobi(probs.data(), batch, st);

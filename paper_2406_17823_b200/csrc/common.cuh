@@ -93,13 +93,19 @@ struct JacGroup {
 };
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream);
 
-// Rank-revealing preconditioner of the row-Jacobi SVD: X (p x q, rows contiguous, ld) <- Q^T X by Householder QR
-// with column pivoting (columns stay in place); rows from the numerical rank on are written as zeros and the
-// rank goes to rank_out (device int, may be null).  One cluster per matrix, column slices in shared memory.
+// Cluster-resident Householder QR of X (p x q, rows contiguous, ld), one cluster per matrix, column slices in
+// shared memory (qrcp.cu).
+//  pivot = 1 (rank-revealing preconditioner of the row-Jacobi SVD): X <- Q^T X in place, columns stay in place,
+//    rows from the numerical rank on are written as zeros and the rank goes to rank_out (device int, may be null).
+//  pivot = 0 (Q-less factor of the L->R sweep): R (q x q upper triangular, ld = q) of X = Q R goes to R_out,
+//    X is left alone; needs p >= q.  With transposed = 1, X is given as Y = X^T (q x p, ld), i.e. R^T = the
+//    L factor of Y = L Q.
 struct QrcpProb {
   double* X;
   int p, q, ld;
   int* rank_out;
+  int transposed;
+  double* R_out;
 };
 #define QTT_QRCP_MAX_BATCH 16
 struct QrcpGroup {
@@ -107,9 +113,11 @@ struct QrcpGroup {
   int cluster;  // CTAs per matrix
   int w;        // columns per CTA (largest problem)
   int pp;       // column pitch in shared memory
+  int chm;      // rows per staged pivot-column chunk (largest problem)
+  int pivot;
   QrcpProb p[QTT_QRCP_MAX_BATCH];
 };
-cudaError_t qtt_launch_qrcp(const QrcpProb* probs, int n, cudaStream_t stream);
+cudaError_t qtt_launch_qrcp(const QrcpProb* probs, int n, int pivot, cudaStream_t stream);
 bool qtt_qrcp_fits(int p, int q);  // the column slices of a p x q matrix fit in a cluster's shared memory
 
 // After rowjacobi: sort the rows by norm, pick the rank, write normalised rows.

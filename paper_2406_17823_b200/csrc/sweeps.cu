@@ -105,9 +105,12 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
   std::vector<LqProb> probs;
   std::vector<TriProb> tris;
   std::vector<LqJob> next;  // second-level jobs of the TSQR tree
+  std::vector<QrcpProb> resident;  // small enough for the cluster-resident Householder kernel (qrcp.cu)
   for (const LqJob& j : jobs) {
     if (j.k > j.m) QTT_THROW(QTT_INVALID_ARG, "internal: LQ needs k <= m");
-    if (j.m <= LQ_MAX_M) {
+    if (qtt_qrcp_fits(j.m, j.k)) {
+      resident.push_back(QrcpProb{j.Y, j.m, j.k, j.ld, nullptr, 1, j.R});
+    } else if (j.m <= LQ_MAX_M) {
       LqProb p;
       p.Y = j.Y; p.k = j.k; p.m = j.m; p.ld = j.ld;
       p.V = p.TV = p.W = nullptr;
@@ -144,6 +147,7 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
       next.push_back(LqJob{stack, j.k, total, total, j.R});
     }
   }
+  if (!resident.empty()) QTT_CU(qtt_launch_qrcp(resident.data(), (int)resident.size(), 0, ctx->stream));
   // reflector scratch: the launcher runs consecutive groups of QTT_LQ_MAX_BATCH problems one after the
   // other on the stream, so problem i can share the scratch slot i % QTT_LQ_MAX_BATCH
   {
@@ -168,6 +172,7 @@ void run_lq(qtt_ctx* ctx, std::vector<LqJob>& jobs) {
   {
     size_t ti = 0;
     for (const LqJob& j : jobs) {
+      if (qtt_qrcp_fits(j.m, j.k)) continue;
       if (j.m <= LQ_MAX_M) {
         t0.push_back(tris[ti++]);
       } else {
@@ -223,7 +228,7 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
     const int* rank_dev = nullptr;
     if (j.p >= 2 && qtt_qrcp_fits(j.p, j.q)) {
       int* rk = reinterpret_cast<int*>(ctx->arena.tmp(1));
-      qp.push_back(QrcpProb{j.X, j.p, j.q, j.q, rk});
+      qp.push_back(QrcpProb{j.X, j.p, j.q, j.q, rk, 0, nullptr});
       rank_dev = rk;
       prow = std::min(j.p, j.q);  // the rows below are exact zeros after the QR
     }
@@ -238,7 +243,7 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
     s.chi_max = j.chi_max;
     sp.push_back(s);
   }
-  if (!qp.empty()) QTT_CU(qtt_launch_qrcp(qp.data(), (int)qp.size(), ctx->stream));
+  if (!qp.empty()) QTT_CU(qtt_launch_qrcp(qp.data(), (int)qp.size(), 1, ctx->stream));
   QTT_CU(qtt_launch_rowjacobi(jp.data(), (int)jp.size(), ctx->stream));
   QTT_CU(qtt_launch_select(sp.data(), (int)sp.size(), ctx->stream));
   jobs.clear();
