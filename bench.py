@@ -150,6 +150,29 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------- replicas (N > 1)
+def replica_seed(rank: int) -> int:
+    """The path does not shard ("replicas only"): rank r advances its own replica, whose
+    perturbation phases are drawn with seed r."""
+    return int(rank)
+
+
+def max_over_ranks(value: float, world: int, device: str = "cuda") -> float:
+    """MAX of a host scalar over the ranks of the default process group (identity for world == 1)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, ms_max: float) -> float:
+    """steps/s summed over all replicas: every rank did `steps` steps within the slowest rank's time."""
+    return world * steps / (ms_max * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------- our arm
 def fp64_peaks(Q, ctx):
     """Measured fp64 issue rates of this GPU (TFLOP/s): the DMMA.8x8x4 tensor pipe and the DFMA pipe."""
@@ -181,7 +204,7 @@ def run_ours(args):
     dx = 1.0 / (1 << n)
     Dx, Dy = Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx)
     Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
-    ux, uy = I.config_fields(args.config, seed=rank)
+    ux, uy = I.config_fields(args.config, seed=replica_seed(rank))
     u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
     ctx.synchronize()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -212,12 +235,9 @@ def run_ours(args):
     clocks = sampler.stop()
     ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
     launches = Q.qtt_ctx_launch_count(ctx) - launches0
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world)
     ms_per_step = ms / args.steps
-    value = world * args.steps / (ms * 1e-3)
+    value = whole_job_value(world, args.steps, ms)
 
     # ---- end to end through the C ABI with HOST buffers: cores in pinned host memory -> device, step, cores back
     host = [Q.qtt_mps_get_cores(ctx, x) for x in u]
@@ -233,10 +253,7 @@ def run_ours(args):
         d2h = sum(a.nbytes for cs in host for a in cs)
     torch.cuda.synchronize()
     e2e_sec = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_sec], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_sec = float(t.item())
+    e2e_sec = max_over_ranks(e2e_sec, world)
     e2e = {"value": world / e2e_sec, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
            "steps": e2e_steps}
 

@@ -19,7 +19,7 @@ namespace {
 constexpr int JNT = 512;
 constexpr int MAXC = 16;
 
-// dynamic shared memory (doubles): slice [p][wp] (if resident) | part [2][MAXC][3*np2] | rot [2*np2]
+// dynamic shared memory (doubles): slice [p][wp] (if resident) | part [2][C][3*np2] | rot [2*np2]
 //                                  | order (ints) [p_even] | counters
 __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constant__ JacGroup g, int pmax, int wp) {
   cg::cluster_group cluster = cg::this_cluster();
@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
   extern __shared__ __align__(16) double sm[];
   double* slice_sm = sm;
   double* part = sm + (g.use_smem ? (size_t)pmax * wp : 0);
-  double* rot = part + 2 * MAXC * 3 * np2_max;
+  double* rot = part + 2 * C * 3 * np2_max;
   int* flags = reinterpret_cast<int*>(rot + 2 * np2_max);  // [0] rotations this sweep
   // Largest squared row norm seen so far, identical in every CTA of the cluster (it is derived from the
   // exchanged totals only): [0] accumulates during phase B1, [1] is the value phase B1 reads.
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
         if (k < np2) {
           for (int dst = gl; dst < C; dst += tpp) {
             double* remote = (C > 1) ? cluster.map_shared_rank(part, dst) : part;
-            double* slot = remote + ((size_t)(par * MAXC + rank) * np2_max + k) * 3;
+            double* slot = remote + ((size_t)(par * C + rank) * np2_max + k) * 3;
             slot[0] = aa;
             slot[1] = bb;
             slot[2] = ab;
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
       for (int k = tid; k < np2; k += JNT) {
         double aa = 0.0, bb = 0.0, ab = 0.0;
         for (int src = 0; src < C; ++src) {
-          const double* slot = part + ((size_t)(par * MAXC + src) * np2_max + k) * 3;
+          const double* slot = part + ((size_t)(par * C + src) * np2_max + k) * 3;
           aa += slot[0];
           bb += slot[1];
           ab += slot[2];
@@ -732,7 +732,8 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
     }
     if (grp.nprob == 0) continue;
     const int pe = (pmax + 1) & ~1;
-    const size_t fixed = ((size_t)2 * MAXC * 3 * (pe / 2) + 2 * (pe / 2) + 8) * sizeof(double);
+    // exchange buffers [2][c][3 * pairs] + rotations: they grow with the cluster size c
+    auto fixed_for = [&](int c) { return ((size_t)2 * c * 3 * (pe / 2) + 2 * (pe / 2) + 8) * sizeof(double); };
     const size_t budget = 216 * 1024;
     // smallest cluster whose slice fits in shared memory, with at least ~16 columns per CTA
     int C = 1, use_smem = 0, w = 0, wp = 0;
@@ -740,7 +741,7 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
       int ww = (qmax + c - 1) / c;
       ww = (ww + 3) & ~3;
       int wpp = ww | 1;
-      size_t need = fixed + (size_t)pmax * wpp * sizeof(double);
+      size_t need = fixed_for(c) + (size_t)pmax * wpp * sizeof(double);
       if (need <= budget) {
         C = c; use_smem = 1; w = ww; wp = wpp;
         break;
@@ -749,22 +750,28 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
     if (use_smem) {
       // more CTAs when there is enough work per round: aim at <= ~8k slice elements per CTA
       while (C < MAXC && (size_t)pmax * w > 8192 && w >= 32) {
-        C *= 2;
-        w = (qmax + C - 1) / C;
-        w = (w + 3) & ~3;
+        const int c2 = C * 2;
+        int ww = (qmax + c2 - 1) / c2;
+        ww = (ww + 3) & ~3;
+        if (fixed_for(c2) + (size_t)pmax * (ww | 1) * sizeof(double) > budget) break;
+        C = c2;
+        w = ww;
         wp = w | 1;
       }
     } else {
+      // the matrix stays in global memory (L2): the largest cluster whose exchange buffers fit
       C = MAXC;
+      while (C > 1 && fixed_for(C) > budget) C /= 2;
+      if (fixed_for(C) > budget) return cudaErrorInvalidConfiguration;
       w = (qmax + C - 1) / C;
       w = (w + 3) & ~3;
       wp = 0;
-      if (fixed > budget) return cudaErrorInvalidConfiguration;
     }
+    const size_t fixed = fixed_for(C);
     grp.cluster = C;
     grp.use_smem = use_smem;
     grp.wslice = w;
-    grp.max_sweeps = 40;
+    grp.max_sweeps = 60;
     size_t smem = fixed + (use_smem ? (size_t)pmax * wp * sizeof(double) : 0);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(C * grp.nprob);

@@ -291,3 +291,72 @@ def test_errors_are_status_codes(Q, ctx):
     assert e.value.status == -2
     with pytest.raises(Q.QttError):
         Q.qtt_round(ctx, a, 0)
+
+
+# ---------------------------------------------------------------- full sizes, in bench.py's launch configuration
+@pytest.fixture(scope="module")
+def big_ctx(Q):
+    c = Q.Context(device=0, workspace_bytes=8 << 30)  # bench.py's default workspace
+    yield c
+    c.close()
+
+
+def schmidt_close(Q, ctx, x, cores):
+    """Per-bond Schmidt values of the GPU result against an independent canonicalisation of the oracle result."""
+    sg = Q.qtt_mps_schmidt(ctx, x)
+    so = O.schmidt_values(cores)
+    for k in range(1, len(cores)):
+        m = min(len(sg[k]), len(so[k]))
+        assert np.max(np.abs(np.asarray(sg[k][:m]) - so[k][:m])) <= 1e-9 * so[k][0]
+
+
+def test_rk4_config3_full_size_matches_oracle(Q, big_ctx):
+    """BASELINE config 3 (the bench workload: 2^10 x 2^10 decaying jet, chi 64, chi_work 128, Re 2e5, dt 5e-5):
+    one graph-replayed qtt_rk4_step against one oracle step, dense 1024 x 1024 fields and Schmidt spectra."""
+    import torch
+    cfg = I.CONFIGS[3]
+    n, chi = cfg["n"], cfg["chi"]
+    ux, uy = I.config_fields(3)
+    g, o = ops(Q, big_ctx, n)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    u = [Q.qtt_mps_from_cores(big_ctx, U[0]), Q.qtt_mps_from_cores(big_ctx, U[1])]
+    Q.qtt_ctx_set_graphs(big_ctx, True)
+    U1 = O.rk4_step(U, o[0], o[1], o[2], cfg["Re"], cfg["dt"], chi)
+    Q.qtt_rk4_step(big_ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+    for i in range(2):
+        assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+        assert rel(gpu_dense(Q, big_ctx, u[i]), O.to_dense(U1[i])) < TOL
+        schmidt_close(Q, big_ctx, u[i], U1[i])
+    assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
+    # from_dense at full size: the GPU TT-SVD of the dense field is the oracle's
+    v = Q.qtt_mps_from_dense(big_ctx, torch.from_numpy(ux).cuda(), chi)
+    assert rel(gpu_dense(Q, big_ctx, v), O.to_dense(U[0])) < TOL
+
+
+def test_config4_size_primitives_match_oracle(Q, big_ctx):
+    """BASELINE config 4 sizes (2^11 x 2^11 decaying turbulence, chi 128): the oracle needs ~13 min for a whole
+    step, so parity is taken primitive by primitive on the same inputs: from_dense, apply(Lap)+round,
+    apply(D1)+round and ONE product u_x (.) D1 u_x (zip-up, chi_work 256)."""
+    import torch
+    cfg = I.CONFIGS[4]
+    n, chi = cfg["n"], cfg["chi"]
+    ux, _ = I.config_fields(4)
+    g, o = ops(Q, big_ctx, n)
+    A = O.from_dense(ux, chi)
+    a = Q.qtt_mps_from_dense(big_ctx, torch.from_numpy(ux).cuda(), chi)
+    assert Q.qtt_mps_bonds(a) == O.bonds(A)
+    assert rel(gpu_dense(Q, big_ctx, a), O.to_dense(A)) < TOL
+    a = Q.qtt_mps_from_cores(big_ctx, A)
+    for which in (2, 0):
+        want = O.round_mps(O.apply_mpo(o[which], A), chi)
+        y = Q.qtt_apply_mpo(big_ctx, g[which], a)
+        Q.qtt_round(big_ctx, y, chi)
+        assert Q.qtt_mps_bonds(y) == O.bonds(want)
+        assert rel(gpu_dense(Q, big_ctx, y), O.to_dense(want)) < TOL
+    G = want  # round(D1 u_x)
+    P = O.round_product(A, G, chi)
+    c = Q.qtt_hadamard(big_ctx, a, y)
+    Q.qtt_round(big_ctx, c, chi)
+    assert Q.qtt_mps_bonds(c) == O.bonds(P)
+    assert rel(gpu_dense(Q, big_ctx, c), O.to_dense(P)) < TOL
+    assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
