@@ -275,6 +275,31 @@ def run_ours(args):
     return 0
 
 
+# dram bytes (read + write) per launch from the committed ncu --set full captures (profiles/), keyed by
+# (family, launch shape tag of qtt_diag_profile_dump)
+NCU_TRAFFIC_BYTES = {("rowjacobi", (512, 512, 4, 16)): 18.03e6}
+KERNEL_NAMES = {"rowjacobi": "qtt_blockjacobi_kernel", "qrcp": "qtt_qrcp_reg_kernel", "gemm": "qtt_gemm_dmma_kernel",
+                "lq_panel": "qtt_lq_panel_kernel / qtt_qrcp_kernel", "lq_update": "qtt_gemm_dmma_kernel",
+                "select": "qtt_select_kernel", "move": "movement kernels"}
+
+
+def launch_records(ctx):
+    """Per-launch (family, shape tag, ms, work) of the event-bracketed launches since the last report."""
+    import tempfile
+    fd, path = tempfile.mkstemp(suffix=".csv")
+    os.close(fd)
+    out = []
+    try:
+        if ctx.lib.qtt_diag_profile_dump(path.encode()) != 0:
+            return out
+        for ln in open(path).read().splitlines()[1:]:
+            f = ln.split(",")
+            out.append({"family": f[0], "shape": tuple(int(x) for x in f[1:5]), "ms": float(f[5]), "work": float(f[6])})
+    finally:
+        os.unlink(path)
+    return out
+
+
 def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     """Per-kernel-family device times of one more (eagerly launched, event-bracketed) step -> roofline of the
     dominant family; the site-contraction TFLOP/s; and the CPU oracle timed on a bounded sample."""
@@ -285,6 +310,7 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     nprof = 2
     for _ in range(nprof):
         Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+    per_launch = launch_records(ctx)  # before the report clears them
     rep = Q.qtt_ctx_profile_report(ctx)
     Q.qtt_ctx_profile(ctx, False)
     tot_ms = sum(v["ms"] for v in rep.values()) or 1.0
@@ -295,28 +321,41 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
                    "work_per_step": v["work"] / nprof}
     dom = max(rep, key=lambda k: rep[k]["ms"])
     d = rep[dom]
-    bound = {"gemm": "tensor", "lq_panel": "alu", "lq_update": "alu", "rowjacobi": "alu", "select": "hbm",
+    bound = {"gemm": "tensor", "lq_panel": "alu", "lq_update": "tensor", "rowjacobi": "alu", "select": "hbm",
              "move": "hbm", "qrcp": "alu"}[dom]
+    # the dominant KERNEL: the launch shape of the dominant family with the largest summed time
+    shapes = {}
+    for r in per_launch:
+        if r["family"] == dom:
+            a = shapes.setdefault(r["shape"], {"ms": 0.0, "work": 0.0, "n": 0})
+            a["ms"] += r["ms"]; a["work"] += r["work"]; a["n"] += 1
+    shape = max(shapes, key=lambda k: shapes[k]["ms"]) if shapes else None
+    k = shapes[shape] if shape else {"ms": d["ms"], "work": d["work"], "n": max(d["launches"], 1)}
     if bound == "hbm":
         try:
             peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
             src = "MEASURED_PEAKS.json hbm_gbs (of measured)"
         except Exception:
             peak, src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
-        achieved = d["work"] / (d["ms"] * 1e-3) * 1e-9
+        achieved = k["work"] / (k["ms"] * 1e-3) * 1e-9
         unit = "GB/s"
     else:
         peak = peaks["dmma"] if bound == "tensor" else peaks["dfma"]
         src = ("qtt_diag_fp64_probe, measured in this run: register-only " +
-               ("DMMA.8x8x4" if bound == "tensor" else "DFMA") + " issue rate (MEASURED_PEAKS.json has no fp64 figure)")
-        achieved = d["work"] / (d["ms"] * 1e-3) * 1e-12
+               ("DMMA.8x8x4" if bound == "tensor" else "DFMA") + " issue rate on all 148 SMs (MEASURED_PEAKS.json has "
+               "no fp64 figure; nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s, DESIGN.md section 6)")
+        achieved = k["work"] / (k["ms"] * 1e-3) * 1e-12
         unit = "TFLOP/s"
-    roof = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
-            "frac": achieved / peak if peak else None, "traffic": None, "peak_source": src,
-            "launches_per_step": d["launches"] // nprof, "avg_launch_ms": d["ms"] / max(d["launches"], 1),
-            "share_of_step_kernel_time": d["ms"] / tot_ms,
-            "algorithmic_work": "nominal SVD count 6ab^2+20b^3 per matrix (DESIGN.md)" if dom == "rowjacobi" else
-            "DESIGN.md per-family formulas"}
+    traffic = NCU_TRAFFIC_BYTES.get((dom, shape))
+    roof = {"kernel": KERNEL_NAMES.get(dom, dom) + (f" launch shape (d0,d1,d2,d3)={shape}" if shape else ""),
+            "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
+            "frac": achieved / peak if peak else None, "traffic": traffic, "peak_source": src,
+            "launches_per_step": k["n"] // nprof, "avg_launch_ms": k["ms"] / max(k["n"], 1),
+            "share_of_step_kernel_time": k["ms"] / tot_ms, "family_share_of_step_kernel_time": d["ms"] / tot_ms,
+            "algorithmic_work": "nominal SVD count 6ab^2+20b^3 per matrix (DESIGN.md section 6)" if dom == "rowjacobi"
+            else "DESIGN.md section 6 per-family formulas",
+            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
+            "launch shape (profiles/r1_blockjacobi_full.md)" if traffic else None}
     g = rep["gemm"]
     out = {"roofline": roof, "families": fams,
            "contraction": {"tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],

@@ -452,6 +452,324 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_kernel(const __grid_constant__ Q
   if (C > 1) cluster.sync();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Register-resident variant for p <= 32 * EPL rows and <= 32 columns per CTA: warp wi owns the local columns wi and
+// wi + 16 and keeps them in REGISTERS for the whole factorisation (lane l holds rows l, l + 32, ...), so a step
+// costs one shared-memory read of the reflector per row slab and four DFMA per element pair; shared memory only
+// carries the reflector, the pivot candidates and the staged pivot column.  The generic kernel above is
+// issue-bound at ~15k warp instructions per step and CTA (ncu, profiles/); this one executes about a third.
+// The step loop is unrolled over the 32-row slabs (JB = j / 32 is a compile-time constant inside the body), so
+// finished slabs cost nothing and the "diagonal" element is reached with a static register index.
+// Pivot-column slabs are staged round-robin: slab e goes to CTA e % C at offset (e / C) * 32 + lane.
+template <int EPL>
+__global__ void __launch_bounds__(QNT) qtt_qrcp_reg_kernel(const __grid_constant__ QrcpGroup g) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = g.cluster;
+  const int rank = (C > 1) ? (int)cluster.block_rank() : 0;
+  const QrcpProb& P = g.p[blockIdx.x / C];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int p = P.p, q = P.q;
+  const int w = g.w, pp = g.pp;
+  const bool pivot = g.pivot != 0;
+
+  extern __shared__ __align__(16) double sm[];
+  double* Xs = sm;
+  double* vb = Xs + (size_t)w * pp;  // 32 * EPL
+  double* red = vb + 32 * EPL;
+  double* diag = red + QNW;
+  double* xfro = diag + w;
+  long long* wval = reinterpret_cast<long long*>(xfro + MAXC);
+  long long* candv = wval + QNW;
+  int* wcol = reinterpret_cast<int*>(candv + 2 * MAXC);
+  int* candc = wcol + QNW;
+  int* stepidx = candc + 2 * MAXC;
+  const int chm = g.chm;
+  double* stage = reinterpret_cast<double*>(stepidx + ((w + 1) & ~1));  // [2][MAXC sources][chm]
+  auto stage_of = [&](int k) { return (C > 1) ? cluster.map_shared_rank(stage, k) : stage; };
+  auto barrier = [&]() {
+    if (C > 1) cluster.sync();
+    else __syncthreads();
+  };
+
+  const int wc = (q - rank + C - 1) / C;  // columns rank, rank + C, ... < q
+  if (P.transposed) {
+    for (int idx = tid; idx < p * wc; idx += QNT) {
+      const int x = idx / p, r = idx - x * p;
+      Xs[(size_t)x * pp + r] = P.X[(i64)(rank + C * x) * P.ld + r];
+    }
+  } else {
+    for (int idx = tid; idx < p * wc; idx += QNT) {
+      const int r = idx / wc, x = idx - r * wc;
+      Xs[(size_t)x * pp + r] = P.X[(i64)r * P.ld + rank + C * x];
+    }
+  }
+  for (int i = tid; i < 32 * EPL; i += QNT) vb[i] = 0.0;
+  __syncthreads();
+  // ---- my two columns into registers
+  const bool has0 = warp < wc, has1 = warp + QNW < wc;
+  const int col0g = rank + C * warp, col1g = rank + C * (warp + QNW);
+  double x0[EPL], x1[EPL];
+  double n0 = 0.0, n1 = 0.0;
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) {
+    const int i = lane + 32 * e;
+    x0[e] = (has0 && i < p) ? Xs[(size_t)warp * pp + i] : 0.0;
+    x1[e] = (has1 && i < p) ? Xs[(size_t)(warp + QNW) * pp + i] : 0.0;
+    n0 += x0[e] * x0[e];
+    n1 += x1[e] * x1[e];
+  }
+  int step0 = -1, step1 = -1;
+  double diag0 = 0.0, diag1 = 0.0, r0 = 0.0, r1 = 0.0;
+  double thresh2 = -1.0;
+  if (pivot) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      n0 += __shfl_xor_sync(0xffffffffu, n0, o);
+      n1 += __shfl_xor_sync(0xffffffffu, n1, o);
+    }
+    r0 = n0;
+    r1 = n1;
+    if (lane == 0) red[warp] = n0 + n1;
+    __syncthreads();
+    double myfro = 0.0;
+    for (int i = 0; i < QNW; ++i) myfro += red[i];
+    if (C > 1) {
+      if (tid < C) {
+        double* remote = cluster.map_shared_rank(xfro, tid);
+        remote[rank] = myfro;
+      }
+      cluster.sync();
+    } else if (tid == 0) {
+      xfro[0] = myfro;
+    }
+    __syncthreads();
+    double fro2 = 0.0;
+    for (int c2 = 0; c2 < C; ++c2) fro2 += xfro[c2];
+    thresh2 = 3.1554436208840472e-30 * fro2;  // (8 eps)^2 ||X||_F^2
+  }
+  __syncthreads();
+
+  const int rmax = min(p, q);
+  int nsteps = 0;
+  bool stop = false;
+#pragma unroll
+  for (int JB = 0; JB < EPL; ++JB) {
+    if (stop || 32 * JB >= rmax) break;
+    for (int jj = 0; jj < 32; ++jj) {
+      const int j = 32 * JB + jj;
+      if (j >= rmax) {
+        stop = true;
+        break;
+      }
+      const int par = j & 1;
+      const bool live0 = has0 && step0 < 0, live1 = has1 && step1 < 0;
+      int gcol = j;
+      int stage_col = -1;  // global column this CTA stages before the barrier
+      if (pivot) {
+        long long bv = live0 ? norm_key(n0) : -1ll;
+        int bc = live0 ? col0g : 0x7fffffff;
+        const long long v1 = live1 ? norm_key(n1) : -1ll;
+        if (v1 > bv) {
+          bv = v1;
+          bc = col1g;
+        }
+        if (lane == 0) {
+          wval[warp] = bv;
+          wcol[warp] = bc;
+        }
+        __syncthreads();
+        bv = wval[lane & 15];
+        bc = wcol[lane & 15];
+        warp_argmax16(bv, bc);
+        if (C > 1 && warp == 0 && lane < C) {
+          long long* rv = cluster.map_shared_rank(candv, lane);
+          int* rc = cluster.map_shared_rank(candc, lane);
+          rv[par * MAXC + rank] = bv;
+          rc[par * MAXC + rank] = bc;
+        }
+        if (bv >= 0) stage_col = bc;
+        gcol = bc;
+        // (the global winner is known after the barrier)
+        if (C == 1 && (bv < 0 || !(__longlong_as_double(bv) > thresh2))) {
+          stop = true;
+          break;
+        }
+      } else if (rank == j % C) {
+        stage_col = j;
+      }
+      // ---- the owning warp stages its column (rows >= j) slab by slab in the peers
+      if (stage_col >= 0 && ((live0 && stage_col == col0g) || (live1 && stage_col == col1g))) {
+        const bool is0 = live0 && stage_col == col0g;
+#pragma unroll
+        for (int e = JB; e < EPL; ++e) {
+          if (32 * e < p) {
+            double* dst = stage_of(e % C);
+            dst[(size_t)(par * MAXC + rank) * chm + (e / C) * 32 + lane] = is0 ? x0[e] : x1[e];
+          }
+        }
+      }
+      barrier();
+      if (pivot && C > 1) {
+        long long gval = (lane & 15) < C ? candv[par * MAXC + (lane & 15)] : -1ll;
+        gcol = (lane & 15) < C ? candc[par * MAXC + (lane & 15)] : 0x7fffffff;
+        warp_argmax16(gval, gcol);
+        if (gval < 0 || !(__longlong_as_double(gval) > thresh2)) {  // what is left is rounding noise (uniform)
+          stop = true;
+          break;
+        }
+      }
+      nsteps = j + 1;
+      const int owner = gcol % C, lc = gcol / C;
+      // ---- gather the pivot column (one row per thread); sum of squares of the rows below j on the way
+      {
+        double s = 0.0;
+        const int i = tid;  // slab = warp
+        if (i >= j && i < p) {
+          const double* src = stage_of(warp % C);
+          const double x = src[(size_t)(par * MAXC + owner) * chm + (warp / C) * 32 + lane];
+          vb[i] = x;
+          if (i > j) s = x * x;
+        }
+        s = warp_sum(s);
+        if (lane == 0) red[warp] = s;
+      }
+      __syncthreads();
+      double sigma = red[lane & 15];
+      sigma += __shfl_xor_sync(0xffffffffu, sigma, 8);
+      sigma += __shfl_xor_sync(0xffffffffu, sigma, 4);
+      sigma += __shfl_xor_sync(0xffffffffu, sigma, 2);
+      sigma += __shfl_xor_sync(0xffffffffu, sigma, 1);
+      const double alpha = vb[j];
+      double beta = alpha, tau = 0.0, scale = 0.0;
+      if (sigma > 0.0) {
+        const double n2 = alpha * alpha + sigma;
+        double r = rsqrt(n2);
+        r = r * (1.5 - 0.5 * n2 * r * r);
+        double nr = n2 * r;
+        nr = nr + 0.5 * r * (n2 - nr * nr);  // sqrt(n2) to full accuracy
+        const double aa = fabs(alpha);
+        beta = -copysign(nr, alpha);
+        tau = 1.0 + aa * r;
+        scale = copysign(1.0 / (aa + nr), alpha);
+      }
+      bool upd0 = live0, upd1 = live1;
+      if (rank == owner) {
+        if (live0 && col0g == gcol) {
+          step0 = j;
+          diag0 = beta;
+          upd0 = false;
+        }
+        if (live1 && col1g == gcol) {
+          step1 = j;
+          diag1 = beta;
+          upd1 = false;
+        }
+      }
+      (void)lc;
+      // ---- apply:  dot = col[j] + scale * sum_{i>j} v_i col_i;  col[j] -= tau dot;  col_i -= (tau dot scale) v_i
+      if ((upd0 || upd1) && (tau != 0.0 || pivot)) {
+        double dot0 = 0.0, dot1 = 0.0;
+#pragma unroll
+        for (int e = JB; e < EPL; ++e) {
+          double v = vb[lane + 32 * e];
+          if (e == JB && lane <= jj) v = 0.0;
+          dot0 += v * x0[e];
+          dot1 += v * x1[e];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          dot0 += __shfl_xor_sync(0xffffffffu, dot0, o);
+          dot1 += __shfl_xor_sync(0xffffffffu, dot1, o);
+        }
+        const double cj0 = __shfl_sync(0xffffffffu, x0[JB], jj), cj1 = __shfl_sync(0xffffffffu, x1[JB], jj);
+        const double d0 = upd0 ? (cj0 + scale * dot0) * tau : 0.0, d1 = upd1 ? (cj1 + scale * dot1) * tau : 0.0;
+        const double ds0 = d0 * scale, ds1 = d1 * scale;
+        const double nj0 = cj0 - d0, nj1 = cj1 - d1;
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int e = JB; e < EPL; ++e) {
+          double v = vb[lane + 32 * e];
+          if (e == JB && lane <= jj) v = 0.0;
+          x0[e] -= ds0 * v;
+          x1[e] -= ds1 * v;
+          if (!(e == JB && lane <= jj)) {
+            s0 += x0[e] * x0[e];
+            s1 += x1[e] * x1[e];
+          }
+        }
+        if (lane == jj) {
+          if (upd0) x0[JB] = nj0;
+          if (upd1) x1[JB] = nj1;
+        }
+        if (pivot) {
+          if (upd0) n0 -= nj0 * nj0;
+          if (upd1) n1 -= nj1 * nj1;
+          const bool re0 = upd0 && !(n0 > 1.5e-8 * r0), re1 = upd1 && !(n1 > 1.5e-8 * r1);
+          if (re0 || re1) {  // warp-uniform: the downdated norm has lost 8 digits, take the exact one
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+              s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+              s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            }
+            if (re0) n0 = r0 = s0;
+            if (re1) n1 = r1 = s1;
+          }
+        }
+      }
+    }
+  }
+  // ---- registers -> shared memory, then the coalesced write-out
+  __syncthreads();
+#pragma unroll
+  for (int e = 0; e < EPL; ++e) {
+    const int i = lane + 32 * e;
+    if (has0 && i < p) Xs[(size_t)warp * pp + i] = x0[e];
+    if (has1 && i < p) Xs[(size_t)(warp + QNW) * pp + i] = x1[e];
+  }
+  if (lane == 0) {
+    if (has0) {
+      stepidx[warp] = step0;
+      diag[warp] = diag0;
+    }
+    if (has1) {
+      stepidx[warp + QNW] = step1;
+      diag[warp + QNW] = diag1;
+    }
+  }
+  __syncthreads();
+  if (P.R_out) {
+    for (int idx = tid; idx < q * wc; idx += QNT) {
+      const int r = idx / wc, x = idx - r * wc;
+      const int s = stepidx[x];
+      double v = 0.0;
+      if (r < nsteps) {
+        if (s < 0 || r < s) v = Xs[(size_t)x * pp + r];
+        else if (r == s) v = diag[x];
+      }
+      P.R_out[(i64)r * q + rank + C * x] = v;
+    }
+  } else {
+    for (int idx = tid; idx < p * wc; idx += QNT) {
+      const int r = idx / wc, x = idx - r * wc;
+      const int s = stepidx[x];
+      double v = 0.0;
+      if (r < nsteps) {
+        if (s < 0 || r < s) v = Xs[(size_t)x * pp + r];
+        else if (r == s) v = diag[x];
+      }
+      P.X[(i64)r * P.ld + rank + C * x] = v;
+    }
+  }
+  if (rank == 0 && tid == 0 && P.rank_out) P.rank_out[0] = nsteps;
+  if (C > 1) cluster.sync();  // no CTA may leave while a peer can still read its shared memory
+}
+
+size_t qrcp_reg_smem_bytes(int w, int pp, int epl, int chm) {
+  const size_t doubles = (size_t)w * pp + 32 * (size_t)epl + QNW + (size_t)w + MAXC + QNW + 2 * MAXC;
+  const size_t ints = QNW + 2 * MAXC + (((size_t)w + 1) & ~(size_t)1);
+  return (doubles + 2 * MAXC * (size_t)chm) * sizeof(double) + ints * sizeof(int) + 16;
+}
+
 size_t qrcp_smem_bytes(int w, int pp, int chm) {
   const size_t doubles = (size_t)w * pp + pp + QNW + 3 * (size_t)w + MAXC + QNW + 2 * MAXC;  // incl. the 64-bit keys
   const size_t ints = QNW + 2 * MAXC + (((size_t)w + 1) & ~(size_t)1);
@@ -466,14 +784,10 @@ int qrcp_cluster(int q) {
   return c2 > MAXC ? MAXC : c2;
 }
 
-template <int EPL>
-cudaError_t launch_qrcp(const QrcpGroup& g, size_t smem, double flops, int pmax, int qmax, cudaStream_t stream) {
-  static bool attr_done = false;
-  if (!attr_done) {
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_qrcp_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024));
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_qrcp_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    attr_done = true;
-  }
+template <class K>
+cudaError_t launch_qrcp(K kern, const QrcpGroup& g, size_t smem, double flops, int pmax, int qmax, cudaStream_t stream) {
+  QTT_CHECK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024));
+  QTT_CHECK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(g.cluster * g.nprob);
   cfg.blockDim = dim3(QNT);
@@ -487,7 +801,7 @@ cudaError_t launch_qrcp(const QrcpGroup& g, size_t smem, double flops, int pmax,
   cfg.attrs = at;
   cfg.numAttrs = 1;
   QttProf prof(g.pivot ? QK_QRCP : QK_LQ_PANEL, stream, flops, pmax, qmax, g.nprob, g.pivot ? g.cluster : -g.cluster);
-  return cudaLaunchKernelEx(&cfg, qtt_qrcp_kernel<EPL>, g);
+  return cudaLaunchKernelEx(&cfg, kern, g);
 }
 
 }  // namespace
@@ -518,13 +832,22 @@ cudaError_t qtt_launch_qrcp(const QrcpProb* probs, int n, int pivot, cudaStream_
     g.cluster = C;
     g.w = (qmax + C - 1) / C;
     g.pp = pmax | 1;
-    g.chm = (pmax + C - 1) / C;
-    const size_t smem = qrcp_smem_bytes(g.w, g.pp, g.chm);
-    if (smem > 224 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e;
-    if (pmax <= 256) e = launch_qrcp<8>(g, smem, flops, pmax, qmax, stream);
-    else if (pmax <= 512) e = launch_qrcp<16>(g, smem, flops, pmax, qmax, stream);
-    else e = launch_qrcp<0>(g, smem, flops, pmax, qmax, stream);
+    if (pmax <= 512 && g.w <= 2 * QNW) {
+      // register-resident columns
+      const int epl = pmax <= 128 ? 4 : (pmax <= 256 ? 8 : 16);
+      g.chm = 32 * ((epl + C - 1) / C);
+      const size_t smem = qrcp_reg_smem_bytes(g.w, g.pp, epl, g.chm);
+      if (smem > 224 * 1024) return cudaErrorInvalidConfiguration;
+      if (epl == 4) e = launch_qrcp(qtt_qrcp_reg_kernel<4>, g, smem, flops, pmax, qmax, stream);
+      else if (epl == 8) e = launch_qrcp(qtt_qrcp_reg_kernel<8>, g, smem, flops, pmax, qmax, stream);
+      else e = launch_qrcp(qtt_qrcp_reg_kernel<16>, g, smem, flops, pmax, qmax, stream);
+    } else {
+      g.chm = (pmax + C - 1) / C;
+      const size_t smem = qrcp_smem_bytes(g.w, g.pp, g.chm);
+      if (smem > 224 * 1024) return cudaErrorInvalidConfiguration;
+      e = launch_qrcp(qtt_qrcp_kernel<0>, g, smem, flops, pmax, qmax, stream);
+    }
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
