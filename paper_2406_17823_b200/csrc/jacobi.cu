@@ -265,9 +265,8 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
   const int Ce = max(1, (p + 2 * bmax - 1) / (2 * bmax));  // CTAs that take part (<= C)
   if (rank >= Ce) return;
   const int q = P.q;
-  const int pitch = ((q + BJ_G - 1) / BJ_G) * BJ_G;  // <= pitchmax
+  constexpr int pitch = BJ_G * EPL;  // every row is zero-padded to the full lane footprint (== pitchmax)
   const int b = (p + 2 * Ce - 1) / (2 * Ce);         // <= bmax
-  const int ne = pitch / BJ_G;                       // elements per lane actually used (<= EPL)
 
   extern __shared__ __align__(16) double sm[];
   const int bme = (bmax + 1) & ~1;
@@ -328,7 +327,7 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         double sq = 0.0;
 #pragma unroll
         for (int e = 0; e < EPL; ++e)
-          if (e < ne) sq += row[e * BJ_G] * row[e * BJ_G];
+          sq += row[e * BJ_G] * row[e * BJ_G];
         sq = warp_sum1(sq);
         if (lane == 0) S[data_sz + r] = sq;
       }
@@ -353,17 +352,18 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         }
         const bool live = ia < b && ib < b;
         double a[EPL], v[EPL];
-        double ab = 0.0;
+        double ab = 0.0, ab2 = 0.0;
         double* ra = S + (size_t)(live ? ia : 0) * pitch + lane;
         double* rb = S + (size_t)(live ? ib : 0) * pitch + lane;
         if (live) {
 #pragma unroll
-          for (int e = 0; e < EPL; ++e)
-            if (e < ne) {
-              a[e] = ra[e * BJ_G];
-              v[e] = rb[e * BJ_G];
-              ab += a[e] * v[e];
-            }
+          for (int e = 0; e < EPL; ++e) {
+            a[e] = ra[e * BJ_G];
+            v[e] = rb[e * BJ_G];
+            if (e & 1) ab2 += a[e] * v[e];
+            else ab += a[e] * v[e];
+          }
+          ab += ab2;
         }
         ab = warp_sum1(ab);
         if (live) {
@@ -371,11 +371,10 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
           const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
           if (R.apply) {
 #pragma unroll
-            for (int e = 0; e < EPL; ++e)
-              if (e < ne) {
-                ra[e * BJ_G] = R.c * a[e] - R.s * v[e];
-                rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
-              }
+            for (int e = 0; e < EPL; ++e) {
+              ra[e * BJ_G] = R.c * a[e] - R.s * v[e];
+              rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
+            }
             if (lane == 0) {
               S[data_sz + ia] = fmax(aa - R.t * ab, 0.0);
               S[data_sz + ib] = fmax(bb + R.t * ab, 0.0);
@@ -395,38 +394,36 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         const bool have = i < b;
         double a[EPL];
         double aa = 0.0;
-        double* rt = T + (size_t)(have ? i : 0) * pitch + lane;
+        double* rt = T + (have ? i : 0) * pitch + lane;
         if (have) {
 #pragma unroll
-          for (int e = 0; e < EPL; ++e)
-            if (e < ne) a[e] = rt[e * BJ_G];
+          for (int e = 0; e < EPL; ++e) a[e] = rt[e * BJ_G];
           aa = T[data_sz + i];
         }
         int j = have ? i : 0;
         for (int r = 0; r < b; ++r) {
-          double v[EPL];
-          double ab = 0.0;
-          double* rb = B + (size_t)j * pitch + lane;
+          double ab = 0.0, ab2 = 0.0, bb = 0.0;
+          double* rb = B + j * pitch + lane;
           if (have) {
+            bb = B[data_sz + j];
 #pragma unroll
-            for (int e = 0; e < EPL; ++e)
-              if (e < ne) {
-                v[e] = rb[e * BJ_G];
-                ab += a[e] * v[e];
-              }
+            for (int e = 0; e < EPL; ++e) {
+              const double ve = rb[e * BJ_G];
+              if (e & 1) ab2 += a[e] * ve;
+              else ab += a[e] * ve;
+            }
           }
-          ab = warp_sum1(ab);
+          ab = warp_sum1(ab + ab2);
           if (have) {
-            const double bb = B[data_sz + j];
             const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
             if (R.apply) {
 #pragma unroll
-              for (int e = 0; e < EPL; ++e)
-                if (e < ne) {
-                  const double an = R.c * a[e] - R.s * v[e];
-                  rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
-                  a[e] = an;
-                }
+              for (int e = 0; e < EPL; ++e) {  // the bottom row is read again: keeping it live costs spills
+                const double ve = rb[e * BJ_G];
+                const double an = R.c * a[e] - R.s * ve;
+                rb[e * BJ_G] = R.s * a[e] + R.c * ve;
+                a[e] = an;
+              }
               aa = fmax(aa - R.t * ab, 0.0);
               if (lane == 0) {
                 B[data_sz + j] = fmax(bb + R.t * ab, 0.0);
@@ -439,8 +436,7 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
         }
         if (have) {
 #pragma unroll
-          for (int e = 0; e < EPL; ++e)
-            if (e < ne) rt[e * BJ_G] = a[e];
+          for (int e = 0; e < EPL; ++e) rt[e * BJ_G] = a[e];
           if (lane == 0) T[data_sz + i] = aa;
         }
       }
@@ -655,7 +651,7 @@ bool blockjacobi_config(int pmax, int qmax, int& EPL, int& C, int& b, int& pitch
   else if (qmax <= 256) EPL = 8;
   else if (qmax <= 512) EPL = 16;
   else return false;
-  pitch = ((qmax + BJ_G - 1) / BJ_G) * BJ_G;
+  pitch = BJ_G * EPL;
   C = (pmax + 31) / 32;
   C = C < 1 ? 1 : (C > MAXC ? MAXC : C);
   b = (pmax + 2 * C - 1) / (2 * C);

@@ -360,3 +360,27 @@ def test_config4_size_primitives_match_oracle(Q, big_ctx):
     assert Q.qtt_mps_bonds(c) == O.bonds(P)
     assert rel(gpu_dense(Q, big_ctx, c), O.to_dense(P)) < TOL
     assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
+
+
+@pytest.mark.parametrize("chi", [16, 32])
+def test_config5_primitive_sweep_matches_oracle(Q, big_ctx, chi):
+    """BASELINE config 5 (2^12 x 2^12, random left-canonical MPS, batch of 6 operands per launch): every operand gets
+    one apply (d/dx, d/dy or Laplacian) + round(chi) and one Hadamard with the next operand + round(chi), batched
+    through qtt_round_batch; dense 4096 x 4096 reconstructions against the oracle."""
+    n = 12
+    g, o = ops(Q, big_ctx, n)
+    cores = [O.canonical_random(I.random_cores(n, chi, seed=s)) for s in range(6)]
+    xs = [Q.qtt_mps_from_cores(big_ctx, c) for c in cores]
+    ys = [Q.qtt_apply_mpo(big_ctx, g[i % 3], xs[i]) for i in range(6)]
+    Q.qtt_round_batch(big_ctx, ys, chi)
+    for i in (0, 2, 5):  # sampled operands: the oracle needs a few seconds per dense 2^24-point reconstruction
+        want = O.round_mps(O.apply_mpo(o[i % 3], cores[i]), chi)
+        assert Q.qtt_mps_bonds(ys[i]) == O.bonds(want)
+        assert rel(gpu_dense(Q, big_ctx, ys[i]), O.to_dense(want)) < TOL
+    hs = [Q.qtt_hadamard(big_ctx, xs[i], xs[(i + 1) % 6]) for i in range(6)]
+    Q.qtt_round_batch(big_ctx, hs, chi)
+    for i in (1, 4):
+        want = O.round_product(cores[i], cores[(i + 1) % 6], chi)
+        assert Q.qtt_mps_bonds(hs[i]) == O.bonds(want)
+        assert rel(gpu_dense(Q, big_ctx, hs[i]), O.to_dense(want)) < TOL
+    assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
