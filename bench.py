@@ -29,7 +29,8 @@ if ROOT not in sys.path:
 
 import qtt_inputs as I  # noqa: E402
 
-METRIC = "QTT RK4 steps/sec at 2^10x2^10, chi=64 fp64"
+METRIC = "QTT RK4 steps/sec at 2^10x2^10, chi=64 fp64"  # BASELINE.json's metric (config 3, the default workload)
+METRICS = {2: "QTT RK4 steps/sec at 2^8x2^8, chi=32 fp64", 3: METRIC, 4: "QTT RK4 steps/sec at 2^11x2^11, chi=128 fp64"}
 UNIT = "steps/s"
 
 
@@ -138,7 +139,7 @@ def run_reference(args):
     val = 1.0 / sec
     cores = blas_threads()
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": METRICS[args.config], "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "note": "CPU oracle (NumPy fp64 + LAPACK) on the host cores; each step is a "
@@ -258,7 +259,7 @@ def run_ours(args):
            "steps": e2e_steps}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRICS[args.config], "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "l2": "256 MiB buffer zeroed between timed steps, outside the per-step CUDA "
@@ -298,6 +299,40 @@ def launch_records(ctx):
     finally:
         os.unlink(path)
     return out
+
+
+def contraction_probe(ctx, chi, peak):
+    """The two GEMM passes of the row-a2 site contraction at the bulk-site shapes of bond chi (working bond 2 chi,
+    4 operands per launch, as in qtt_rk4_step), run through the same grouped DMMA kernel (qtt_diag_gemm) on random
+    operands: X[r,b,(w,a')] = sum_a R[r,a,b] A[a,(w,a')] and T[(r,a'),b'] = sum_b X[(r,a'),b] B[b,b'] per omega."""
+    import ctypes as C
+    import torch
+    r = 2 * chi
+    st = C.c_void_p(ctx.stream.cuda_stream)
+    shapes = [(4 * chi, chi, chi, 4 * r, 1), (r * chi, chi, chi, 16, 0)]  # (M, N, K, nbatch, transA)
+    tot_ms, tot_fl = 0.0, 0.0
+    with torch.cuda.stream(ctx.stream):
+        for (M, N, K, nb, ta) in shapes:
+            A = torch.randn(nb * M * K, dtype=torch.float64, device="cuda")
+            B = torch.randn(nb * K * N, dtype=torch.float64, device="cuda")
+            Cm = torch.empty(nb * M * N, dtype=torch.float64, device="cuda")
+            def go():
+                return ctx.lib.qtt_diag_gemm(st, C.c_void_p(A.data_ptr()), C.c_void_p(B.data_ptr()), C.c_void_p(Cm.data_ptr()),
+                                             M, N, K, ta, 0, M if ta else K, N, N, 1.0, 0.0, nb, M * K, K * N, M * N)
+            for _ in range(3):
+                assert go() == 0
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(ctx.stream)
+            for _ in range(5):
+                go()
+            e1.record(ctx.stream)
+            e1.synchronize()
+            tot_ms += e0.elapsed_time(e1) / 5
+            tot_fl += 2.0 * M * N * K * nb
+    tf = tot_fl / (tot_ms * 1e-3) * 1e-12
+    return {"tflops": tf, "peak_tflops": peak, "frac": tf / peak if peak else None, "chi": chi,
+            "what": "both GEMM passes of the row-a2 site contraction at the chi=128 bulk-site shapes (config 4 / config 5), "
+                    "4 operands per launch, operands larger than L2 in total (0.5 GiB), CUDA events on the launching stream"}
 
 
 def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
@@ -357,7 +392,18 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
             "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
             "launch shape (profiles/r1_blockjacobi_full.md)" if traffic else None}
     g = rep["gemm"]
+    # the Hadamard site contractions proper at the bulk sites of this workload:
+    # pass 1 (4 chi x chi x chi, batched over the working bond) and pass 2 (2 chi^2 x chi x chi, batched over omega)
+    a2 = [r for r in per_launch if r["family"] == "gemm" and r["shape"][1] == chi and r["shape"][2] == chi
+          and r["shape"][0] in (4 * chi, 2 * chi * chi)]
+    a2_ms, a2_work = sum(r["ms"] for r in a2), sum(r["work"] for r in a2)
     out = {"roofline": roof, "families": fams,
+           "contraction_a2": {"tflops": a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],
+                              "frac": (a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,
+                              "launches_per_step": len(a2) // nprof,
+                              "what": f"row a2 only: the two DMMA GEMM passes of the Hadamard site contraction at the bulk "
+                                      f"sites (chi={chi}, working bond {2 * chi}), inside the profiled steps"},
+           "contraction_chi128": contraction_probe(ctx, 128, peaks["dmma"]),
            "contraction": {"tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],
                            "frac": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,
                            "what": "sum 2MNK of all DMMA site-contraction GEMMs of a step / their summed kernel time"},
