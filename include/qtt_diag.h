@@ -26,6 +26,12 @@ int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, do
  * [1] += matrices that hit the sweep limit.  SURVEY.md section 8 row a5. */
 int qtt_diag_rowjacobi(void* stream, double* X_dev, int batch, int p, int q, int ld, int* status_dev);
 
+/* The same iteration for matrices too large for a cluster's shared memory (q <= 1024 columns, any p): L2-streamed
+ * block Jacobi, one launch per tournament round over 16-row blocks, a static number of launches that return at once
+ * after convergence.  work_dev: 8 doubles of scratch per matrix.  SURVEY.md section 8 row a6 (chi = 128). */
+int qtt_diag_rowjacobi_streamed(void* stream, double* X_dev, int batch, int p, int q, int ld, int* status_dev,
+                                double* work_dev);
+
 /* The production SVD front end on `batch` matrices X_i (p x q, ld, stride p*ld), in place: rank-revealing
  * Householder QR with column pivoting X <- Q^T X (columns stay in place, rows from the numerical rank on are
  * exact zeros, rank_dev[i] <- rank), then -- unless status_dev is NULL -- one-sided Jacobi on the first

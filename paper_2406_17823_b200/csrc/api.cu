@@ -838,9 +838,23 @@ int qtt_diag_rowjacobi(void* stream, double* X, int batch, int p, int q, int ld,
     probs[i].X = X + (size_t)i * p * ld;
     probs[i].p = p; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = nullptr;
+    probs[i].work = nullptr;
     probs[i].status = status;
   }
   return (int)qtt_launch_rowjacobi(probs.data(), batch, static_cast<cudaStream_t>(stream));
+}
+
+int qtt_diag_rowjacobi_streamed(void* stream, double* X, int batch, int p, int q, int ld, int* status, double* work) {
+  if (!qtt_sbj_fits(p, q) || !work) return (int)cudaErrorInvalidConfiguration;
+  std::vector<JacProb> probs(batch);
+  for (int i = 0; i < batch; ++i) {
+    probs[i].X = X + (size_t)i * p * ld;
+    probs[i].p = p; probs[i].q = q; probs[i].ld = ld;
+    probs[i].p_dev = nullptr;
+    probs[i].work = work + 8 * (size_t)i;
+    probs[i].status = status;
+  }
+  return (int)qtt_launch_sbj(probs.data(), batch, static_cast<cudaStream_t>(stream));
 }
 
 int qtt_diag_svd_rows(void* stream, double* X, int batch, int p, int q, int ld, int* rank_dev, int* status) {
@@ -853,6 +867,7 @@ int qtt_diag_svd_rows(void* stream, double* X, int batch, int p, int q, int ld, 
     probs[i].X = qp[i].X;
     probs[i].p = p < q ? p : q; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = rank_dev + i;
+    probs[i].work = nullptr;
     probs[i].status = status;
   }
   cudaError_t e = qtt_launch_qrcp(qp.data(), batch, 1, st);

@@ -80,6 +80,7 @@ struct JacProb {
   double* X;
   int p, q, ld;
   const int* p_dev;  // if non-null: number of rows to rotate (<= p), read on the device (numerical rank from qrcp)
+  double* work;      // 8 doubles of device scratch (any content) for the L2-streamed path, or null
   int* status;  // device ints, may be shared by all problems: [0] <- max(sweeps used), [1] += 1 if the sweep limit was hit
 };
 #define QTT_JAC_MAX_BATCH 16
@@ -92,6 +93,9 @@ struct JacGroup {
   JacProb p[QTT_JAC_MAX_BATCH];
 };
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream);
+// L2-streamed block Jacobi (sbj.cu) for q <= 1024 columns, any number of rows; needs JacProb::work.
+cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream);
+bool qtt_sbj_fits(int p, int q);
 
 // Cluster-resident Householder QR of X (p x q, rows contiguous, ld), one cluster per matrix, column slices in
 // shared memory (qrcp.cu).

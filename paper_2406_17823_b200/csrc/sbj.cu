@@ -1,0 +1,291 @@
+// L2-streamed block Jacobi: the one-sided (Hestenes) Jacobi SVD of jacobi.cu for matrices too large for a
+// cluster's shared memory (512 < q <= 1024 columns; any number of rows), e.g. the 1024 x 1024 triangular factor of
+// the zip-up at chi = 128.
+//
+// The p rows are cut into P blocks of 16 rows (P even).  One LAUNCH per round of the round-robin tournament over
+// the blocks: every CTA takes one block pair, keeps the rows of its "top" block in registers (one warp per row,
+// lane l holds columns l, l + 32, ...), the "bot" block in shared memory, lets every top row meet every bot row
+// (16 inner rounds of 16 disjoint pairs, exactly the inner loop of the cluster-resident kernel) and writes both
+// blocks back; the matrix lives in L2 between the launches.  The pairs inside a block are done by one more launch
+// per sweep.  With 4 operands of 1024 rows a round is 128 CTAs, one wave on 148 SMs.  The number of launches is
+// static (CUDA-graph friendly): max_sweeps x P of them; after convergence (a sweep without a rotation of
+// cos^2 > 1e-15) the remaining launches return at once.
+//
+// Scratch per problem (JacProb::work, 8 doubles): [0] ||X||_F^2, [1] converged flag, [2] "big" rotations of the
+// current sweep, [3] sweeps done.
+#include "common.cuh"
+#include "jacobi_rot.cuh"
+
+namespace {
+
+constexpr int SB = 16;    // rows per block
+constexpr int SNTH = 512;  // 16 warps: one per top row
+constexpr int SEPL = 32;   // elements per lane: q <= 1024
+constexpr int SPITCH = 32 * SEPL;
+
+struct SbjGroup {
+  int nprob;
+  int P;       // blocks per matrix (even), largest problem
+  int round;   // 0 .. P-2
+  int sweep;
+  int max_sweeps;
+  JacProb p[QTT_JAC_MAX_BATCH];
+};
+
+__device__ __forceinline__ int sbj_rows(const JacProb& P) { return P.p_dev ? min(P.p, P.p_dev[0]) : P.p; }
+
+// ||X||_F^2 -> work[0]; clears the flags.  One CTA per problem.
+__global__ void __launch_bounds__(SNTH) qtt_sbj_init_kernel(const __grid_constant__ SbjGroup g) {
+  const JacProb& P = g.p[blockIdx.x];
+  const int p = sbj_rows(P), q = P.q;
+  __shared__ double red[SNTH / 32];
+  double s = 0.0;
+  for (i64 idx = threadIdx.x; idx < (i64)p * q; idx += SNTH) {
+    const int r = (int)(idx / q), x = (int)(idx - (i64)r * q);
+    const double v = P.X[(i64)r * P.ld + x];
+    s += v * v;
+  }
+  s = warp_sum1(s);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int i = 0; i < SNTH / 32; ++i) t += red[i];
+    P.work[0] = t;
+    P.work[1] = (p < 2) ? 1.0 : 0.0;
+    P.work[2] = 0.0;
+    P.work[3] = 0.0;
+  }
+}
+
+// End of a sweep: converged if no big rotation happened; books the sweep count / the limit hit.
+__global__ void qtt_sbj_check_kernel(const __grid_constant__ SbjGroup g) {
+  const JacProb& P = g.p[blockIdx.x];
+  if (threadIdx.x != 0) return;
+  if (P.work[1] != 0.0) return;
+  P.work[3] += 1.0;
+  if (P.work[2] == 0.0) P.work[1] = 1.0;
+  P.work[2] = 0.0;
+  const bool last = g.sweep + 1 == g.max_sweeps;
+  if (P.status && (P.work[1] != 0.0 || last)) {
+    atomicMax(&P.status[0], (int)P.work[3]);
+    if (P.work[1] == 0.0) atomicAdd(&P.status[1], 1);
+  }
+}
+
+// round-robin pairing of P players (P even) in round t: pair k of P/2
+__device__ __forceinline__ void rr_pair(int P, int t, int k, int& ia, int& ib) {
+  if (k == 0) {
+    ia = P - 1;
+    ib = t;
+  } else {
+    ia = (t + k) % (P - 1);
+    ib = (t - k + (P - 1)) % (P - 1);
+  }
+}
+
+// shared memory: Bs [SB][SPITCH] | nB [SB] | flags
+// Pairs inside one block (once per sweep): CTA = block, 8 warps busy per round of the 16-player tournament.
+__global__ void __launch_bounds__(SNTH) qtt_sbj_intra_kernel(const __grid_constant__ SbjGroup g) {
+  const JacProb& P = g.p[blockIdx.x / g.P];
+  const int blk = blockIdx.x % g.P;
+  if (P.work[1] != 0.0) return;
+  const int p = sbj_rows(P), q = P.q;
+  if (blk * SB >= p) return;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  extern __shared__ __align__(16) double sm[];
+  double* Bs = sm;
+  double* nB = sm + SB * SPITCH;
+  {
+    const int row = blk * SB + warp;
+    double sq = 0.0;
+#pragma unroll
+    for (int e = 0; e < SEPL; ++e) {
+      const int x = lane + 32 * e;
+      const double v = (row < p && x < q) ? P.X[(i64)row * P.ld + x] : 0.0;
+      Bs[warp * SPITCH + x] = v;
+      sq += v * v;
+    }
+    sq = warp_sum1(sq);
+    if (lane == 0) nB[warp] = sq;
+  }
+  __syncthreads();
+  const double floor2 = 4.930380657631324e-32 * P.work[0] / (double)p;
+  const double tol = 2.220446049250313e-16 * sqrt((double)q);
+  const double tol2 = tol * tol;
+  int mybig = 0;
+  for (int round = 0; round < SB - 1; ++round) {
+    if (warp < SB / 2) {
+      int ia, ib;
+      rr_pair(SB, round, warp, ia, ib);
+      double* ra = Bs + ia * SPITCH + lane;
+      double* rb = Bs + ib * SPITCH + lane;
+      double ab = 0.0, ab2 = 0.0;
+#pragma unroll
+      for (int e = 0; e < SEPL; ++e) {
+        if (e & 1) ab2 += ra[32 * e] * rb[32 * e];
+        else ab += ra[32 * e] * rb[32 * e];
+      }
+      ab = warp_sum1(ab + ab2);
+      const double aa = nB[ia], bb = nB[ib];
+      const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
+      if (R.apply) {
+#pragma unroll
+        for (int e = 0; e < SEPL; ++e) {
+          const double a = ra[32 * e], v = rb[32 * e];
+          ra[32 * e] = R.c * a - R.s * v;
+          rb[32 * e] = R.s * a + R.c * v;
+        }
+        if (lane == 0) {
+          nB[ia] = fmax(aa - R.t * ab, 0.0);
+          nB[ib] = fmax(bb + R.t * ab, 0.0);
+          if (R.big) ++mybig;
+        }
+      }
+    }
+    __syncthreads();
+  }
+  {
+    const int row = blk * SB + warp;
+    if (row < p) {
+#pragma unroll
+      for (int e = 0; e < SEPL; ++e) {
+        const int x = lane + 32 * e;
+        if (x < q) P.X[(i64)row * P.ld + x] = Bs[warp * SPITCH + x];
+      }
+    }
+  }
+  if (lane == 0 && mybig) atomicAdd(&P.work[2], (double)mybig);
+}
+
+// One round of the block tournament: CTA = block pair, top rows in registers, bot block in shared memory.
+__global__ void __launch_bounds__(SNTH) qtt_sbj_round_kernel(const __grid_constant__ SbjGroup g) {
+  const int half = g.P / 2;
+  const JacProb& P = g.p[blockIdx.x / half];
+  const int k = blockIdx.x % half;
+  if (P.work[1] != 0.0) return;
+  const int p = sbj_rows(P), q = P.q;
+  int Pi = (p + SB - 1) / SB;
+  Pi += Pi & 1;  // blocks of this problem (even)
+  if (Pi < 2 || g.round >= Pi - 1 || k >= Pi / 2) return;
+  int ia, ib;
+  rr_pair(Pi, g.round, k, ia, ib);
+  if (ia * SB >= p || ib * SB >= p) return;  // an empty padding block
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  extern __shared__ __align__(16) double sm[];
+  double* Bs = sm;
+  double* nB = sm + SB * SPITCH;
+  const int rowa = ia * SB + warp, rowb = ib * SB + warp;
+  double a[SEPL];
+  double aa = 0.0;
+  {
+    double sq = 0.0;
+#pragma unroll
+    for (int e = 0; e < SEPL; ++e) {
+      const int x = lane + 32 * e;
+      a[e] = (rowa < p && x < q) ? P.X[(i64)rowa * P.ld + x] : 0.0;
+      const double v = (rowb < p && x < q) ? P.X[(i64)rowb * P.ld + x] : 0.0;
+      Bs[warp * SPITCH + x] = v;
+      aa += a[e] * a[e];
+      sq += v * v;
+    }
+    aa = warp_sum1(aa);
+    sq = warp_sum1(sq);
+    if (lane == 0) nB[warp] = sq;
+  }
+  __syncthreads();
+  const double floor2 = 4.930380657631324e-32 * P.work[0] / (double)p;
+  const double tol = 2.220446049250313e-16 * sqrt((double)q);
+  const double tol2 = tol * tol;
+  int mybig = 0;
+  int j = warp;
+  for (int r = 0; r < SB; ++r) {
+    double* rb = Bs + j * SPITCH + lane;
+    const double bb = nB[j];
+    double ab = 0.0, ab2 = 0.0;
+#pragma unroll
+    for (int e = 0; e < SEPL; ++e) {
+      if (e & 1) ab2 += a[e] * rb[32 * e];
+      else ab += a[e] * rb[32 * e];
+    }
+    ab = warp_sum1(ab + ab2);
+    const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
+    if (R.apply) {
+#pragma unroll
+      for (int e = 0; e < SEPL; ++e) {
+        const double v = rb[32 * e];
+        const double an = R.c * a[e] - R.s * v;
+        rb[32 * e] = R.s * a[e] + R.c * v;
+        a[e] = an;
+      }
+      aa = fmax(aa - R.t * ab, 0.0);
+      if (lane == 0) {
+        nB[j] = fmax(bb + R.t * ab, 0.0);
+        if (R.big) ++mybig;
+      }
+    }
+    j = (j + 1 == SB) ? 0 : j + 1;
+    __syncthreads();
+  }
+#pragma unroll
+  for (int e = 0; e < SEPL; ++e) {
+    const int x = lane + 32 * e;
+    if (x < q) {
+      if (rowa < p) P.X[(i64)rowa * P.ld + x] = a[e];
+      if (rowb < p) P.X[(i64)rowb * P.ld + x] = Bs[warp * SPITCH + x];
+    }
+  }
+  if (lane == 0 && mybig) atomicAdd(&P.work[2], (double)mybig);
+}
+
+}  // namespace
+
+bool qtt_sbj_fits(int p, int q) { return p >= 2 && q >= 1 && q <= SPITCH; }
+
+cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
+  static bool attr_done = false;
+  const size_t smem = ((size_t)SB * SPITCH + SB + 2) * sizeof(double);
+  if (!attr_done) {
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_intra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_done = true;
+  }
+  for (int b0 = 0; b0 < n; b0 += QTT_JAC_MAX_BATCH) {
+    SbjGroup g;
+    g.nprob = 0;
+    int pmax = 0, qmax = 0;
+    double flops = 0.0;
+    for (int i = b0; i < n && g.nprob < QTT_JAC_MAX_BATCH; ++i) {
+      const JacProb& pr = probs[i];
+      if (pr.p < 2 || pr.q < 1) continue;
+      if (!pr.work || pr.q > SPITCH) return cudaErrorInvalidValue;
+      g.p[g.nprob++] = pr;
+      pmax = pr.p > pmax ? pr.p : pmax;
+      qmax = pr.q > qmax ? pr.q : qmax;
+      const double a = pr.p > pr.q ? pr.p : pr.q, bb = pr.p > pr.q ? pr.q : pr.p;
+      flops += 6.0 * a * bb * bb + 20.0 * bb * bb * bb;
+    }
+    if (g.nprob == 0) continue;
+    int P = (pmax + SB - 1) / SB;
+    P += P & 1;
+    g.P = P;
+    g.max_sweeps = 30;
+    g.round = 0;
+    g.sweep = 0;
+    // the whole iteration is booked as ONE profiler record of the family (first launch .. last launch)
+    QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, g.nprob, 0);
+    qtt_sbj_init_kernel<<<g.nprob, SNTH, 0, stream>>>(g);
+    for (int sweep = 0; sweep < g.max_sweeps; ++sweep) {
+      g.sweep = sweep;
+      qtt_sbj_intra_kernel<<<P * g.nprob, SNTH, smem, stream>>>(g);
+      for (int t = 0; t < P - 1; ++t) {
+        g.round = t;
+        qtt_sbj_round_kernel<<<(P / 2) * g.nprob, SNTH, smem, stream>>>(g);
+      }
+      qtt_sbj_check_kernel<<<g.nprob, 32, 0, stream>>>(g);
+    }
+    QTT_CHECK_CUDA(cudaGetLastError());
+    g_qtt_launch_count += (long long)g.max_sweeps * (P + 1);  // + the init launch counted by QttProf
+  }
+  return cudaSuccess;
+}

@@ -234,6 +234,7 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
     }
     JacProb a;
     a.X = j.X; a.p = prow; a.q = j.q; a.ld = j.q; a.p_dev = rank_dev; a.status = ctx->jac_status;
+    a.work = ctx->arena.tmp(8);
     jp.push_back(a);
     SelProb s;
     s.X = j.X; s.p = prow; s.q = j.q; s.ld = j.q;

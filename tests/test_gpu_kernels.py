@@ -251,3 +251,34 @@ def test_pivoted_qr_preconditioner_then_jacobi(env, p, q, batch, rk):
         big = d > 1e-9 * d.max()
         off = (G - np.diag(np.diag(G))) / np.outer(d, d)
         assert np.max(np.abs(off[np.ix_(big, big)])) < 1e-13 * np.sqrt(q) * 4
+
+
+@pytest.mark.parametrize("p,q,batch", [(40, 600, 2), (300, 700, 2), (100, 1000, 1), (1024, 1024, 2)])
+def test_streamed_block_jacobi(env, p, q, batch):
+    """qtt_diag_rowjacobi_streamed (rows too long for the cluster-resident kernel): singular values against LAPACK,
+    mutually orthogonal rows, unchanged Frobenius norm."""
+    lib, torch, stream = env
+    rng = np.random.default_rng(p + q)
+    mn = min(p, q)
+    # graded rows, as the triangular factors of the zip-up are
+    X = rng.standard_normal((batch, p, q)) * np.logspace(0, -8, p)[None, :, None]
+    dX = dev(torch, X)
+    status = torch.zeros(2, dtype=torch.int32, device="cuda")
+    work = torch.zeros(8 * batch, dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    assert lib.qtt_diag_rowjacobi_streamed(C.c_void_p(stream.cuda_stream), ptr(dX), batch, p, q, q, ptr(status),
+                                           ptr(work)) == 0
+    stream.synchronize()
+    Z = dX.cpu().numpy()
+    stt = status.cpu().numpy()
+    assert stt[1] == 0 and 1 <= stt[0] <= 30, stt
+    for b in range(batch):
+        s = np.sort(np.linalg.norm(Z[b], axis=1))[::-1]
+        want = np.linalg.svd(X[b], compute_uv=False)
+        assert np.max(np.abs(s[:mn] - want)) <= 1e-12 * want[0]
+        G = Z[b] @ Z[b].T
+        d = np.sqrt(np.maximum(np.diag(G), 1e-300))
+        big = d > 1e-9 * d.max()
+        off = (G - np.diag(np.diag(G))) / np.outer(d, d)
+        assert np.max(np.abs(off[np.ix_(big, big)])) < 1e-13 * np.sqrt(q) * 4
+        assert abs(np.linalg.norm(Z[b]) - np.linalg.norm(X[b])) <= 1e-13 * np.linalg.norm(X[b])
