@@ -10,6 +10,7 @@
 // Trailing update: a separate grid, one warp per pair of rows, Y2 <- Y2 - (Y2 V^T) (T V), compact WY.
 #include <cooperative_groups.h>
 #include <cstring>
+#include <vector>
 
 #include "common.cuh"
 namespace cg = cooperative_groups;
@@ -262,6 +263,18 @@ __global__ void __launch_bounds__(UPD_NT) qtt_lq_update_kernel(const __grid_cons
   }
 }
 
+// W[0..n) <- sum_z W[z * n + ..): the K-chunks of the skinny first product of the trailing update, fixed order
+struct SumProb { double* W; int n, Z; };
+struct SumGroup { int nprob; SumProb p[QTT_LQ_MAX_BATCH]; };
+__global__ void qtt_sum_partials_kernel(const __grid_constant__ SumGroup g) {
+  const SumProb& P = g.p[blockIdx.y];
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= P.n || P.Z <= 1) return;
+  double s = P.W[idx];
+  for (int z = 1; z < P.Z; ++z) s += P.W[(i64)z * P.n + idx];
+  P.W[idx] = s;
+}
+
 __global__ void qtt_extract_tri_kernel(const __grid_constant__ TriGroup g) {
   const TriProb& P = g.p[blockIdx.y];
   const i64 n = (i64)P.k * P.k;
@@ -356,21 +369,44 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
         QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
       }
       if (ctas > 0) {
-        // trailing update of the rows below the panel, Y2 <- Y2 - (Y2 V^T)(T V), as two grouped DMMA GEMMs
-        GemmProb g1[QTT_LQ_MAX_BATCH], g2[QTT_LQ_MAX_BATCH];
+        // trailing update of the rows below the panel, Y2 <- Y2 - (Y2 V^T)(T V), as grouped DMMA GEMMs.  The first
+        // product is skinny (16 columns) with a long contraction (the row length): it is cut into up to 8 K-chunks
+        // (one GEMM problem each, so that enough CTAs work on it), whose partial results a small kernel adds up in
+        // a fixed order.
+        std::vector<GemmProb> g1;
+        GemmProb g2[QTT_LQ_MAX_BATCH];
+        SumGroup sg;
+        sg.nprob = 0;
         for (int i = 0; i < ug.nprob; ++i) {
           const LqProb& p = ug.p[i];
           const int nbp = (p.k - p0 < NB) ? p.k - p0 : NB;
           const int r0 = p0 + nbp, rem = p.k - r0, mw = p.m - p0;
-          GemmProb a;
-          memset(&a, 0, sizeof(a));
-          a.nbatch = 1;
-          a.alpha = 1.0; a.beta = 0.0;
-          a.A = p.Y + (i64)r0 * p.ld + p0; a.a_lo = p.ld; a.a_k = 1;
-          a.B = p.V + p0; a.b_k = 1; a.b_n = p.m;
-          a.C = p.W; a.c_lo = NB; a.c_n = 1;
-          a.M = rem; a.N = nbp; a.K = mw;
-          g1[i] = a;
+          int Z = mw / 512;
+          Z = Z > 8 ? 8 : Z;
+          if (Z > p.m / rem) Z = p.m / rem;  // the partials live in the NB x m scratch W
+          Z = Z < 1 ? 1 : Z;
+          int chunk = (mw + Z - 1) / Z;
+          chunk = (chunk + 15) & ~15;
+          for (int z = 0; z < Z; ++z) {
+            const int k0 = z * chunk, kz = (mw - k0 < chunk) ? mw - k0 : chunk;
+            GemmProb a;
+            memset(&a, 0, sizeof(a));
+            a.nbatch = 1;
+            a.alpha = 1.0; a.beta = 0.0;
+            a.A = p.Y + (i64)r0 * p.ld + p0 + k0; a.a_lo = p.ld; a.a_k = 1;
+            a.B = p.V + p0 + k0; a.b_k = 1; a.b_n = p.m;
+            a.C = p.W + (i64)z * rem * NB; a.c_lo = NB; a.c_n = 1;
+            a.M = rem; a.N = nbp; a.K = kz > 0 ? kz : 0;
+            if (a.K > 0) g1.push_back(a);
+            else {  // (cannot happen with chunk >= 16, kept for safety: an empty chunk contributes zeros)
+              Z = z;
+              break;
+            }
+          }
+          sg.p[sg.nprob].W = p.W;
+          sg.p[sg.nprob].n = rem * NB;
+          sg.p[sg.nprob].Z = Z;
+          ++sg.nprob;
           GemmProb b;
           memset(&b, 0, sizeof(b));
           b.nbatch = 1;
@@ -381,7 +417,20 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
           b.M = rem; b.N = mw; b.K = nbp;
           g2[i] = b;
         }
-        QTT_CHECK_CUDA(qtt_launch_gemm(g1, ug.nprob, stream, QK_LQ_UPDATE));
+        QTT_CHECK_CUDA(qtt_launch_gemm(g1.data(), (int)g1.size(), stream, QK_LQ_UPDATE));
+        {
+          bool any = false;
+          int nmax = 0;
+          for (int i = 0; i < sg.nprob; ++i) {
+            any = any || sg.p[i].Z > 1;
+            nmax = sg.p[i].n > nmax ? sg.p[i].n : nmax;
+          }
+          if (any) {
+            QttProf prof(QK_LQ_UPDATE, stream, 0.0, 0, 0, sg.nprob, -1);
+            qtt_sum_partials_kernel<<<dim3((nmax + 255) / 256, sg.nprob), 256, 0, stream>>>(sg);
+            QTT_CHECK_CUDA(cudaGetLastError());
+          }
+        }
         QTT_CHECK_CUDA(qtt_launch_gemm(g2, ug.nprob, stream, QK_LQ_UPDATE));
         (void)fu;
       }
