@@ -597,16 +597,15 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_reg_kernel(const __grid_constant
       } else if (rank == j % C) {
         stage_col = j;
       }
-      // ---- the owning warp stages its column (rows >= j) slab by slab in the peers
-      if (stage_col >= 0 && ((live0 && stage_col == col0g) || (live1 && stage_col == col1g))) {
-        const bool is0 = live0 && stage_col == col0g;
-#pragma unroll
-        for (int e = JB; e < EPL; ++e) {
-          if (32 * e < p) {
-            double* dst = stage_of(e % C);
-            dst[(size_t)(par * MAXC + rank) * chm + (e / C) * 32 + lane] = is0 ? x0[e] : x1[e];
-          }
-        }
+      // ---- stage the column (rows >= j) slab by slab in the peers: warp e pushes slab e from the shared-memory
+      //      copy (kept current by the write-through of the update below); one warp pushing all slabs would
+      //      serialise ~250 cycles per remote store
+      if (!pivot) __syncthreads();  // (with pivoting the barrier above orders the write-through)
+      if (stage_col >= 0 && warp >= JB && 32 * warp < p && warp < EPL) {
+        const double* col = Xs + (size_t)(stage_col / C) * pp;
+        double* dst = stage_of(warp % C);
+        const int i = 32 * warp + lane;
+        dst[(size_t)(par * MAXC + rank) * chm + (warp / C) * 32 + lane] = (i < p) ? col[i] : 0.0;
       }
       barrier();
       if (pivot && C > 1) {
@@ -700,6 +699,15 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_reg_kernel(const __grid_constant
         if (lane == jj) {
           if (upd0) x0[JB] = nj0;
           if (upd1) x1[JB] = nj1;
+        }
+        // write-through: the shared-memory copy of my columns is what gets staged when one of them is the pivot
+#pragma unroll
+        for (int e = JB; e < EPL; ++e) {
+          const int i = lane + 32 * e;
+          if (i < p) {
+            if (upd0) Xs[(size_t)warp * pp + i] = x0[e];
+            if (upd1) Xs[(size_t)(warp + QNW) * pp + i] = x1[e];
+          }
         }
         if (pivot) {
           if (upd0) n0 -= nj0 * nj0;
