@@ -264,6 +264,17 @@ qtt_status qtt_ctx_create(qtt_ctx** out, int device, void* cuda_stream, qtt_allo
   ctx->arena.size = workspace_bytes & ~(size_t)255;
   try {
     // persistent constants at the bottom of the workspace
+    if (ctx->arena.size >= ((size_t)256 << 20)) {
+      const size_t side = (ctx->arena.size / 4) & ~(size_t)255;
+      ctx->side_arena.base = ctx->arena.base + (ctx->arena.size - side);
+      ctx->side_arena.size = side;
+      ctx->side_arena.lo = 0;
+      ctx->side_arena.hi = side;
+      ctx->arena.size -= side;
+      QTT_CU(cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking));
+      QTT_CU(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+      QTT_CU(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
+    }
     ctx->arena.lo = 0;
     ctx->arena.hi = ctx->arena.size;
     ctx->ones = ctx->arena.keep(32);
@@ -272,6 +283,9 @@ qtt_status qtt_ctx_create(qtt_ctx** out, int device, void* cuda_stream, qtt_allo
     QTT_CU(cudaMemsetAsync(ctx->jac_status, 0, 32 * sizeof(double), ctx->stream));
     qtt_kernels_init();
   } catch (const QttError& e) {
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     release(ctx->arena.base, user);
     delete ctx;
     return e.status;
@@ -284,6 +298,12 @@ void qtt_ctx_destroy(qtt_ctx* ctx) {
   if (!ctx) return;
   cudaStreamSynchronize(ctx->stream);
   for (Rk4Plan* p : ctx->plans) plan_free(ctx, p);
+  if (ctx->side) {
+    cudaStreamSynchronize(ctx->side);
+    cudaStreamDestroy(ctx->side);
+  }
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->arena.base) ctx->release(ctx->arena.base, ctx->user);
   delete ctx;
 }

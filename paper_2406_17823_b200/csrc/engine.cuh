@@ -82,6 +82,11 @@ struct qtt_ctx {
   qtt_release_fn release = nullptr;
   void* user = nullptr;
   Arena arena;
+  // a second stream with its own scratch region (the top quarter of the workspace): qtt_rk4_step runs the two
+  // Laplacian roundings of a right-hand side there, concurrently with the four products that do not need them
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  Arena side_arena;
   std::string err;
   int chi_work = 0;
   size_t mat_limit = (size_t)2 << 30;

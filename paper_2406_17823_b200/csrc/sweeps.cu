@@ -792,6 +792,18 @@ std::vector<OutMps> alloc_outs_keep(qtt_ctx* ctx, const std::vector<std::vector<
   }
   return out;
 }
+// Enqueue on the side stream with the side scratch region: swaps them into the context for the scope.
+struct SideScope {
+  qtt_ctx* ctx;
+  explicit SideScope(qtt_ctx* c) : ctx(c) {
+    std::swap(ctx->stream, ctx->side);
+    std::swap(ctx->arena, ctx->side_arena);
+  }
+  ~SideScope() {
+    std::swap(ctx->stream, ctx->side);
+    std::swap(ctx->arena, ctx->side_arena);
+  }
+};
 View view_of(const OutMps& o) {
   View v;
   v.n = o.n;
@@ -803,9 +815,56 @@ View view_of(const OutMps& o) {
 // f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i   (oracle O8)
 void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap, double Re, int chi, double eps,
          int chi_work, View f[2]) {
-  // level 1: six applies + roundings in one batch: (D1 u_i, D2 u_i, Lap u_i) for i = 0, 1
+  // level 1: six applies + roundings: (D1 u_i, D2 u_i, Lap u_i) for i = 0, 1.  The two Laplacians are only needed by
+  // level 3, so -- when the context has a side stream whose scratch region is large enough -- they are rounded
+  // there, concurrently with the four D_j u_i on the main stream and with the products of level 2.
   std::vector<View> g(6);
+  bool forked = false;
   {
+    size_t need = (size_t)64 << 20;
+    for (int i = 0; i < 2; ++i)
+      for (int k = 0; k < u[i].n; ++k)
+        need += (size_t)6 * 8 * 4 * (size_t)Lap->D[k] * u[i].r[k] * (size_t)Lap->D[k + 1] * u[i].r[k + 1];
+    forked = ctx->side != nullptr && ctx->side_arena.size >= need;
+  }
+  if (forked) {
+    std::vector<std::vector<int>> capsL;
+    for (int i = 0; i < 2; ++i) {
+      std::vector<int> re(u[i].n + 1);
+      for (int k = 0; k <= u[i].n; ++k) re[k] = Lap->D[k] * u[i].r[k];
+      capsL.push_back(qtt_round_caps(re, chi));
+    }
+    std::vector<OutMps> lout = alloc_outs_keep(ctx, capsL);  // results live in the main keep stack
+    QTT_CU(cudaEventRecord(ctx->ev_fork, ctx->stream));
+    QTT_CU(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    {
+      SideScope sc(ctx);  // ctx->stream / ctx->arena are the side stream and its scratch region in this scope
+      const size_t mark = ctx->arena.hi;
+      std::vector<const MpoData*> W{Lap, Lap};
+      std::vector<View> X{u[0], u[1]};
+      std::vector<View> ex;
+      qtt_expand_apply_batch(ctx, W, X, ex);
+      qtt_round_dense_batch(ctx, ex, chi, eps, lout);
+      ctx->arena.hi = mark;
+      QTT_CU(cudaEventRecord(ctx->ev_join, ctx->stream));
+    }
+    g[2] = view_of(lout[0]);
+    g[5] = view_of(lout[1]);
+    const size_t mark = ctx->arena.hi;
+    std::vector<const MpoData*> W{Dj[0], Dj[1], Dj[0], Dj[1]};
+    std::vector<View> X{u[0], u[0], u[1], u[1]};
+    std::vector<View> ex;
+    qtt_expand_apply_batch(ctx, W, X, ex);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : ex) caps.push_back(qtt_round_caps(e.r, chi));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, ex, chi, eps, out);
+    g[0] = view_of(out[0]);
+    g[1] = view_of(out[1]);
+    g[3] = view_of(out[2]);
+    g[4] = view_of(out[3]);
+    ctx->arena.hi = mark;
+  } else {
     const size_t mark = ctx->arena.hi;
     std::vector<const MpoData*> W{Dj[0], Dj[1], Lap, Dj[0], Dj[1], Lap};
     std::vector<View> X{u[0], u[0], u[0], u[1], u[1], u[1]};
@@ -836,6 +895,7 @@ void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap
     ctx->arena.hi = mark;
   }
   // level 3: f_i = -c_i1 - c_i2 + lap_i / Re, one rounding each
+  if (forked) QTT_CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
   {
     const size_t mark = ctx->arena.hi;
     std::vector<std::vector<std::pair<double, View>>> terms(2);
