@@ -384,3 +384,25 @@ def test_config5_primitive_sweep_matches_oracle(Q, big_ctx, chi):
         assert Q.qtt_mps_bonds(hs[i]) == O.bonds(want)
         assert rel(gpu_dense(Q, big_ctx, hs[i]), O.to_dense(want)) < TOL
     assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
+
+
+def test_rk4_step_eps_rule_matches_oracle(Q, ctx):
+    """qtt_rk4_step with eps > 0 (data-dependent ranks, one stream synchronisation per bond; the Laplacian branch on
+    the side stream): same bonds and fields as the oracle, whose ranks come from the same rule."""
+    n, chi, Re, dt, eps = 6, 24, 100.0, 1e-3, 1e-6
+    g, o = ops(Q, ctx, n)
+    X, Y = I.grid(n)
+    ux = np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y) + 0.3 * smooth_field(n, 7)
+    uy = -np.cos(2 * np.pi * X) * np.sin(2 * np.pi * Y) + 0.3 * smooth_field(n, 8)
+    U = [O.from_dense(ux, chi, eps), O.from_dense(uy, chi, eps)]
+    u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+    U1 = O.rk4_step(U, o[0], o[1], o[2], Re, dt, chi, eps)
+    Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], Re, dt, chi, eps)
+    for i in range(2):
+        # a singular value within rounding distance of the threshold may fall on either side: the fields must agree
+        # to the accuracy the threshold itself guarantees, and the ranks within one
+        bg, bo = Q.qtt_mps_bonds(u[i]), O.bonds(U1[i])
+        assert all(abs(a - b) <= 1 for a, b in zip(bg, bo)), (bg, bo)
+        tol = TOL if bg == bo else 10 * eps
+        assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < tol
+    assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
