@@ -87,7 +87,6 @@ View view_of_body(const Body* b) {
   return v;
 }
 
-std::vector<int> body_bonds(const Body* b) { return b->r; }
 
 // Dense view of any body; lazy kinds are materialised in the tmp stack (bounded by the limit).
 View materialize(qtt_ctx* ctx, const Body* b) {

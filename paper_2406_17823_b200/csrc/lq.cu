@@ -200,68 +200,12 @@ __global__ void __launch_bounds__(PANEL_NT) qtt_lq_panel_kernel(const __grid_con
   }
 }
 
-// Trailing update for the rows below the panel: y <- y - (y V^T) (T V), columns p0..m-1.
-constexpr int UPD_NT = 256;
-constexpr int UPD_ROWS_PER_WARP = 2;
-constexpr int UPD_RB = (UPD_NT / 32) * UPD_ROWS_PER_WARP;
+// Problems that still have rows below the current panel (their trailing update is done by grouped GEMMs).
 
 struct UpdGroup {
   int nprob, p0;
-  int cta0[QTT_LQ_MAX_BATCH + 1];
   LqProb p[QTT_LQ_MAX_BATCH];
 };
-
-__global__ void __launch_bounds__(UPD_NT) qtt_lq_update_kernel(const __grid_constant__ UpdGroup g) {
-  int pi = 0;
-  for (int i = 1; i < g.nprob; ++i)
-    if ((int)blockIdx.x >= g.cta0[i]) pi = i;
-  const LqProb& P = g.p[pi];
-  const int p0 = g.p0;
-  const int nbp = min(NB, P.k - p0);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int r0 = p0 + nbp + ((int)blockIdx.x - g.cta0[pi]) * UPD_RB + warp * UPD_ROWS_PER_WARP;
-  const int m = P.m;
-  double acc[UPD_ROWS_PER_WARP][NB];
-  double* y[UPD_ROWS_PER_WARP];
-  bool ok[UPD_ROWS_PER_WARP];
-#pragma unroll
-  for (int r = 0; r < UPD_ROWS_PER_WARP; ++r) {
-    ok[r] = (r0 + r) < P.k;
-    y[r] = P.Y + (i64)(ok[r] ? r0 + r : p0) * P.ld;
-#pragma unroll
-    for (int j = 0; j < NB; ++j) acc[r][j] = 0.0;
-  }
-  if (!ok[0]) return;
-  for (int c = p0 + lane; c < m; c += 32) {
-    double yv[UPD_ROWS_PER_WARP];
-#pragma unroll
-    for (int r = 0; r < UPD_ROWS_PER_WARP; ++r) yv[r] = ok[r] ? y[r][c] : 0.0;
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      double v = (j < nbp) ? P.V[(i64)j * m + c] : 0.0;
-#pragma unroll
-      for (int r = 0; r < UPD_ROWS_PER_WARP; ++r) acc[r][j] += yv[r] * v;
-    }
-  }
-#pragma unroll
-  for (int r = 0; r < UPD_ROWS_PER_WARP; ++r)
-#pragma unroll
-    for (int j = 0; j < NB; ++j) acc[r][j] = warp_sum(acc[r][j]);
-  for (int c = p0 + lane; c < m; c += 32) {
-    double d[UPD_ROWS_PER_WARP];
-#pragma unroll
-    for (int r = 0; r < UPD_ROWS_PER_WARP; ++r) d[r] = 0.0;
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      double t = (j < nbp) ? P.TV[(i64)j * m + c] : 0.0;
-#pragma unroll
-      for (int r = 0; r < UPD_ROWS_PER_WARP; ++r) d[r] += acc[r][j] * t;
-    }
-#pragma unroll
-    for (int r = 0; r < UPD_ROWS_PER_WARP; ++r)
-      if (ok[r]) y[r][c] -= d[r];
-  }
-}
 
 // W[0..n) <- sum_z W[z * n + ..): the K-chunks of the skinny first product of the trailing update, fixed order
 struct SumProb { double* W; int n, Z; };
@@ -333,9 +277,8 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
         mwmax = (p.m - p0) > mwmax ? (p.m - p0) : mwmax;
         int rem = p.k - (p0 + (p.k - p0 < NB ? p.k - p0 : NB));
         if (rem > 0) {
-          ug.cta0[ug.nprob] = ctas;
           ug.p[ug.nprob++] = p;
-          ctas += (rem + UPD_RB - 1) / UPD_RB;
+          ctas += 1;
         }
       }
       if (grp.nprob == 0) break;
