@@ -278,7 +278,7 @@ def run_ours(args):
 
 # dram bytes (read + write) per launch from the committed ncu --set full captures (profiles/), keyed by
 # (family, launch shape tag of qtt_diag_profile_dump)
-NCU_TRAFFIC_BYTES = {("rowjacobi", (512, 512, 4, 16)): 18.03e6}
+NCU_TRAFFIC_BYTES = {("rowjacobi", (512, 512, 4, 16)): 8.43e6}
 KERNEL_NAMES = {"rowjacobi": "qtt_blockjacobi_kernel", "qrcp": "qtt_qrcp_reg_kernel", "gemm": "qtt_gemm_dmma_kernel",
                 "lq_panel": "qtt_lq_panel_kernel / qtt_qrcp_kernel", "lq_update": "qtt_gemm_dmma_kernel",
                 "select": "qtt_select_kernel", "move": "movement kernels"}
