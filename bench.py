@@ -425,9 +425,22 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workspace-gib", type=float, default=8.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
+                    help="only run the row-a2 site-contraction GEMM passes at the bulk-site shapes of bond CHI and "
+                         "print their TFLOP/s (the command the ncu capture in profiles/ is taken on)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe_contraction:
+        import torch
+        import paper_2406_17823_b200 as Q
+        if not torch.cuda.is_available():
+            raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+        ctx = Q.Context(device=0, workspace_bytes=1 << 28)
+        peaks = fp64_peaks(Q, ctx)
+        print(json.dumps({"contraction": contraction_probe(ctx, args.probe_contraction, peaks["dmma"]),
+                          "fp64_peaks_tflops": peaks}), flush=True)
+        return 0
     return run_ours(args)
 
 
