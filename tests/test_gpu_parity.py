@@ -406,3 +406,26 @@ def test_rk4_step_eps_rule_matches_oracle(Q, ctx):
         tol = TOL if bg == bo else 10 * eps
         assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < tol
     assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+
+
+def test_rk4_step_is_bitwise_reproducible(Q, ctx):
+    """No atomics or timing-dependent orders on the data path: the same step from the same cores gives bit-identical
+    cores, run to run and graph replay against eager launches (a data race in a kernel would show up here)."""
+    cfg = I.CONFIGS[2]
+    n, chi = cfg["n"], cfg["chi"]
+    ux, uy = I.config_fields(2)
+    ux = ux + 0.05 * smooth_field(n, 11)  # a rank that really fills chi
+    g, _ = ops(Q, ctx, n)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    results = []
+    for graphs in (True, True, False):
+        Q.qtt_ctx_set_graphs(ctx, graphs)
+        u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+        for _ in range(2):
+            Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+        results.append([Q.qtt_mps_get_cores(ctx, x) for x in u])
+    Q.qtt_ctx_set_graphs(ctx, True)
+    for other in results[1:]:
+        for a, b in zip(results[0], other):
+            for ca, cb in zip(a, b):
+                assert ca.shape == cb.shape and np.array_equal(ca, cb)
