@@ -138,6 +138,13 @@ qtt_status qtt_mps_norm(qtt_ctx* ctx, const qtt_mps* x, double* out_host);
 /* Schmidt values of every bond 1..n-1 (Eq. 16-17): sigma_host[bond*cap + i], counts[bond];
  * entries beyond counts[bond] are untouched.  Synchronous. */
 qtt_status qtt_mps_schmidt(qtt_ctx* ctx, const qtt_mps* x, double* sigma_host, int cap, int* counts /* n+1 */);
+/* PAPER.md:160 Eq. 12: fidelity F = <a|b>^2 / (||a||^2 ||b||^2) by MPS overlaps (qtt_mps_dot, qtt_mps_norm).
+ * Synchronous; 0 if either operand is zero. */
+qtt_status qtt_mps_fidelity(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, double* out_host);
+/* PAPER.md:238-244 Eq. 16-17: chi_l(eps), the number of Schmidt values bipartition l = 1..n-1 needs for a relative
+ * truncation error sqrt(sum_{i > chi_l} sigma_i^2) / ||x|| <= eps, written to chi_host[l] (n+1 ints, ends = 1), and
+ * chi = max_l chi_l to *chi_max_host (may be NULL).  Synchronous. */
+qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_host, int* chi_max_host);
 qtt_status qtt_mps_clone(qtt_ctx* ctx, const qtt_mps* x, qtt_mps** out);
 void qtt_mps_free(qtt_mps* x);
 

@@ -33,6 +33,7 @@ where the paper is silent/garbled and the reading taken):
   O8  rhs                       PAPER.md:49-53 Eq. 2 without pressure (Burgers form)
   O9  rk4_step                  PAPER.md:124-128 Eq. 11
   O10 mpo_d1 / mpo_d2 / mpo_laplacian   PAPER.md:391-424 App. A, Eq. A1-A3, Table II
+  O11 fidelity, chi_eps         PAPER.md:160 Eq. 12; Eq. 16-17 (diagnostics)
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
 grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
@@ -40,7 +41,7 @@ analytic finite-difference of sin/cos, bond-2 closed forms, the root-sum-square
 truncation identity, norm preservation, dense TT-SVD, dense RK4 of the same
 stencils.
 
-Parity-pin status: O1-O6, O8-O10 pinned.  O7 is pinned where chi_work >= every
+Parity-pin status: O1-O6, O8-O11 pinned.  O7 is pinned where chi_work >= every
 intermediate rank (then it equals O6 applied to O4, checked against dense brute
 force) and by its error bound; for a finite chi_work that really truncates, the
 result is DEFINED by the step-by-step algorithm below (the paper gives none) --
@@ -438,3 +439,33 @@ def canonical_random(raw_cores):
     C = _sweep_lr(raw_cores)
     C[-1] = C[-1] / np.linalg.norm(C[-1])
     return C
+
+
+# ------------------------------------------------------- diagnostics
+def fidelity(A, B) -> float:
+    """F = <a|b>^2 / (||a||^2 ||b||^2)  (Eq. 12)."""
+    na, nb = norm(A), norm(B)
+    if na == 0.0 or nb == 0.0:
+        return 0.0
+    return dot(A, B) ** 2 / (na * na * nb * nb)
+
+
+def chi_eps(cores, eps: float):
+    """chi_l(eps) for every bipartition l = 1..n-1 and chi = max_l chi_l (Eq. 16-17): the
+    number of Schmidt values needed so that the relative truncation error of that bipartition,
+    sqrt(sum_{i > chi_l} sigma_i^2) / ||u||, is <= eps.  Returns ([1, chi_1, ..., chi_{n-1}, 1], chi)."""
+    sv = schmidt_values(cores)
+    n = len(cores)
+    out = [1] * (n + 1)
+    for k in range(1, n):
+        s = np.asarray(sv[k], dtype=np.float64)
+        tot = math.sqrt(float(np.sum(s[::-1] ** 2)))
+        chi = len(s)
+        for cand in range(len(s), 0, -1):
+            tail = math.sqrt(float(np.sum(s[cand:][::-1] ** 2)))
+            if tail <= eps * tot:
+                chi = cand
+            else:
+                break
+        out[k] = max(1, chi)
+    return out, max(out)

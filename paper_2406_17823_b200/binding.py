@@ -241,6 +241,21 @@ def qtt_mps_schmidt(ctx: Context, x: Mps) -> list:
     return [None] + [buf[k, : counts[k]].copy() for k in range(1, n)] + [None]
 
 
+def qtt_mps_fidelity(ctx: Context, a: Mps, b: Mps) -> float:
+    v = C.c_double()
+    ctx.check(ctx.lib.qtt_mps_fidelity(ctx.h, a.h, b.h, C.byref(v)))
+    return v.value
+
+
+def qtt_mps_chi_eps(ctx: Context, x: Mps, eps: float) -> tuple[list[int], int]:
+    """(chi_l for l = 0..n, max_l chi_l) of PAPER.md Eq. 16-17."""
+    n = len(qtt_mps_bonds(x)) - 1
+    out = (C.c_int * (n + 1))()
+    mx = C.c_int()
+    ctx.check(ctx.lib.qtt_mps_chi_eps(ctx.h, x.h, float(eps), out, C.byref(mx)))
+    return list(out), mx.value
+
+
 def qtt_mps_clone(ctx: Context, x: Mps) -> Mps:
     h = C.c_void_p()
     ctx.check(ctx.lib.qtt_mps_clone(ctx.h, x.h, C.byref(h)))

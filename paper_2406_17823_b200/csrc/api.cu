@@ -812,6 +812,51 @@ qtt_status qtt_mps_norm(qtt_ctx* ctx, const qtt_mps* x, double* out_host) {
   QTT_API_END(ctx)
 }
 
+// PAPER.md:160 Eq. 12 and PAPER.md:238-244 Eq. 16-17: compositions of the calls above
+qtt_status qtt_mps_fidelity(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, double* out_host) {
+  if (!ctx || !a || !b || !out_host) return QTT_INVALID_ARG;
+  double ab = 0.0, na = 0.0, nb = 0.0;
+  qtt_status st = qtt_mps_dot(ctx, a, b, &ab);
+  if (st == QTT_OK) st = qtt_mps_norm(ctx, a, &na);
+  if (st == QTT_OK) st = qtt_mps_norm(ctx, b, &nb);
+  if (st != QTT_OK) return st;
+  const double d = na * na * nb * nb;
+  *out_host = d > 0.0 ? ab * ab / d : 0.0;
+  return QTT_OK;
+}
+
+qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_host, int* chi_max_host) {
+  if (!ctx || !x || !chi_host || !(eps >= 0.0)) return QTT_INVALID_ARG;
+  const int n = qtt_mps_num_sites(x);
+  std::vector<int> r(n + 1), counts(n + 1, 0);
+  qtt_status st = qtt_mps_bonds(x, r.data());
+  if (st != QTT_OK) return st;
+  int cap = 1;
+  for (int k = 0; k <= n; ++k) cap = std::max(cap, r[k]);
+  cap *= 4;
+  std::vector<double> sig((size_t)(n + 1) * cap, 0.0);
+  st = qtt_mps_schmidt(ctx, x, sig.data(), cap, counts.data());
+  if (st != QTT_OK) return st;
+  int worst = 1;
+  for (int k = 0; k <= n; ++k) chi_host[k] = 1;
+  for (int k = 1; k < n; ++k) {
+    const double* s = sig.data() + (size_t)k * cap;
+    double tot = 0.0;
+    for (int i = counts[k] - 1; i >= 0; --i) tot += s[i] * s[i];
+    // smallest chi with sqrt(sum_{i >= chi} s_i^2) <= eps * ||x||   (||x||^2 = sum of all s_i^2 at any bond)
+    double tail = 0.0;
+    int chi = counts[k];
+    for (int cand = counts[k]; cand >= 1; --cand) {
+      if (std::sqrt(tail) <= eps * std::sqrt(tot)) chi = cand; else break;
+      tail += s[cand - 1] * s[cand - 1];
+    }
+    chi_host[k] = std::max(1, chi);
+    worst = std::max(worst, chi_host[k]);
+  }
+  if (chi_max_host) *chi_max_host = worst;
+  return QTT_OK;
+}
+
 // ------------------------------------------------------------------------------------------ diagnostics
 int qtt_diag_gemm(void* stream, const double* A, const double* B, double* C, int M, int N, int K, int transA,
                   int transB, long long lda, long long ldb, long long ldc, double alpha, double beta, int nbatch,

@@ -429,3 +429,18 @@ def test_rk4_step_is_bitwise_reproducible(Q, ctx):
         for a, b in zip(results[0], other):
             for ca, cb in zip(a, b):
                 assert ca.shape == cb.shape and np.array_equal(ca, cb)
+
+
+def test_diagnostics_match_oracle(Q, ctx):
+    """qtt_mps_fidelity (Eq. 12) and qtt_mps_chi_eps (Eq. 16-17) against the oracle."""
+    n, chi = 7, 24
+    F = smooth_field(n, 21) + 1e-2 * np.random.default_rng(1).standard_normal((1 << n, 1 << n))
+    G = smooth_field(n, 22)
+    A, B = O.from_dense(F, chi), O.from_dense(G, chi)
+    a, b = Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B)
+    assert abs(Q.qtt_mps_fidelity(ctx, a, b) - O.fidelity(A, B)) <= 1e-12
+    assert abs(Q.qtt_mps_fidelity(ctx, a, a) - 1.0) <= 1e-12
+    for eps in (1e-1, 1e-2, 1e-4):
+        got, gmax = Q.qtt_mps_chi_eps(ctx, a, eps)
+        want, wmax = O.chi_eps(A, eps)
+        assert got == want and gmax == wmax

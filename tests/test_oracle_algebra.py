@@ -279,3 +279,41 @@ def test_canonical_random_is_unit_norm_left_canonical():
     C = O.canonical_random(raw)
     assert abs(O.norm(C) - 1.0) < 1e-13
     assert O.bonds(C) == I.bond_profile(6, 8)
+
+
+# ---------------------------------------------------------------- diagnostics (Eq. 12, 16-17)
+def test_fidelity_closed_forms():
+    n = 6
+    X, Y = I.grid(n)
+    s = O.from_dense(np.sin(2 * np.pi * X))
+    c = O.from_dense(np.cos(2 * np.pi * X))
+    assert abs(O.fidelity(s, s) - 1.0) < 1e-13
+    assert O.fidelity(s, c) < 1e-26                      # orthogonal on the periodic grid
+    m = O.from_dense(np.sin(2 * np.pi * X) + np.cos(2 * np.pi * X))
+    assert abs(O.fidelity(s, m) - 0.5) < 1e-13           # cos^2 of 45 degrees
+    # against the dense definition on a random pair
+    rng = np.random.default_rng(3)
+    F, G = rng.standard_normal((64, 64)), rng.standard_normal((64, 64))
+    want = np.sum(F * G) ** 2 / (np.sum(F * F) * np.sum(G * G))
+    assert abs(O.fidelity(O.from_dense(F), O.from_dense(G)) - want) < 1e-13
+
+
+def test_chi_eps_against_dense_truncation():
+    n = 6
+    X, Y = I.grid(n)
+    # sin(2 pi (x + y)) has exactly two Schmidt values at every interior bipartition
+    chis, chi = O.chi_eps(O.from_dense(np.sin(2 * np.pi * (X + Y))), 1e-12)
+    assert chi == 2 and chis[2:n - 1] == [2] * (n - 3)
+    # definition check on a generic field: truncating bipartition l of the DENSE tensor to chi_l Schmidt values gives
+    # a relative error <= eps, and chi_l - 1 values do not
+    rng = np.random.default_rng(5)
+    F = np.tanh((Y - 0.5) / 0.1) + 0.05 * rng.standard_normal((64, 64))
+    eps = 0.02
+    chis, chi = O.chi_eps(O.from_dense(F), eps)
+    T = O.encode(F)
+    for l in range(1, n):
+        s = np.linalg.svd(T.reshape(4 ** l, -1), compute_uv=False)
+        err = lambda k: np.sqrt(np.sum(s[k:] ** 2)) / np.linalg.norm(s)
+        assert err(chis[l]) <= eps * (1 + 1e-12)
+        assert chis[l] == 1 or err(chis[l] - 1) > eps * (1 - 1e-12)
+    assert chi == max(chis)
