@@ -363,32 +363,47 @@ def mpo_to_dense(W) -> np.ndarray:
 
 
 # --------------------------------------------------------------------------- O8
-def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None):
+def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False):
     """f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i, i = 1,2 (PAPER.md:49-53
     Eq. 2 without the pressure term; convective form, reading 4), with one rounding
-    after every apply, product and sum (reading 7)."""
+    after every apply, product and sum (reading 7).
+
+    skew=True: the paper's skew-symmetric convection (PAPER.md:432-435 Eq. B2),
+    1/2 sum_j (u_j (.) D_j u_i + D_j (u_j (.) u_i)): in addition p_ij = round(u_j (.) u_i)
+    (p_12 = p_21 computed once, as u_1 (.) u_2), d_ij = round(D_j p_ij), and
+    f_i = round(-1/2 c_i1 - 1/2 c_i2 - 1/2 d_i1 - 1/2 d_i2 + (1/Re) Lap u_i) (one 5-term sum)."""
     Dj = (Dx, Dy)
+    if skew:
+        p11 = round_product(u[0], u[0], chi_max, eps, chi_work)
+        p12 = round_product(u[0], u[1], chi_max, eps, chi_work)
+        p22 = round_product(u[1], u[1], chi_max, eps, chi_work)
+        pij = [[p11, p12], [p12, p22]]
     f = []
     for i in range(2):
         g = [round_mps(apply_mpo(Dj[j], u[i]), chi_max, eps) for j in range(2)]
         lap = round_mps(apply_mpo(Lap, u[i]), chi_max, eps)
         c = [round_product(u[j], g[j], chi_max, eps, chi_work) for j in range(2)]
-        f.append(round_mps(lincomb([(-1.0, c[0]), (-1.0, c[1]), (1.0 / Re, lap)]), chi_max, eps))
+        if skew:
+            d = [round_mps(apply_mpo(Dj[j], pij[i][j]), chi_max, eps) for j in range(2)]
+            terms = [(-0.5, c[0]), (-0.5, c[1]), (-0.5, d[0]), (-0.5, d[1]), (1.0 / Re, lap)]
+        else:
+            terms = [(-1.0, c[0]), (-1.0, c[1]), (1.0 / Re, lap)]
+        f.append(round_mps(lincomb(terms), chi_max, eps))
     return f
 
 
 # --------------------------------------------------------------------------- O9
-def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None):
+def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False):
     """Classical RK4 (Eq. 11) on the MPS pair u = [u_1, u_2]; all
     roundings with the same (chi_max, eps); final combination as one 5-term sum
     and one rounding (reading 10)."""
     def stage(k, h):
         return [round_mps(lincomb([(1.0, u[i]), (h, k[i])]), chi_max, eps) for i in range(2)]
 
-    k1 = rhs(u, Dx, Dy, Lap, Re, chi_max, eps, chi_work)
-    k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
-    k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
-    k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work)
+    k1 = rhs(u, Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
+    k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
+    k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
+    k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
     return [
         round_mps(
             lincomb([(1.0, u[i]), (dt / 6, k1[i]), (dt / 3, k2[i]), (dt / 3, k3[i]), (dt / 6, k4[i])]),

@@ -24,19 +24,29 @@ def lap5(F, dx):
     return (np.roll(F, -1, 0) + np.roll(F, 1, 0) + np.roll(F, -1, 1) + np.roll(F, 1, 1) - 4.0 * F) / dx**2
 
 
-def rhs_dense(ux, uy, Re, dx):
-    """PAPER.md:49-53 Eq. 2 without pressure, convective form."""
+def convection_skew(ux, uy, dx):
+    """PAPER.md:432-435 Eq. B2: 1/2 (u_j d_j u_i + d_j (u_j u_i)), summed over j."""
+    cx = 0.5 * (ux * ddx(ux, dx) + uy * ddy(ux, dx) + ddx(ux * ux, dx) + ddy(uy * ux, dx))
+    cy = 0.5 * (ux * ddx(uy, dx) + uy * ddy(uy, dx) + ddx(ux * uy, dx) + ddy(uy * uy, dx))
+    return cx, cy
+
+
+def rhs_dense(ux, uy, Re, dx, skew=False):
+    """PAPER.md:49-53 Eq. 2 without pressure; convective form, or the skew-symmetric form of Eq. B2."""
+    if skew:
+        cx, cy = convection_skew(ux, uy, dx)
+        return -cx + lap5(ux, dx) / Re, -cy + lap5(uy, dx) / Re
     fx = -(ux * ddx(ux, dx) + uy * ddy(ux, dx)) + lap5(ux, dx) / Re
     fy = -(ux * ddx(uy, dx) + uy * ddy(uy, dx)) + lap5(uy, dx) / Re
     return fx, fy
 
 
-def rk4_dense(ux, uy, Re, dt, dx):
+def rk4_dense(ux, uy, Re, dt, dx, skew=False):
     """PAPER.md:126 Eq. 11."""
-    k1 = rhs_dense(ux, uy, Re, dx)
-    k2 = rhs_dense(ux + dt / 2 * k1[0], uy + dt / 2 * k1[1], Re, dx)
-    k3 = rhs_dense(ux + dt / 2 * k2[0], uy + dt / 2 * k2[1], Re, dx)
-    k4 = rhs_dense(ux + dt * k3[0], uy + dt * k3[1], Re, dx)
+    k1 = rhs_dense(ux, uy, Re, dx, skew)
+    k2 = rhs_dense(ux + dt / 2 * k1[0], uy + dt / 2 * k1[1], Re, dx, skew)
+    k3 = rhs_dense(ux + dt / 2 * k2[0], uy + dt / 2 * k2[1], Re, dx, skew)
+    k4 = rhs_dense(ux + dt * k3[0], uy + dt * k3[1], Re, dx, skew)
     return (ux + dt / 6 * (k1[0] + 2 * k2[0] + 2 * k3[0] + k4[0]),
             uy + dt / 6 * (k1[1] + 2 * k2[1] + 2 * k3[1] + k4[1]))
 

@@ -317,3 +317,42 @@ def test_chi_eps_against_dense_truncation():
         assert err(chis[l]) <= eps * (1 + 1e-12)
         assert chis[l] == 1 or err(chis[l] - 1) > eps * (1 - 1e-12)
     assert chi == max(chis)
+
+
+# ---------------------------------------------------------------- skew-symmetric convection (PAPER.md Eq. B2)
+@pytest.mark.parametrize("n", [4, 5])
+def test_skew_rhs_and_rk4_equal_dense_at_full_rank(n):
+    """with nothing discarded the QTT right-hand side / RK4 step in the paper's
+    skew-symmetric form equals the dense one built from np.roll stencils (an independent restatement of Eq. B2)."""
+    Dx, Dy, Lap, dx = _ops(n)
+    ux, uy = smooth_field(n, 17), smooth_field(n, 18)
+    Re, dt = 50.0, 1e-3
+    u = [O.from_dense(ux), O.from_dense(uy)]
+    chi = 4 ** (n // 2)
+    f = O.rhs(u, Dx, Dy, Lap, Re, chi, chi_work=10**6, skew=True)
+    fx, fy = R.rhs_dense(ux, uy, Re, dx, skew=True)
+    assert rel(O.to_dense(f[0]), fx) < 1e-11 and rel(O.to_dense(f[1]), fy) < 1e-11
+    # the two forms differ on a field that is not divergence free: a dropped 1/2 or a missing term would show
+    gx, _ = R.rhs_dense(ux, uy, Re, dx)
+    assert rel(fx, gx) > 1e-3
+    v = O.rk4_step(u, Dx, Dy, Lap, Re, dt, chi, chi_work=10**6, skew=True)
+    vx, vy = R.rk4_dense(ux, uy, Re, dt, dx, skew=True)
+    assert rel(O.to_dense(v[0]), vx) < 1e-12 and rel(O.to_dense(v[1]), vy) < 1e-12
+
+
+def test_skew_convection_conserves_discrete_energy():
+    """The point of Eq. B2 ("better numerical stability"): with D^T = -D the
+    skew-symmetric convection does no work, sum_i <u_i, conv_i(u)> = 0 exactly, for ANY field; the convective form
+    does not have this property.  Checked on the oracle's QTT result at full rank."""
+    n = 5
+    Dx, Dy, Lap, dx = _ops(n)
+    ux, uy = smooth_field(n, 27), smooth_field(n, 28)
+    u = [O.from_dense(ux), O.from_dense(uy)]
+    chi = 4 ** (n // 2)
+    Re = 1e300  # no diffusion: f = -convection
+    f = O.rhs(u, Dx, Dy, Lap, Re, chi, chi_work=10**6, skew=True)
+    work = O.dot(u[0], f[0]) + O.dot(u[1], f[1])
+    scale = O.norm(u[0]) * O.norm(f[0]) + O.norm(u[1]) * O.norm(f[1])
+    assert abs(work) < 1e-12 * scale
+    g = O.rhs(u, Dx, Dy, Lap, Re, chi, chi_work=10**6)
+    assert abs(O.dot(u[0], g[0]) + O.dot(u[1], g[1])) > 1e-4 * scale
