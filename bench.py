@@ -34,11 +34,15 @@ METRICS = {2: "QTT RK4 steps/sec at 2^8x2^8, chi=32 fp64", 3: METRIC, 4: "QTT RK
 UNIT = "steps/s"
 
 
+SKEW = False  # --convection skew: the paper's skew-symmetric convection (PAPER.md Eq. B2) instead of the convective form
+
+
 def workload(cfg: int):
     c = I.CONFIGS[cfg]
     name = {2: "config2 double shear layer", 3: "config3 decaying jet", 4: "config4 decaying turbulence"}[cfg]
     desc = (f"{name}: 2^{c['n']}x2^{c['n']} grid ({c['n']} sites, d=4), chi_max={c['chi']}, chi_work={2 * c['chi']}, "
-            f"Re={c['Re']:g}, dt={c['dt']:g}, eps=0, one qtt_rk4_step per step")
+            f"Re={c['Re']:g}, dt={c['dt']:g}, eps=0, "
+            f"{'skew-symmetric convection (PAPER.md Eq. B2)' if SKEW else 'convective form'}, one qtt_rk4_step per step")
     return c, desc
 
 
@@ -108,7 +112,7 @@ def oracle_sample_seconds(cfg: int, state=None):
                      Lap=O.mpo_laplacian(n, dx))
     U = state["U"]
     t0 = time.perf_counter()
-    k1 = O.rhs(U, state["Dx"], state["Dy"], state["Lap"], c["Re"], chi)
+    k1 = O.rhs(U, state["Dx"], state["Dy"], state["Lap"], c["Re"], chi, skew=SKEW)
     U2 = [O.round_mps(O.lincomb([(1.0, U[i]), (c["dt"] / 2, k1[i])]), chi) for i in range(2)]
     t = time.perf_counter() - t0
     state["U"] = U2  # the next sample continues from the half-step state
@@ -202,6 +206,7 @@ def run_ours(args):
     c, desc = workload(args.config)
     n, chi = c["n"], c["chi"]
     ctx = Q.Context(device=local, workspace_bytes=int(args.workspace_gib * (1 << 30)))
+    Q.qtt_ctx_set_convection(ctx, SKEW)
     dx = 1.0 / (1 << n)
     Dx, Dy = Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx)
     Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
@@ -425,10 +430,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workspace-gib", type=float, default=8.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--convection", default="convective", choices=("convective", "skew"),
+                    help="convective (BASELINE.json's configs, default) or the paper's skew-symmetric form (Eq. B2)")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
                     help="only run the row-a2 site-contraction GEMM passes at the bulk-site shapes of bond CHI and "
                          "print their TFLOP/s (the command the ncu capture in profiles/ is taken on)")
     args = ap.parse_args()
+    global SKEW
+    SKEW = args.convection == "skew"
     if args.impl == "reference":
         return run_reference(args)
     if args.probe_contraction:

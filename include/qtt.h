@@ -66,6 +66,10 @@ qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes);
 /* 1: qtt_rk4_step with eps == 0 is captured once into a CUDA graph per shape signature and replayed
  * (default); 0: launches are issued eagerly every step. */
 qtt_status qtt_ctx_set_graphs(qtt_ctx* ctx, int enabled);
+/* Convection form of qtt_rk4_step.  0 (default): convective, u_j (.) D_j u_i (BASELINE config 2; reading 4).
+ * 1: the paper's skew-symmetric form, PAPER.md:432-435 Eq. B2, 1/2 (u_j (.) D_j u_i + D_j (u_j (.) u_i)): per
+ * right-hand side three more products (u_1 u_1, u_1 u_2, u_2 u_2), four more applies and 5-term sums. */
+qtt_status qtt_ctx_set_convection(qtt_ctx* ctx, int skew_symmetric);
 /* Synchronises the stream and reports the Jacobi convergence record since the last call:
  * the largest number of sweeps any SVD used, and how many SVDs hit the sweep limit (then QTT_NUMERIC). */
 qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits);

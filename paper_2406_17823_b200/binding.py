@@ -266,6 +266,10 @@ def qtt_ctx_set_chi_work(ctx: Context, chi_work: int) -> None:
     ctx.check(ctx.lib.qtt_ctx_set_chi_work(ctx.h, int(chi_work)))
 
 
+def qtt_ctx_set_convection(ctx: Context, skew_symmetric: bool) -> None:
+    ctx.check(ctx.lib.qtt_ctx_set_convection(ctx.h, 1 if skew_symmetric else 0))
+
+
 def qtt_ctx_set_graphs(ctx: Context, enabled: bool) -> None:
     ctx.check(ctx.lib.qtt_ctx_set_graphs(ctx.h, 1 if enabled else 0))
 

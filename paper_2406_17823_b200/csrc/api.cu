@@ -150,7 +150,7 @@ struct Rk4Plan {
   std::vector<int> rin[2], rout[2];
   const MpoData *Dx, *Dy, *Lap;
   double Re, dt;
-  int chi, chi_work;
+  int chi, chi_work, skew;
   double* in_buf[2] = {nullptr, nullptr};
   double* out_buf[2] = {nullptr, nullptr};
   cudaGraph_t graph = nullptr;
@@ -200,7 +200,7 @@ OutMps packed_out(const std::vector<int>& r, double* base) {
 
 // static output bonds of one RK4 step (eps == 0)
 void rk4_out_bonds(const std::vector<int> rin[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, int chi,
-                   int chi_work, std::vector<int> rout[2]) {
+                   int chi_work, int skew, std::vector<int> rout[2]) {
   auto applied = [&](const MpoData* W, const std::vector<int>& r) {
     std::vector<int> e(r.size());
     for (size_t k = 0; k < r.size(); ++k) e[k] = W->D[k] * r[k];
@@ -219,7 +219,14 @@ void rk4_out_bonds(const std::vector<int> rin[2], const MpoData* Dx, const MpoDa
       std::vector<int> rw, c0, c1;
       qtt_zip_caps(u[0], g0, chi, chi_work, rw, c0);
       qtt_zip_caps(u[1], g1, chi, chi_work, rw, c1);
-      f[i] = summed({c0, c1, l});
+      if (skew) {
+        std::vector<int> p0, p1;
+        qtt_zip_caps(u[0], u[i], chi, chi_work, rw, p0);
+        qtt_zip_caps(u[i], u[1], chi, chi_work, rw, p1);
+        f[i] = summed({c0, c1, applied(Dx, p0), applied(Dy, p1), l});
+      } else {
+        f[i] = summed({c0, c1, l});
+      }
     }
   };
   std::vector<int> k1[2], k2[2], k3[2], k4[2], us[2];
@@ -317,6 +324,11 @@ qtt_status qtt_ctx_set_chi_work(qtt_ctx* ctx, int chi_work) {
 qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes) {
   if (!ctx) return QTT_INVALID_ARG;
   ctx->mat_limit = bytes;
+  return QTT_OK;
+}
+qtt_status qtt_ctx_set_convection(qtt_ctx* ctx, int skew_symmetric) {
+  if (!ctx || (skew_symmetric != 0 && skew_symmetric != 1)) return QTT_INVALID_ARG;
+  ctx->skew = skew_symmetric;
   return QTT_OK;
 }
 qtt_status qtt_ctx_set_graphs(qtt_ctx* ctx, int enabled) {
@@ -635,12 +647,12 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
     // eager path (eps > 0 synchronises once per bond)
     View uv[2] = {materialize(ctx, u[0]->body), materialize(ctx, u[1]->body)};
     std::vector<int> rin[2] = {uv[0].r, uv[1].r}, rout[2];
-    rk4_out_bonds(rin, Dx->data, Dy->data, Lap->data, chi_max, cw, rout);
+    rk4_out_bonds(rin, Dx->data, Dy->data, Lap->data, chi_max, cw, ctx->skew, rout);
     Body* fresh[2] = {body_new_dense(ctx, rout[0]), nullptr};
     try {
       fresh[1] = body_new_dense(ctx, rout[1]);
       OutMps out[2] = {out_of_body(fresh[0]), out_of_body(fresh[1])};
-      qtt_rk4_eager(ctx, uv, Dx->data, Dy->data, Lap->data, Re, dt, chi_max, eps, cw, out);
+      qtt_rk4_eager(ctx, uv, Dx->data, Dy->data, Lap->data, Re, dt, chi_max, eps, cw, ctx->skew, out);
       body_set_bonds(fresh[0], out[0].r);
       body_set_bonds(fresh[1], out[1].r);
     } catch (...) {
@@ -660,7 +672,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
   Rk4Plan* plan = nullptr;
   for (Rk4Plan* p : ctx->plans)
     if (p->rin[0] == uv[0].r && p->rin[1] == uv[1].r && p->Dx == Dx->data && p->Dy == Dy->data &&
-        p->Lap == Lap->data && p->Re == Re && p->dt == dt && p->chi == chi_max && p->chi_work == cw &&
+        p->Lap == Lap->data && p->Re == Re && p->dt == dt && p->chi == chi_max && p->chi_work == cw && p->skew == ctx->skew &&
         p->lo0 == ctx->arena.lo && p->hi0 == ctx->arena.hi)
       plan = p;
   if (!plan) {
@@ -672,10 +684,10 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
     plan = new Rk4Plan();
     plan->Dx = Dx->data; plan->Dy = Dy->data; plan->Lap = Lap->data;
     ++Dx->data->refs; ++Dy->data->refs; ++Lap->data->refs;
-    plan->Re = Re; plan->dt = dt; plan->chi = chi_max; plan->chi_work = cw;
+    plan->Re = Re; plan->dt = dt; plan->chi = chi_max; plan->chi_work = cw; plan->skew = ctx->skew;
     plan->lo0 = ctx->arena.lo; plan->hi0 = ctx->arena.hi;
     for (int i = 0; i < 2; ++i) plan->rin[i] = uv[i].r;
-    rk4_out_bonds(plan->rin, Dx->data, Dy->data, Lap->data, chi_max, cw, plan->rout);
+    rk4_out_bonds(plan->rin, Dx->data, Dy->data, Lap->data, chi_max, cw, ctx->skew, plan->rout);
     try {
       for (int i = 0; i < 2; ++i) {
         plan->in_buf[i] = static_cast<double*>(ctx->alloc(cores_doubles(plan->rin[i]) * sizeof(double), ctx->user));
@@ -687,7 +699,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
       const long long launches_before = g_qtt_launch_count;  // captured launches run at replay, counted there
       QTT_CU(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed));
       try {
-        qtt_rk4_eager(ctx, pin, Dx->data, Dy->data, Lap->data, Re, dt, chi_max, 0.0, cw, pout);
+        qtt_rk4_eager(ctx, pin, Dx->data, Dy->data, Lap->data, Re, dt, chi_max, 0.0, cw, ctx->skew, pout);
       } catch (...) {
         cudaGraph_t junk = nullptr;
         g_qtt_launch_count = launches_before;

@@ -91,6 +91,7 @@ struct qtt_ctx {
   int chi_work = 0;
   size_t mat_limit = (size_t)2 << 30;
   int graphs = 1;
+  int skew = 0;  // 1: skew-symmetric convection (PAPER.md Eq. B2) in qtt_rk4_step
   int profiling = 0;
   double* ones = nullptr;   // device: 1.0
   int* jac_status = nullptr;  // device: [max sweeps, limit hits]
@@ -134,7 +135,7 @@ void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<doub
 View qtt_kron(qtt_ctx* ctx, const View& a, const View& b);
 
 void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
-                   double dt, int chi, double eps, int chi_work, OutMps out[2]);
+                   double dt, int chi, double eps, int chi_work, int skew, OutMps out[2]);
 
 void qtt_to_dense_view(qtt_ctx* ctx, const View& v, double* dense_dev_out);
 void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, double eps, OutMps& out);

@@ -814,7 +814,7 @@ View view_of(const OutMps& o) {
 
 // f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i   (oracle O8)
 void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap, double Re, int chi, double eps,
-         int chi_work, View f[2]) {
+         int chi_work, int skew, View f[2]) {
   // level 1: six applies + roundings: (D1 u_i, D2 u_i, Lap u_i) for i = 0, 1.  The two Laplacians are only needed by
   // level 3, so -- when the context has a side stream whose scratch region is large enough -- they are rounded
   // there, concurrently with the four D_j u_i on the main stream and with the products of level 2.
@@ -877,14 +877,20 @@ void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap
     for (int i = 0; i < 6; ++i) g[i] = view_of(out[i]);
     ctx->arena.hi = mark;
   }
-  // level 2: four products c_ij = u_j (.) g_ij
-  std::vector<View> c(4);
+  // level 2: four products c_ij = u_j (.) g_ij; with the skew-symmetric convection (PAPER.md:432-435 Eq. B2) also
+  // p_11 = u_1 (.) u_1, p_12 = u_1 (.) u_2 (= p_21), p_22 = u_2 (.) u_2 in the same batch
+  std::vector<View> c(4), pq(3);
   {
     const size_t mark = ctx->arena.hi;
     std::vector<View> A{u[0], u[1], u[0], u[1]};
     std::vector<View> B{g[0], g[1], g[3], g[4]};
+    if (skew) {
+      A.push_back(u[0]); B.push_back(u[0]);
+      A.push_back(u[0]); B.push_back(u[1]);
+      A.push_back(u[1]); B.push_back(u[1]);
+    }
     std::vector<std::vector<int>> caps;
-    for (int i = 0; i < 4; ++i) {
+    for (size_t i = 0; i < A.size(); ++i) {
       std::vector<int> rw, ro;
       qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro);
       caps.push_back(ro);
@@ -892,6 +898,23 @@ void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap
     std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
     qtt_round_product_batch(ctx, A, B, chi, eps, chi_work, out);
     for (int i = 0; i < 4; ++i) c[i] = view_of(out[i]);
+    if (skew)
+      for (int i = 0; i < 3; ++i) pq[i] = view_of(out[4 + i]);
+    ctx->arena.hi = mark;
+  }
+  // level 2b (skew only): d_ij = round(D_j p_ij) for (i,j) = (1,1), (1,2), (2,1), (2,2)
+  std::vector<View> d(4);
+  if (skew) {
+    const size_t mark = ctx->arena.hi;
+    std::vector<const MpoData*> W{Dj[0], Dj[1], Dj[0], Dj[1]};
+    std::vector<View> X{pq[0], pq[1], pq[1], pq[2]};
+    std::vector<View> ex;
+    qtt_expand_apply_batch(ctx, W, X, ex);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : ex) caps.push_back(qtt_round_caps(e.r, chi));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, ex, chi, eps, out);
+    for (int i = 0; i < 4; ++i) d[i] = view_of(out[i]);
     ctx->arena.hi = mark;
   }
   // level 3: f_i = -c_i1 - c_i2 + lap_i / Re, one rounding each
@@ -899,7 +922,12 @@ void rhs(qtt_ctx* ctx, const View u[2], const MpoData* Dj[2], const MpoData* Lap
   {
     const size_t mark = ctx->arena.hi;
     std::vector<std::vector<std::pair<double, View>>> terms(2);
-    for (int i = 0; i < 2; ++i) terms[i] = {{-1.0, c[2 * i]}, {-1.0, c[2 * i + 1]}, {1.0 / Re, g[3 * i + 2]}};
+    for (int i = 0; i < 2; ++i) {
+      if (skew)
+        terms[i] = {{-0.5, c[2 * i]}, {-0.5, c[2 * i + 1]}, {-0.5, d[2 * i]}, {-0.5, d[2 * i + 1]}, {1.0 / Re, g[3 * i + 2]}};
+      else
+        terms[i] = {{-1.0, c[2 * i]}, {-1.0, c[2 * i + 1]}, {1.0 / Re, g[3 * i + 2]}};
+    }
     std::vector<View> s;
     qtt_concat_batch(ctx, terms, s);
     std::vector<std::vector<int>> caps;
@@ -923,7 +951,7 @@ void lincomb_round(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double,
 }  // namespace
 
 void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
-                   double dt, int chi, double eps, int chi_work, OutMps out[2]) {
+                   double dt, int chi, double eps, int chi_work, int skew, OutMps out[2]) {
   const MpoData* Dj[2] = {Dx, Dy};
   View k1[2], k2[2], k3[2], k4[2], us[2];
   auto stage = [&](const View kk[2], double h, View dst[2]) {
@@ -940,13 +968,13 @@ void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoDa
     lincomb_round(ctx, terms, chi, eps, o);
     for (int i = 0; i < 2; ++i) dst[i] = view_of(o[i]);
   };
-  rhs(ctx, u, Dj, Lap, Re, chi, eps, chi_work, k1);
+  rhs(ctx, u, Dj, Lap, Re, chi, eps, chi_work, skew, k1);
   stage(k1, dt / 2, us);
-  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k2);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, skew, k2);
   stage(k2, dt / 2, us);
-  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k3);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, skew, k3);
   stage(k3, dt, us);
-  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k4);
+  rhs(ctx, us, Dj, Lap, Re, chi, eps, chi_work, skew, k4);
   std::vector<std::vector<std::pair<double, View>>> terms(2);
   for (int i = 0; i < 2; ++i)
     terms[i] = {{1.0, u[i]}, {dt / 6, k1[i]}, {dt / 3, k2[i]}, {dt / 3, k3[i]}, {dt / 6, k4[i]}};

@@ -444,3 +444,41 @@ def test_diagnostics_match_oracle(Q, ctx):
         got, gmax = Q.qtt_mps_chi_eps(ctx, a, eps)
         want, wmax = O.chi_eps(A, eps)
         assert got == want and gmax == wmax
+
+
+@pytest.mark.parametrize("graphs", [False, True])
+def test_rk4_step_skew_symmetric_matches_oracle(Q, ctx, graphs):
+    """qtt_ctx_set_convection(1): the paper's skew-symmetric convection (PAPER.md Eq. B2, section 8f next-2), two steps
+    on a 2^6 x 2^6 grid and one step of BASELINE config 2, against the oracle's rhs(skew=True)."""
+    Q.qtt_ctx_set_convection(ctx, True)
+    Q.qtt_ctx_set_graphs(ctx, graphs)
+    try:
+        n, chi, Re, dt = 6, 12, 100.0, 1e-3
+        g, o = ops(Q, ctx, n)
+        X, Y = I.grid(n)
+        ux = np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y) + 0.3 * smooth_field(n, 4)
+        uy = -np.cos(2 * np.pi * X) * np.sin(2 * np.pi * Y) + 0.3 * smooth_field(n, 5)
+        U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+        u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+        for _ in range(2):
+            U = O.rk4_step(U, o[0], o[1], o[2], Re, dt, chi, skew=True)
+            Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], Re, dt, chi)
+            for i in range(2):
+                assert Q.qtt_mps_bonds(u[i]) == O.bonds(U[i])
+                assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U[i])) < TOL
+        if graphs:
+            cfg = I.CONFIGS[2]
+            n, chi = cfg["n"], cfg["chi"]
+            fx, fy = I.config_fields(2)
+            g, o = ops(Q, ctx, n)
+            U = [O.from_dense(fx, chi), O.from_dense(fy, chi)]
+            u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+            U1 = O.rk4_step(U, o[0], o[1], o[2], cfg["Re"], cfg["dt"], chi, skew=True)
+            Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+            for i in range(2):
+                assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+                assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < TOL
+        assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+    finally:
+        Q.qtt_ctx_set_convection(ctx, False)
+        Q.qtt_ctx_set_graphs(ctx, True)
