@@ -246,7 +246,7 @@ def run_ours(args):
     value = whole_job_value(world, args.steps, ms)
 
     # ---- end to end through the C ABI with HOST buffers: cores in pinned host memory -> device, step, cores back
-    host = [Q.qtt_mps_get_cores(ctx, x) for x in u]
+    host = [Q.qtt_mps_get_cores(ctx, x, pinned=True) for x in u]
     h2d = sum(a.nbytes for cs in host for a in cs)
     e2e_steps = max(1, min(args.steps, 5))
     barrier()
@@ -255,7 +255,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         v = [Q.qtt_mps_from_cores(ctx, cs) for cs in host]
         Q.qtt_rk4_step(ctx, v, Dx, Dy, Lap, c["Re"], c["dt"], chi)
-        host = [Q.qtt_mps_get_cores(ctx, x) for x in v]
+        host = [Q.qtt_mps_get_cores(ctx, x, pinned=True) for x in v]
         d2h = sum(a.nbytes for cs in host for a in cs)
     torch.cuda.synchronize()
     e2e_sec = (time.perf_counter() - t0) / e2e_steps

@@ -207,15 +207,22 @@ def qtt_mps_bonds(x: Mps) -> list[int]:
     return list(b)
 
 
-def qtt_mps_get_core(ctx: Context, x: Mps, k: int) -> np.ndarray:
+def _host_array(shape, pinned: bool) -> np.ndarray:
+    """A float64 host array; pinned=True backs it with page-locked memory (torch owns it, the array is a view)."""
+    if not pinned:
+        return np.empty(shape, dtype=np.float64)
+    return torch.empty(shape, dtype=torch.float64, pin_memory=True).numpy()
+
+
+def qtt_mps_get_core(ctx: Context, x: Mps, k: int, pinned: bool = False) -> np.ndarray:
     r = qtt_mps_bonds(x)
-    out = np.empty((r[k], 4, r[k + 1]), dtype=np.float64)
+    out = _host_array((r[k], 4, r[k + 1]), pinned)
     ctx.check(ctx.lib.qtt_mps_get_core(ctx.h, x.h, k, out.ctypes.data_as(C.POINTER(C.c_double))))
     return out
 
 
-def qtt_mps_get_cores(ctx: Context, x: Mps) -> list[np.ndarray]:
-    return [qtt_mps_get_core(ctx, x, k) for k in range(ctx.lib.qtt_mps_num_sites(x.h))]
+def qtt_mps_get_cores(ctx: Context, x: Mps, pinned: bool = False) -> list[np.ndarray]:
+    return [qtt_mps_get_core(ctx, x, k, pinned) for k in range(ctx.lib.qtt_mps_num_sites(x.h))]
 
 
 def qtt_mps_dot(ctx: Context, a: Mps, b: Mps) -> float:
