@@ -33,6 +33,7 @@ where the paper is silent/garbled and the reading taken):
   O8  rhs                       PAPER.md:49-53 Eq. 2 without pressure (Burgers form)
   O9  rk4_step                  PAPER.md:124-128 Eq. 11
   O10 mpo_d1 / mpo_d2 / mpo_laplacian   PAPER.md:391-424 App. A, Eq. A1-A3, Table II
+      mpo_stencil (any order)   PAPER.md:98, same construction
   O11 fidelity, chi_eps         PAPER.md:160 Eq. 12; Eq. 16-17 (diagnostics)
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
@@ -350,6 +351,43 @@ def mpo_laplacian(n: int, dx: float):
             C[0, :, :, base + a] = src[0, :, :, a]       # start a shift, no carry out
             C[base + a, :, :, base + a] = src[a, :, :, a]  # shift with carry out
     return _fold_boundaries([C] * n, np.ones(5), np.array([-4.0, 1.0, 1.0, 1.0, 1.0]) / dx**2)
+
+
+def mpo_stencil(n: int, direction: int, coeffs):
+    """General periodic finite-difference stencil along one direction as an MPO ("MPOs for finite-difference
+    stencils of any order"):
+        (O F)[x] = sum_{k=-K..K} coeffs[k + K] * F[x + k]      (x periodic, the other coordinate untouched),
+    2K + 1 = len(coeffs).  Same construction as App. A: the bond carries the carry of the
+    addition x + k, running from the least-significant site to the most-significant one.  Bond index
+    alpha = carry + K, carry in [-K, K]; at a site with output bit b (of the shifted coordinate) and incoming carry c,
+    the input bit is (b + c) mod 2 and the outgoing carry floor((b + c) / 2).  L = ones (periodic: the last carry is
+    dropped), R[c + K] = coeffs[c + K] (the offset k enters as the initial carry).  Index order [alpha_m][w][w'][alpha_{m+1}],
+    w = output (reading 1)."""
+    coeffs = np.asarray(coeffs, dtype=np.float64)
+    assert direction in (1, 2) and len(coeffs) % 2 == 1 and n >= 2
+    K = (len(coeffs) - 1) // 2
+    D = 2 * K + 1
+    C = np.zeros((D, D_PHYS, D_PHYS, D))
+    for cin in range(-K, K + 1):
+        for w in range(D_PHYS):
+            xb, yb = w >> 1, w & 1
+            b = xb if direction == 1 else yb
+            s = b + cin
+            bin_ = s % 2
+            cout = (s - bin_) // 2
+            wp = (bin_ << 1 | yb) if direction == 1 else (xb << 1 | bin_)
+            C[cout + K, w, wp, cin + K] = 1.0
+    cores = [C.copy() for _ in range(n)]
+    cores[0] = np.einsum("a,awvb->wvb", np.ones(D), C)[None]          # L on the most-significant end
+    cores[-1] = np.einsum("awvb,b->awv", C, coeffs)[..., None]        # R on the least-significant end
+    return cores
+
+
+def fd_coefficients(order: int, dx: float):
+    """Central first-derivative coefficients of even order 2, 4, 6, 8 for offsets -K..K (K = order / 2)."""
+    table = {2: [0.5], 4: [2.0 / 3, -1.0 / 12], 6: [0.75, -0.15, 1.0 / 60], 8: [0.8, -0.2, 4.0 / 105, -1.0 / 280]}
+    pos = table[order]
+    return np.array([-c for c in pos[::-1]] + [0.0] + pos) / dx
 
 
 def mpo_to_dense(W) -> np.ndarray:

@@ -177,3 +177,47 @@ def test_derivative_of_sine_is_analytic_stencil_and_rounds_to_bond_two():
     # Laplacian: -(2 - 2 cos(2 pi dx))/dx^2 * sin
     Lp = O.apply_mpo(O.mpo_laplacian(n, dx), A)
     assert rel(O.to_dense(Lp), -(2 - 2 * np.cos(2 * np.pi * dx)) / dx**2 * np.sin(2 * np.pi * X)) < 1e-11
+
+
+# ---------------------------------------------------------------- stencils of any order
+def _roll_stencil(F, coeffs, axis):
+    K = (len(coeffs) - 1) // 2
+    return sum(c * np.roll(F, -k, axis=axis) for k, c in zip(range(-K, K + 1), coeffs))
+
+
+@pytest.mark.parametrize("direction", [1, 2])
+@pytest.mark.parametrize("order", [2, 4, 8])
+def test_mpo_stencil_equals_rolled_stencil(direction, order):
+    n = 5
+    dx = 1.0 / (1 << n)
+    c = O.fd_coefficients(order, dx)
+    W = O.mpo_stencil(n, direction, c)
+    F = np.random.default_rng(order + direction).standard_normal((1 << n, 1 << n))
+    got = O.to_dense(O.apply_mpo(W, O.from_dense(F)))
+    want = _roll_stencil(F, c, axis=direction - 1)
+    assert np.linalg.norm(got - want) <= 1e-12 * np.linalg.norm(want)
+    assert [w.shape[0] for w in W[1:]] == [order + 1] * (n - 1)      # bond 2K + 1
+
+
+def test_mpo_stencil_order_two_is_table_II_operator():
+    """K = 1 with (-1, 0, 1) / (2 dx) is the operator of PAPER.md Table II (a different bond basis, same matrix)."""
+    n = 4
+    dx = 1.0 / (1 << n)
+    for direction, ref in ((1, O.mpo_d1(n, dx)), (2, O.mpo_d2(n, dx))):
+        A = O.mpo_to_dense(O.mpo_stencil(n, direction, O.fd_coefficients(2, dx)))
+        B = O.mpo_to_dense(ref)
+        assert np.max(np.abs(A - B)) <= 1e-12 * np.max(np.abs(B))
+
+
+def test_mpo_stencil_convergence_orders():
+    """d/dx sin(2 pi x) by the order-p stencil has error ~ dx^p: halving dx divides it by 2^p (within 15 %)."""
+    for order in (2, 4, 6):
+        errs = []
+        for n in (4, 5):
+            dx = 1.0 / (1 << n)
+            X, _ = I.grid(n)
+            F = np.sin(2 * np.pi * X)
+            got = O.to_dense(O.apply_mpo(O.mpo_stencil(n, 1, O.fd_coefficients(order, dx)), O.from_dense(F)))
+            errs.append(np.max(np.abs(got - 2 * np.pi * np.cos(2 * np.pi * X))))
+        ratio = errs[0] / errs[1]
+        assert 0.85 * 2**order < ratio < 1.15 * 2**order, (order, ratio)
