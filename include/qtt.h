@@ -108,6 +108,11 @@ qtt_status qtt_mpo_central_difference(qtt_ctx* ctx, int n_sites, int direction, 
 /* Compact periodic 5-point Laplacian MPO, bond 5 (reading 3): channels identity, x+1, x-1, y+1, y-1;
  * L = (1,1,1,1,1), R = (-4,1,1,1,1)/dx^2.  n_sites >= 2. */
 qtt_status qtt_mpo_laplacian(qtt_ctx* ctx, int n_sites, double dx, qtt_mpo** out);
+/* PAPER.md:98 ("MPOs for finite-difference stencils of any order"), construction of App. A generalised: the periodic
+ * stencil (O F)[x] = sum_{k=-K..K} coeffs_host[k + K] * F[x + k] along direction 1 (x) or 2 (y), K = half_width in
+ * 1..16, as an MPO of bond 2K + 1 (bond index = carry of the addition x + k + K).  n_sites >= 2. */
+qtt_status qtt_mpo_stencil(qtt_ctx* ctx, int n_sites, int direction, int half_width, const double* coeffs_host,
+                           qtt_mpo** out);
 void qtt_mpo_free(qtt_mpo* w);
 
 /* y = W x, exact, bond D*chi, composite bond index = alpha*chi + a (lazy). */

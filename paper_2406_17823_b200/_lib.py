@@ -45,6 +45,7 @@ PROTOTYPES = {
     "qtt_to_dense": (C.c_int, [_P, _P, _P]),
     "qtt_mpo_create": (C.c_int, [_P, C.c_int, _IP, _DPP, _PP]),
     "qtt_mpo_central_difference": (C.c_int, [_P, C.c_int, C.c_int, C.c_double, _PP]),
+    "qtt_mpo_stencil": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, _DP, _PP]),
     "qtt_mpo_laplacian": (C.c_int, [_P, C.c_int, C.c_double, _PP]),
     "qtt_mpo_free": (None, [_P]),
     "qtt_apply_mpo": (C.c_int, [_P, _P, _P, _PP]),

@@ -162,6 +162,17 @@ def qtt_mpo_central_difference(ctx: Context, n_sites: int, direction: int, dx: f
     return Mpo(ctx, h)
 
 
+def qtt_mpo_stencil(ctx: Context, n_sites: int, direction: int, coeffs: Sequence[float]) -> Mpo:
+    """(O F)[x] = sum_k coeffs[k + K] F[x + k], 2K + 1 = len(coeffs), along direction 1 (x) or 2 (y)."""
+    c = np.ascontiguousarray(coeffs, dtype=np.float64)
+    if c.ndim != 1 or len(c) % 2 != 1 or len(c) < 3:
+        raise ValueError("coeffs must hold 2K + 1 >= 3 values")
+    h = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mpo_stencil(ctx.h, int(n_sites), int(direction), (len(c) - 1) // 2,
+                                      c.ctypes.data_as(C.POINTER(C.c_double)), C.byref(h)))
+    return Mpo(ctx, h)
+
+
 def qtt_mpo_laplacian(ctx: Context, n_sites: int, dx: float) -> Mpo:
     h = C.c_void_p()
     ctx.check(ctx.lib.qtt_mpo_laplacian(ctx.h, n_sites, float(dx), C.byref(h)))

@@ -77,6 +77,39 @@ qtt_status qtt_mpo_central_difference(qtt_ctx* ctx, int n_sites, int direction, 
   return build(ctx, n_sites, ch, R, out);
 }
 
+qtt_status qtt_mpo_stencil(qtt_ctx* ctx, int n_sites, int direction, int half_width, const double* coeffs_host,
+                           qtt_mpo** out) {
+  if (!ctx || !out || !coeffs_host || n_sites < 2 || half_width < 1 || half_width > 16) return QTT_INVALID_ARG;
+  if (direction != 1 && direction != 2) return QTT_INVALID_ARG;
+  // carry automaton of x + k (App. A generalised to |k| <= K): bond index = carry + K
+  const int K = half_width, D = 2 * K + 1;
+  std::vector<double> C((size_t)D * 16 * D, 0.0);
+  for (int cin = -K; cin <= K; ++cin)
+    for (int w = 0; w < 4; ++w) {
+      const int xb = w >> 1, yb = w & 1;
+      const int b = (direction == 1) ? xb : yb;
+      const int s = b + cin;
+      const int bin = ((s % 2) + 2) % 2;
+      const int cout = (s - bin) / 2;  // exact: s - bin is even
+      const int wp = (direction == 1) ? ((bin << 1) | yb) : ((xb << 1) | bin);
+      C[(((size_t)(cout + K) * 4 + w) * 4 + wp) * D + (cin + K)] = 1.0;
+    }
+  std::vector<double> first((size_t)16 * D, 0.0), last((size_t)D * 16, 0.0);
+  for (int am = 0; am < D; ++am)
+    for (int e = 0; e < 16; ++e)
+      for (int a1 = 0; a1 < D; ++a1) {
+        const double v = C[((size_t)am * 16 + e) * D + a1];
+        first[(size_t)e * D + a1] += v;                        // L = ones on the most-significant end
+        last[(size_t)am * 16 + e] += v * coeffs_host[a1];      // R = coefficients on the least-significant end
+      }
+  std::vector<int> bonds(n_sites + 1, D);
+  bonds[0] = bonds[n_sites] = 1;
+  std::vector<const double*> cores(n_sites, C.data());
+  cores[0] = first.data();
+  cores[n_sites - 1] = last.data();
+  return qtt_mpo_create(ctx, n_sites, bonds.data(), cores.data(), out);
+}
+
 qtt_status qtt_mpo_laplacian(qtt_ctx* ctx, int n_sites, double dx, qtt_mpo** out) {
   if (!(dx > 0.0)) return QTT_INVALID_ARG;
   std::vector<Channel> ch{{-1, 0}, {1, +1}, {1, -1}, {0, +1}, {0, -1}};

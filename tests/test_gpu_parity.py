@@ -482,3 +482,44 @@ def test_rk4_step_skew_symmetric_matches_oracle(Q, ctx, graphs):
     finally:
         Q.qtt_ctx_set_convection(ctx, False)
         Q.qtt_ctx_set_graphs(ctx, True)
+
+
+@pytest.mark.parametrize("order", [2, 4, 8])
+def test_stencil_mpo_matches_oracle(Q, ctx, order):
+    """qtt_mpo_stencil (stencils of any order; section 8f next-2): exact apply and apply + round against
+    the oracle's mpo_stencil, both directions."""
+    n, chi = 6, 10
+    dx = 1.0 / (1 << n)
+    A = O.from_dense(smooth_field(n, 31) + 1e-2 * np.random.default_rng(2).standard_normal((1 << n, 1 << n)), chi)
+    a = Q.qtt_mps_from_cores(ctx, A)
+    c = O.fd_coefficients(order, dx)
+    for direction in (1, 2):
+        Wo = O.mpo_stencil(n, direction, c)
+        Wg = Q.qtt_mpo_stencil(ctx, n, direction, c)
+        y = Q.qtt_apply_mpo(ctx, Wg, a)
+        assert Q.qtt_mps_bonds(y) == O.bonds(O.apply_mpo(Wo, A))
+        assert rel(gpu_dense(Q, ctx, y), O.to_dense(O.apply_mpo(Wo, A))) < 1e-13
+        Q.qtt_round(ctx, y, chi)
+        want = O.round_mps(O.apply_mpo(Wo, A), chi)
+        assert Q.qtt_mps_bonds(y) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, y), O.to_dense(want)) < TOL
+
+
+def test_rk4_step_with_fourth_order_stencils_matches_oracle(Q, ctx):
+    """One qtt_rk4_step with 4th-order first-derivative MPOs (bond 5) in place of the 2nd-order ones."""
+    n, chi, Re, dt = 6, 12, 100.0, 1e-3
+    dx = 1.0 / (1 << n)
+    g, o = ops(Q, ctx, n)
+    c4 = O.fd_coefficients(4, dx)
+    Dg = [Q.qtt_mpo_stencil(ctx, n, d, c4) for d in (1, 2)]
+    Do = [O.mpo_stencil(n, d, c4) for d in (1, 2)]
+    X, Y = I.grid(n)
+    ux = np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y) + 0.3 * smooth_field(n, 4)
+    uy = -np.cos(2 * np.pi * X) * np.sin(2 * np.pi * Y) + 0.3 * smooth_field(n, 5)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+    U1 = O.rk4_step(U, Do[0], Do[1], o[2], Re, dt, chi)
+    Q.qtt_rk4_step(ctx, u, Dg[0], Dg[1], g[2], Re, dt, chi)
+    for i in range(2):
+        assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+        assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < TOL
