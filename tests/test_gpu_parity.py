@@ -362,7 +362,7 @@ def test_config4_size_primitives_match_oracle(Q, big_ctx):
     assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
 
 
-@pytest.mark.parametrize("chi", [16, 32])
+@pytest.mark.parametrize("chi", [16, 32, 64, 128])
 def test_config5_primitive_sweep_matches_oracle(Q, big_ctx, chi):
     """BASELINE config 5 (2^12 x 2^12, random left-canonical MPS, batch of 6 operands per launch): every operand gets
     one apply (d/dx, d/dy or Laplacian) + round(chi) and one Hadamard with the next operand + round(chi), batched
