@@ -340,6 +340,68 @@ def contraction_probe(ctx, chi, peak):
                     "4 operands per launch, operands larger than L2 in total (0.5 GiB), CUDA events on the launching stream"}
 
 
+def primitive_sweep(args):
+    """BASELINE.json configs[4]: 2^12 x 2^12 (12 sites), random N(0,1) site tensors with the full bond profile, batch of
+    6 operands per launch; per chi: one apply (d/dx, d/dy or Laplacian MPO) + round(chi) and one Hadamard with the next
+    operand + round(chi), each timed with CUDA events on the context's stream (median of `steps` repetitions after
+    `warmup`), plus the kernel-family split of one profiled repetition.  Prints ONE JSON line."""
+    import torch
+    import paper_2406_17823_b200 as Q
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    n = 12
+    ctx = Q.Context(device=0, workspace_bytes=int(max(args.workspace_gib, 24.0) * (1 << 30)))
+    dx = 1.0 / (1 << n)
+    mpos = [Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx),
+            Q.qtt_mpo_laplacian(ctx, n, dx)]
+    peaks = fp64_peaks(Q, ctx)
+    out = {}
+    for chi in (16, 32, 64, 128):
+        xs = [Q.qtt_mps_from_cores(ctx, I.random_cores(n, chi, seed=s)) for s in range(6)]
+
+        def apply_round():
+            ys = [Q.qtt_apply_mpo(ctx, mpos[i % 3], xs[i]) for i in range(6)]
+            Q.qtt_round_batch(ctx, ys, chi)
+
+        def hadamard_round():
+            hs = [Q.qtt_hadamard(ctx, xs[i], xs[(i + 1) % 6]) for i in range(6)]
+            Q.qtt_round_batch(ctx, hs, chi)
+
+        res = {}
+        for name, fn in (("apply_round", apply_round), ("hadamard_round", hadamard_round)):
+            for _ in range(max(args.warmup, 1)):
+                fn()
+            ctx.synchronize()
+            times = []
+            with torch.cuda.stream(ctx.stream):
+                for _ in range(max(args.steps, 1)):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(ctx.stream)
+                    fn()
+                    e1.record(ctx.stream)
+                    e1.synchronize()
+                    times.append(e0.elapsed_time(e1))
+            Q.qtt_ctx_profile(ctx, True)
+            Q.qtt_ctx_profile_report(ctx)
+            fn()
+            rep = Q.qtt_ctx_profile_report(ctx)
+            Q.qtt_ctx_profile(ctx, False)
+            g = rep["gemm"]
+            res[name] = {"ms_per_batch_of_6": float(np.median(times)),
+                         "family_ms": {k: round(v["ms"], 3) for k, v in rep.items()},
+                         "gemm_tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12,
+                         "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"]}
+        out[str(chi)] = res
+        del xs
+    line = {"metric": "primitive sweep at 2^12x2^12, batch 6 (BASELINE.json configs[4])", "unit": "ms per batch of 6",
+            "dtype": "f64", "data": "synthetic", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "chi": out, "fp64_peaks_tflops": peaks,
+            "not_run": {"256": "the zip-up SVD at chi = 256 has 2048 columns: beyond the streamed Jacobi kernel (<= 1024), "
+                               "see DESIGN.md known limits"}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     """Per-kernel-family device times of one more (eagerly launched, event-bracketed) step -> roofline of the
     dominant family; the site-contraction TFLOP/s; and the CPU oracle timed on a bounded sample."""
@@ -430,6 +492,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workspace-gib", type=float, default=8.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--primitive-sweep", action="store_true",
+                    help="BASELINE.json configs[4]: time apply+round and hadamard+round at 2^12 x 2^12, chi = 16..128, "
+                         "batch 6, instead of the RK4 step")
     ap.add_argument("--convection", default="convective", choices=("convective", "skew"),
                     help="convective (BASELINE.json's configs, default) or the paper's skew-symmetric form (Eq. B2)")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
@@ -440,6 +505,8 @@ def main():
     SKEW = args.convection == "skew"
     if args.impl == "reference":
         return run_reference(args)
+    if args.primitive_sweep:
+        return primitive_sweep(args)
     if args.probe_contraction:
         import torch
         import paper_2406_17823_b200 as Q
