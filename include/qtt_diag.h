@@ -18,7 +18,7 @@ int qtt_diag_gemm(void* stream, const double* A_dev, const double* B_dev, double
  * k*ld, DESTROYED unless small); R_i = L_i^T (k x k upper triangular, row-major, consecutive) with Y = L Q.
  * Matrices whose slices fit a cluster's shared memory go through the cluster-resident Householder kernel (and
  * are left alone), larger ones through the blocked panel + DMMA trailing-update path.
- * scratch_dev: batch * 3 * 16 * m doubles.  SURVEY.md section 8 row a4. */
+ * scratch_dev: batch * 3 * 64 * m doubles.  SURVEY.md section 8 row a4. */
 int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, double* R_dev, double* scratch_dev);
 
 /* One-sided Jacobi on the rows of `batch` matrices X_i (p x q, ld, stride p*ld), in place: rows of the result

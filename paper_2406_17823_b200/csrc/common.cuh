@@ -51,9 +51,9 @@ cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream, i
 struct LqProb {
   double* Y;
   int k, m, ld;
-  double* V;   // scratch  nb x m : clean reflector rows of the current panel
-  double* TV;  // scratch  nb x m : T * V of the current panel
-  double* W;   // scratch  nb x m : (rows below the panel) x nb product Y2 V^T of the trailing update
+  double* V;   // scratch  64 x m : clean reflector rows of the current super-panel (4 sub-panels of 16 rows)
+  double* TV;  // scratch  64 x m : T_agg * V_agg of the current super-panel
+  double* W;   // scratch  64 x m : products X V^T of the trailing updates and their K-chunk partials
 };
 #define QTT_LQ_MAX_BATCH 16
 #define QTT_LQ_NB 16

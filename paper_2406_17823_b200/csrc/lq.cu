@@ -200,13 +200,6 @@ __global__ void __launch_bounds__(PANEL_NT) qtt_lq_panel_kernel(const __grid_con
   }
 }
 
-// Problems that still have rows below the current panel (their trailing update is done by grouped GEMMs).
-
-struct UpdGroup {
-  int nprob, p0;
-  LqProb p[QTT_LQ_MAX_BATCH];
-};
-
 // W[0..n) <- sum_z W[z * n + ..): the K-chunks of the skinny first product of the trailing update, fixed order
 struct SumProb { double* W; int n, Z; };
 struct SumGroup { int nprob; SumProb p[QTT_LQ_MAX_BATCH]; };
@@ -246,8 +239,98 @@ int pick_cluster(int mw) {
 
 }  // namespace
 
-size_t qtt_lq_scratch_doubles(int m) { return (size_t)NB * m; }
 
+namespace {
+
+// One target of a compact-WY update  X <- X - (X V^T)(TV)  over the columns [col0, m):  X is rows x mw (ld), V and TV
+// are nv x mw (leading dimension m), W is scratch for the rows x nv product and its K-chunk partials.
+struct UpdTarget {
+  double* X;
+  i64 ld;
+  int rows;
+  const double* V;
+  const double* TV;
+  int m, nv, mw;
+  double* W;
+  i64 wcap;  // doubles available at W
+};
+
+// Grouped DMMA GEMMs.  The first product is skinny (nv <= 64 columns) with a long contraction (the row length): it
+// is cut into up to 8 K-chunks (one GEMM problem each, so that enough CTAs work on it), whose partial results a small
+// kernel adds up in a fixed order.
+cudaError_t apply_updates(const std::vector<UpdTarget>& ts, cudaStream_t stream) {
+  if (ts.empty()) return cudaSuccess;
+  std::vector<GemmProb> g1, g2;
+  std::vector<SumProb> sums;
+  for (const UpdTarget& t : ts) {
+    if (t.rows <= 0 || t.nv <= 0 || t.mw <= 0) continue;
+    int Z = t.mw / 512;
+    Z = Z > 8 ? 8 : Z;
+    const i64 per = (i64)t.rows * t.nv;
+    if ((i64)Z * per > t.wcap) Z = (int)(t.wcap / per);
+    Z = Z < 1 ? 1 : Z;
+    int chunk = (t.mw + Z - 1) / Z;
+    chunk = (chunk + 15) & ~15;
+    int zused = 0;
+    for (int z = 0; z < Z; ++z) {
+      const int k0 = z * chunk, kz = (t.mw - k0 < chunk) ? t.mw - k0 : chunk;
+      if (kz <= 0) break;
+      GemmProb a;
+      memset(&a, 0, sizeof(a));
+      a.nbatch = 1;
+      a.alpha = 1.0; a.beta = 0.0;
+      a.A = t.X + k0; a.a_lo = t.ld; a.a_k = 1;
+      a.B = t.V + k0; a.b_k = 1; a.b_n = t.m;
+      a.C = t.W + (i64)z * per; a.c_lo = t.nv; a.c_n = 1;
+      a.M = t.rows; a.N = t.nv; a.K = kz;
+      g1.push_back(a);
+      ++zused;
+    }
+    sums.push_back(SumProb{t.W, (int)per, zused});
+    GemmProb b;
+    memset(&b, 0, sizeof(b));
+    b.nbatch = 1;
+    b.alpha = -1.0; b.beta = 1.0;
+    b.A = t.W; b.a_lo = t.nv; b.a_k = 1;
+    b.B = t.TV; b.b_k = t.m; b.b_n = 1;
+    b.C = t.X; b.c_lo = t.ld; b.c_n = 1;
+    b.M = t.rows; b.N = t.mw; b.K = t.nv;
+    g2.push_back(b);
+  }
+  if (g2.empty()) return cudaSuccess;
+  QTT_CHECK_CUDA(qtt_launch_gemm(g1.data(), (int)g1.size(), stream, QK_LQ_UPDATE));
+  for (size_t s0 = 0; s0 < sums.size(); s0 += QTT_LQ_MAX_BATCH) {
+    SumGroup sg;
+    sg.nprob = 0;
+    bool any = false;
+    int nmax = 0;
+    for (size_t i = s0; i < sums.size() && sg.nprob < QTT_LQ_MAX_BATCH; ++i) {
+      sg.p[sg.nprob++] = sums[i];
+      any = any || sums[i].Z > 1;
+      nmax = sums[i].n > nmax ? sums[i].n : nmax;
+    }
+    if (any) {
+      QttProf prof(QK_LQ_UPDATE, stream, 0.0, 0, 0, sg.nprob, -1);
+      qtt_sum_partials_kernel<<<dim3((nmax + 255) / 256, sg.nprob), 256, 0, stream>>>(sg);
+      QTT_CHECK_CUDA(cudaGetLastError());
+    }
+  }
+  return qtt_launch_gemm(g2.data(), (int)g2.size(), stream, QK_LQ_UPDATE);
+}
+
+constexpr int NS_MAX = 4;          // sub-panels per super-panel (scratch is sized for this)
+constexpr int SP_MAX = NS_MAX * NB;
+
+}  // namespace
+
+size_t qtt_lq_scratch_doubles(int m) { return (size_t)SP_MAX * m; }
+
+// Two-level blocking.  A super-panel is 4 sub-panels of 16 rows.  After each sub-panel (panel kernel: reflector rows
+// V_s and T_s V_s) only the rest of the super-panel is updated -- and the rows A = T_agg V_agg accumulated so far, which
+// transform exactly like trailing rows: (I - V_1..k^T A_k)(I - V_{k+1}^T TV_{k+1}) = I - V_1..k+1^T [A_k Q_{k+1}; TV_{k+1}].
+// The rows below the super-panel then get ONE update with 64 reflectors, so the big trailing matrix (0.5 GB per operand
+// at chi = 128: HBM-bound) is streamed once per 64 rows instead of once per 16.  Batches that fit the L2 (config 3: 67 MB)
+// keep one-level blocking: there the extra small updates cost more than the saved passes.
 cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
   static bool attr_done = false;
   if (!attr_done) {
@@ -256,127 +339,87 @@ cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
     attr_done = true;
   }
   for (int b0 = 0; b0 < n; b0 += QTT_LQ_MAX_BATCH) {
-    int nb = n - b0 < QTT_LQ_MAX_BATCH ? n - b0 : QTT_LQ_MAX_BATCH;
+    const int nb = n - b0 < QTT_LQ_MAX_BATCH ? n - b0 : QTT_LQ_MAX_BATCH;
     int kmax = 0;
+    double bytes = 0.0;
     for (int i = 0; i < nb; ++i) {
       if (probs[b0 + i].k > probs[b0 + i].m) return cudaErrorInvalidValue;
       kmax = probs[b0 + i].k > kmax ? probs[b0 + i].k : kmax;
+      bytes += (double)probs[b0 + i].k * probs[b0 + i].m * sizeof(double);
     }
-    for (int p0 = 0; p0 < kmax; p0 += NB) {
-      LqGroup grp;
-      UpdGroup ug;
-      grp.nprob = 0;
-      grp.p0 = p0;
-      ug.nprob = 0;
-      ug.p0 = p0;
-      int mwmax = 0, ctas = 0;
+    const int NS = bytes > 96e6 ? NS_MAX : 1;
+    const int SP = NS * NB;
+    for (int P0 = 0; P0 < kmax; P0 += SP) {
+      // the reflector rows of a sub-panel start at its own first column: zero what lies before it inside the super-panel
+      for (int i = 0; i < nb && NS > 1; ++i) {
+        const LqProb& p = probs[b0 + i];
+        if (p.k <= P0) continue;
+        const size_t wbytes = (size_t)((p.m - P0 < SP) ? p.m - P0 : SP) * sizeof(double);
+        QTT_CHECK_CUDA(cudaMemset2DAsync(p.V + P0, (size_t)p.m * sizeof(double), 0, wbytes, SP, stream));
+        QTT_CHECK_CUDA(cudaMemset2DAsync(p.TV + P0, (size_t)p.m * sizeof(double), 0, wbytes, SP, stream));
+      }
+      for (int s = 0; s < NS; ++s) {
+        const int p0 = P0 + s * NB;
+        if (p0 >= kmax) break;
+        LqGroup grp;
+        grp.nprob = 0;
+        grp.p0 = p0;
+        int mwmax = 0;
+        std::vector<UpdTarget> small;
+        double fp = 0.0;
+        for (int i = 0; i < nb; ++i) {
+          const LqProb& p = probs[b0 + i];
+          if (p.k <= p0) continue;
+          LqProb q = p;
+          q.V = p.V + (size_t)s * NB * p.m;
+          q.TV = p.TV + (size_t)s * NB * p.m;
+          grp.p[grp.nprob++] = q;
+          const int mw = p.m - p0, nbp = (p.k - p0 < NB) ? p.k - p0 : NB;
+          mwmax = mw > mwmax ? mw : mwmax;
+          fp += 2.0 * nbp * nbp * (double)mw;
+          const int pend = (P0 + SP < p.k) ? P0 + SP : p.k;
+          const int r0 = p0 + nbp;
+          const i64 half = (i64)SP_MAX * p.m / 2;
+          if (pend > r0)  // the rest of the super-panel
+            small.push_back(UpdTarget{p.Y + (i64)r0 * p.ld + p0, p.ld, pend - r0, q.V + p0, q.TV + p0, p.m, nbp, mw, p.W, half});
+          if (s > 0 && p.k > pend)  // the accumulated T V rows (only needed if rows remain below the super-panel)
+            small.push_back(UpdTarget{p.TV + p0, p.m, s * NB, q.V + p0, q.TV + p0, p.m, nbp, mw, p.W + half, half});
+        }
+        if (grp.nprob == 0) break;
+        const int C = pick_cluster(mwmax);
+        int w = (mwmax + C - 1) / C;
+        w = (w + 1) & ~1;
+        const int wp = w + 1;
+        const size_t smem = panel_smem_doubles(wp) * sizeof(double);
+        if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(C * grp.nprob);
+        cfg.blockDim = dim3(PANEL_NT);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = C;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        {
+          QttProf prof(QK_LQ_PANEL, stream, fp, grp.p[0].k, grp.p[0].m, grp.nprob, p0);
+          QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
+        }
+        QTT_CHECK_CUDA(apply_updates(small, stream));
+      }
+      // ---- the rows below the super-panel: one update with all its reflectors
+      std::vector<UpdTarget> big;
       for (int i = 0; i < nb; ++i) {
         const LqProb& p = probs[b0 + i];
-        if (p.k <= p0) continue;
-        grp.p[grp.nprob++] = p;
-        mwmax = (p.m - p0) > mwmax ? (p.m - p0) : mwmax;
-        int rem = p.k - (p0 + (p.k - p0 < NB ? p.k - p0 : NB));
-        if (rem > 0) {
-          ug.p[ug.nprob++] = p;
-          ctas += 1;
-        }
+        const int pend = (P0 + SP < p.k) ? P0 + SP : p.k;
+        if (p.k <= P0 || p.k <= pend) continue;
+        big.push_back(UpdTarget{p.Y + (i64)pend * p.ld + P0, p.ld, p.k - pend, p.V + P0, p.TV + P0, p.m, pend - P0, p.m - P0,
+                                p.W, (i64)SP_MAX * p.m});
       }
-      if (grp.nprob == 0) break;
-      int C = pick_cluster(mwmax);
-      int w = (mwmax + C - 1) / C;
-      w = (w + 1) & ~1;
-      int wp = w + 1;
-      size_t smem = panel_smem_doubles(wp) * sizeof(double);
-      if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3(C * grp.nprob);
-      cfg.blockDim = dim3(PANEL_NT);
-      cfg.dynamicSmemBytes = smem;
-      cfg.stream = stream;
-      cudaLaunchAttribute at[1];
-      at[0].id = cudaLaunchAttributeClusterDimension;
-      at[0].val.clusterDim.x = C;
-      at[0].val.clusterDim.y = 1;
-      at[0].val.clusterDim.z = 1;
-      cfg.attrs = at;
-      cfg.numAttrs = 1;
-      // Householder count of this panel step: panel 2 nb^2 mw, trailing update 4 nb mw rows_below
-      double fp = 0.0, fu = 0.0;
-      for (int i = 0; i < grp.nprob; ++i) {
-        const double mw = grp.p[i].m - p0, nbp = (grp.p[i].k - p0 < NB) ? grp.p[i].k - p0 : NB;
-        fp += 2.0 * nbp * nbp * mw;
-        fu += 4.0 * nbp * mw * (grp.p[i].k - p0 - nbp);
-      }
-      {
-        QttProf prof(QK_LQ_PANEL, stream, fp, grp.p[0].k, grp.p[0].m, grp.nprob, p0);
-        QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_lq_panel_kernel, grp, wp));
-      }
-      if (ctas > 0) {
-        // trailing update of the rows below the panel, Y2 <- Y2 - (Y2 V^T)(T V), as grouped DMMA GEMMs.  The first
-        // product is skinny (16 columns) with a long contraction (the row length): it is cut into up to 8 K-chunks
-        // (one GEMM problem each, so that enough CTAs work on it), whose partial results a small kernel adds up in
-        // a fixed order.
-        std::vector<GemmProb> g1;
-        GemmProb g2[QTT_LQ_MAX_BATCH];
-        SumGroup sg;
-        sg.nprob = 0;
-        for (int i = 0; i < ug.nprob; ++i) {
-          const LqProb& p = ug.p[i];
-          const int nbp = (p.k - p0 < NB) ? p.k - p0 : NB;
-          const int r0 = p0 + nbp, rem = p.k - r0, mw = p.m - p0;
-          int Z = mw / 512;
-          Z = Z > 8 ? 8 : Z;
-          if (Z > p.m / rem) Z = p.m / rem;  // the partials live in the NB x m scratch W
-          Z = Z < 1 ? 1 : Z;
-          int chunk = (mw + Z - 1) / Z;
-          chunk = (chunk + 15) & ~15;
-          for (int z = 0; z < Z; ++z) {
-            const int k0 = z * chunk, kz = (mw - k0 < chunk) ? mw - k0 : chunk;
-            GemmProb a;
-            memset(&a, 0, sizeof(a));
-            a.nbatch = 1;
-            a.alpha = 1.0; a.beta = 0.0;
-            a.A = p.Y + (i64)r0 * p.ld + p0 + k0; a.a_lo = p.ld; a.a_k = 1;
-            a.B = p.V + p0 + k0; a.b_k = 1; a.b_n = p.m;
-            a.C = p.W + (i64)z * rem * NB; a.c_lo = NB; a.c_n = 1;
-            a.M = rem; a.N = nbp; a.K = kz > 0 ? kz : 0;
-            if (a.K > 0) g1.push_back(a);
-            else {  // (cannot happen with chunk >= 16, kept for safety: an empty chunk contributes zeros)
-              Z = z;
-              break;
-            }
-          }
-          sg.p[sg.nprob].W = p.W;
-          sg.p[sg.nprob].n = rem * NB;
-          sg.p[sg.nprob].Z = Z;
-          ++sg.nprob;
-          GemmProb b;
-          memset(&b, 0, sizeof(b));
-          b.nbatch = 1;
-          b.alpha = -1.0; b.beta = 1.0;
-          b.A = p.W; b.a_lo = NB; b.a_k = 1;
-          b.B = p.TV + p0; b.b_k = p.m; b.b_n = 1;
-          b.C = p.Y + (i64)r0 * p.ld + p0; b.c_lo = p.ld; b.c_n = 1;
-          b.M = rem; b.N = mw; b.K = nbp;
-          g2[i] = b;
-        }
-        QTT_CHECK_CUDA(qtt_launch_gemm(g1.data(), (int)g1.size(), stream, QK_LQ_UPDATE));
-        {
-          bool any = false;
-          int nmax = 0;
-          for (int i = 0; i < sg.nprob; ++i) {
-            any = any || sg.p[i].Z > 1;
-            nmax = sg.p[i].n > nmax ? sg.p[i].n : nmax;
-          }
-          if (any) {
-            QttProf prof(QK_LQ_UPDATE, stream, 0.0, 0, 0, sg.nprob, -1);
-            qtt_sum_partials_kernel<<<dim3((nmax + 255) / 256, sg.nprob), 256, 0, stream>>>(sg);
-            QTT_CHECK_CUDA(cudaGetLastError());
-          }
-        }
-        QTT_CHECK_CUDA(qtt_launch_gemm(g2, ug.nprob, stream, QK_LQ_UPDATE));
-        (void)fu;
-      }
+      QTT_CHECK_CUDA(apply_updates(big, stream));
     }
   }
   return cudaSuccess;

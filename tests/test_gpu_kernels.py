@@ -80,7 +80,8 @@ def test_gemm_odd_leading_dimensions(env):
 
 
 LQ_CASES = [(4, 4, 1), (12, 16, 2), (16, 48, 3), (48, 64, 1), (192, 768, 2), (100, 333, 2), (320, 1280, 1),
-            (64, 4096, 2), (256, 9000, 1)]
+            (64, 4096, 2), (256, 9000, 1),
+            (500, 8192, 3)]  # > 96 MB per batch: the two-level (64-row super-panel) blocking
 
 
 @pytest.mark.parametrize("k,m,batch", LQ_CASES)
@@ -92,7 +93,7 @@ def test_lq_triangular_factor(env, k, m, batch):
     Y = rng.standard_normal((batch, k, m))
     dY = dev(torch, Y)
     dR = torch.zeros((batch, k, k), dtype=torch.float64, device="cuda")
-    scratch = torch.zeros(batch * 3 * 16 * m, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(batch * 3 * 64 * m, dtype=torch.float64, device="cuda")
     torch.cuda.synchronize()
     st = lib.qtt_diag_lq(C.c_void_p(stream.cuda_stream), ptr(dY), batch, k, m, m, ptr(dR), ptr(scratch))
     assert st == 0
@@ -114,7 +115,7 @@ def test_lq_rank_deficient(env):
     Y[10] = 0.0
     dY = dev(torch, Y)
     dR = torch.zeros((k, k), dtype=torch.float64, device="cuda")
-    scratch = torch.zeros(3 * 16 * m, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(3 * 64 * m, dtype=torch.float64, device="cuda")
     torch.cuda.synchronize()
     assert lib.qtt_diag_lq(C.c_void_p(stream.cuda_stream), ptr(dY), 1, k, m, m, ptr(dR), ptr(scratch)) == 0
     stream.synchronize()
