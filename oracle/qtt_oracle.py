@@ -42,11 +42,12 @@ analytic finite-difference of sin/cos, bond-2 closed forms, the root-sum-square
 truncation identity, norm preservation, dense TT-SVD, dense RK4 of the same
 stencils.
 
-Parity-pin status: O1-O6, O8-O11 pinned.  O7 is pinned where chi_work >= every
-intermediate rank (then it equals O6 applied to O4, checked against dense brute
-force) and by its error bound; for a finite chi_work that really truncates, the
-result is DEFINED by the step-by-step algorithm below (the paper gives none) --
-"parity unpinned" for that regime beyond the error bound.
+Parity-pin status: O1-O11 pinned.  O7 with a working bond that really truncates is algorithm-defined
+(reading 8), and each of its steps is pinned in tests/test_oracle_zipup_pins.py: per site Q^T Q = I,
+R' = Q^T T, ||T - Q R'||_F = the tail of an independent svdvals(T) beyond keep = min(chi_work, rows, cols)
+(Eckart-Young), T_l = (Phi_{<l}^T (x) I_4) X_l with X_l from the explicit hadamard() cores, a planted spectrum
+with a gap at chi_work, and the projected dense product as the state handed to the R->L sweep; the eps rank
+rule by hand-computed tails, brute-force minimality and a case where the 1/sqrt(n-1) split decides the rank.
 """
 from __future__ import annotations
 
@@ -266,6 +267,7 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
     n = len(A)
     R = np.ones((1, 1, 1))
     cores = []
+    zip_log = []  # per site: the matrix T that was factorised, Q, R' and the branch taken (read by the pins only)
     for l in range(n - 1):
         T4 = np.einsum("rab,awc,bwd->rwcd", R, A[l], B[l], optimize=True)
         r, d, a2, b2 = T4.shape
@@ -274,18 +276,25 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
         if m <= min(k, chi_work):
             Q = np.eye(m)
             Rn = T
+            branch = "identity"
         elif k < m and k <= chi_work:
             Q, Rn = np.linalg.qr(T)
+            branch = "qr"
         else:
             U, s, Vt = np.linalg.svd(T, full_matrices=False)
             keep = min(chi_work, len(s))
             Q = U[:, :keep]
             Rn = s[:keep, None] * Vt[:keep]
+            branch = "svd"
+        zip_log.append(dict(T=T, Q=Q, R=Rn, branch=branch))
         rn = Q.shape[1]
         cores.append(Q.reshape(r, d, rn))
         R = Rn.reshape(rn, a2, b2)
     T4 = np.einsum("rab,awc,bwd->rwcd", R, A[n - 1], B[n - 1], optimize=True)
     cores.append(T4.reshape(T4.shape[0], D_PHYS, 1))
+    if info is not None:
+        info["zip"] = zip_log
+        info["zip_cores"] = [c.copy() for c in cores]  # Q_1..Q_{n-1}, T_n: the state the R->L sweep starts from
     return _sweep_rl(cores, chi_max, eps, info)
 
 
