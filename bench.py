@@ -98,10 +98,10 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------- CPU oracle leg
-def oracle_sample_seconds(cfg: int, state=None):
-    """Times a bounded sample of one RK4 step with the oracle as it stands: ONE of the four rhs evaluations
-    (6 apply+round, 4 hadamard+round, 2 three-term sums) plus ONE of the four stage combinations, and
-    extrapolates one step as 4 x that sample.  Returns (seconds per extrapolated step, description, state)."""
+def oracle_step_seconds(cfg: int, state=None):
+    """Times ONE WHOLE RK4 step of the oracle as it stands (4 rhs evaluations, 3 stage combinations, the final 5-term
+    sum: 56 roundings) on the host cores.  Returns (seconds, description, state); the next call continues from the
+    state this step produced."""
     from oracle import qtt_oracle as O
     c, _ = workload(cfg)
     n, chi = c["n"], c["chi"]
@@ -110,13 +110,10 @@ def oracle_sample_seconds(cfg: int, state=None):
         dx = 1.0 / (1 << n)
         state = dict(U=[O.from_dense(ux, chi), O.from_dense(uy, chi)], Dx=O.mpo_d1(n, dx), Dy=O.mpo_d2(n, dx),
                      Lap=O.mpo_laplacian(n, dx))
-    U = state["U"]
     t0 = time.perf_counter()
-    k1 = O.rhs(U, state["Dx"], state["Dy"], state["Lap"], c["Re"], chi, skew=SKEW)
-    U2 = [O.round_mps(O.lincomb([(1.0, U[i]), (c["dt"] / 2, k1[i])]), chi) for i in range(2)]
+    state["U"] = O.rk4_step(state["U"], state["Dx"], state["Dy"], state["Lap"], c["Re"], c["dt"], chi, skew=SKEW)
     t = time.perf_counter() - t0
-    state["U"] = U2  # the next sample continues from the half-step state
-    return 4.0 * t, "1 of the 4 rhs evaluations + 1 of the 4 stage combinations of one RK4 step, x4", state
+    return t, "one whole oracle RK4 step per timed step (no extrapolation)", state
 
 
 def blas_threads():
@@ -133,12 +130,15 @@ def run_reference(args):
         return 0
     c, desc = workload(args.config)
     state = None
-    for _ in range(args.warmup):
-        _, _, state = oracle_sample_seconds(args.config, state)
+    # a CPU program needs no warm-up beyond the first touch of its BLAS threads: at most ONE untimed whole step, so
+    # that the run (K + 1 whole oracle steps, ~19 s each at config 3 on 16 cores) stays within minutes
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
+        _, _, state = oracle_step_seconds(args.config, state)
     tot, sample = 0.0, ""
     for _ in range(args.steps):
-        s, sample, state = oracle_sample_seconds(args.config, state)
-        tot += s
+        sec1, sample, state = oracle_step_seconds(args.config, state)
+        tot += sec1
     sec = tot / max(args.steps, 1)
     val = 1.0 / sec
     cores = blas_threads()
@@ -146,8 +146,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRICS[args.config], "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": desc, "note": "CPU oracle (NumPy fp64 + LAPACK) on the host cores; each step is a "
-                   "bounded sample extrapolated to one RK4 step"},
+        "config": {"workload": desc, "note": "CPU oracle (NumPy fp64 + LAPACK) on the host cores; every timed step is one "
+                   f"WHOLE oracle RK4 step (free-running trajectory); untimed warm-up steps run: {warm}"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -176,6 +176,95 @@ def max_over_ranks(value: float, world: int, device: str = "cuda") -> float:
 def whole_job_value(world: int, steps: int, ms_max: float) -> float:
     """steps/s summed over all replicas: every rank did `steps` steps within the slowest rank's time."""
     return world * steps / (ms_max * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------- algorithmic work model
+def _bond_profile(n, chi):
+    return [1] + [min(4 ** l, 4 ** (n - l), chi) for l in range(1, n)] + [1]
+
+
+def _svd_nominal(a, b):
+    a, b = max(a, b), min(a, b)
+    return 6.0 * a * b * b + 20.0 * b ** 3
+
+
+def _round_dense_work(r, chi, D=1):
+    """SURVEY.md section 8(d) per-site formulas for round(dense MPS with bonds r): (GEMM-shaped flops, QR flops, nominal
+    SVD flops, algorithmic bytes = operand cores read once + rounded cores written once)."""
+    n = len(r) - 1
+    p = [1] * (n + 1)
+    for k in range(1, n + 1):
+        p[k] = min(4 * p[k - 1], r[k])
+    out = [1] * (n + 1)
+    for k in range(n - 1, 0, -1):
+        out[k] = max(1, min(chi, p[k], 4 * out[k + 1]))
+    g = q = sv = 0.0
+    for l in range(1, n):                      # L->R: thin QR of (4 p_{l-1}) x r_l, carry R into the next core
+        m, k = 4 * p[l - 1], r[l]
+        if m > k:
+            q += 4.0 * m * k * k - (4.0 / 3.0) * k ** 3
+        if m > k or l > 1:
+            g += 2.0 * p[l] * r[l] * 4 * r[l + 1] / D
+    for l in range(n, 1, -1):                  # R->L: SVD of p_{l-1} x (4 r'_l), absorb U S into the left neighbour
+        sv += _svd_nominal(p[l - 1], 4 * out[l])
+        g += 2.0 * 4 * p[l - 2] * p[l - 1] * out[l - 1]
+    byts = 8.0 * (sum(r[k] * 4 * r[k + 1] for k in range(n)) / (D * D if D > 1 else 1) * (1 + D * D if D > 1 else 1)
+                  + sum(out[k] * 4 * out[k + 1] for k in range(n)))
+    return g, q, sv, byts
+
+
+def _zip_work(ra, rb, chi, cw):
+    """The same for the fused Hadamard + round (zip-up with working bond cw)."""
+    n = len(ra) - 1
+    rw = [1] * (n + 1)
+    for k in range(1, n):
+        rw[k] = min(4 * rw[k - 1], ra[k] * rb[k], cw)
+    out = [1] * (n + 1)
+    for k in range(n - 1, 0, -1):
+        out[k] = max(1, min(chi, rw[k], 4 * out[k + 1]))
+    g = q = sv = 0.0
+    byts = 8.0 * (sum(ra[k] * 4 * ra[k + 1] + rb[k] * 4 * rb[k + 1] for k in range(n))
+                  + sum(out[k] * 4 * out[k + 1] for k in range(n)))
+    for l in range(1, n + 1):
+        r, pa, pb, qa, qb = rw[l - 1], ra[l - 1], rb[l - 1], ra[l], rb[l]
+        g += 8.0 * r * pa * pb * qa + 8.0 * r * qa * pb * qb        # row a2, two GEMM passes
+        byts += 2 * 8.0 * 4 * r * qa * qb                            # T written once, read once
+        if l == n:
+            break
+        m, k = 4 * r, qa * qb
+        if m <= min(k, cw):
+            continue
+        keep = min(m, k, cw)
+        q += float(m) * m * k                                        # Gram-equivalent count of the (4r) x (ab) factorisation
+        sv += _svd_nominal(m, min(m, k))
+        g += 2.0 * keep * m * k                                      # carry R' = Q^T T
+    for l in range(n, 1, -1):
+        sv += _svd_nominal(rw[l - 1], 4 * out[l])
+        g += 2.0 * 4 * rw[l - 2] * rw[l - 1] * out[l - 1]
+    return g, q, sv, byts
+
+
+def step_work_model(n, chi, cw=None, skew=False):
+    """Algorithmic work of ONE qtt_rk4_step from SURVEY.md section 8(d)'s per-site formulas:
+    per rhs 4 apply(D=3)+round, 2 apply(D=5)+round, 4 zip-ups, 2 three-term sums (skew: 7 zip-ups, 8 applies(D=3),
+    2 five-term sums); 3 two-term stage sums x2 and one five-term sum x2.  Returns flops split and bytes."""
+    cw = cw or 2 * chi
+    r = _bond_profile(n, chi)
+    mul = lambda D: [D * x if 0 < i < n else x for i, x in enumerate(r)]
+    parts = {"apply3": _round_dense_work(mul(3), chi, 3), "apply5": _round_dense_work(mul(5), chi, 5),
+             "had": _zip_work(r, r, chi, cw), "sum2": _round_dense_work(mul(2), chi),
+             "sum3": _round_dense_work(mul(3), chi), "sum5": _round_dense_work(mul(5), chi)}
+    if skew:
+        counts = {"apply3": 32, "apply5": 8, "had": 28, "sum2": 6, "sum3": 0, "sum5": 8 + 2}
+    else:
+        counts = {"apply3": 16, "apply5": 8, "had": 16, "sum2": 6, "sum3": 8, "sum5": 2}
+    G = sum(parts[k][0] * counts[k] for k in parts)
+    Qf = sum(parts[k][1] * counts[k] for k in parts)
+    S = sum(parts[k][2] * counts[k] for k in parts)
+    B = sum(parts[k][3] * counts[k] for k in parts)
+    return {"flops": G + Qf + S, "gemm_shaped_flops": G, "qr_flops": Qf, "svd_nominal_flops": S,
+            "rounding_sweep_bytes": B,
+            "per_primitive_gflop": {k: sum(v[:3]) * 1e-9 for k, v in parts.items()}, "counts": counts}
 
 
 # ------------------------------------------------------------------------------------------- our arm
@@ -239,6 +328,15 @@ def run_ours(args):
             e1.record(ctx.stream)
     barrier()
     clocks = sampler.stop()
+    # what was timed must be a converged, finite computation: no Jacobi SVD hit its sweep limit, norms are finite
+    max_sweeps, limit_hits = Q.qtt_ctx_jacobi_stats(ctx)
+    norms = [Q.qtt_mps_norm(ctx, x) for x in u]
+    if limit_hits != 0 or not all(np.isfinite(v) and v > 0 for v in norms):
+        raise RuntimeError(f"timed steps are invalid: jacobi limit hits {limit_hits}, norms {norms}")
+    validation = {"jacobi_max_sweeps": int(max_sweeps), "jacobi_limit_hits": int(limit_hits),
+                  "norms_after_timed_steps": [float(v) for v in norms],
+                  "parity": "tests/test_gpu_parity.py compares this launch configuration with the oracle (config 3: "
+                            "steps 1-3; config 4: one full step against tests/golden/cfg4_step1.npz)"}
     ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
     launches = Q.qtt_ctx_launch_count(ctx) - launches0
     ms = max_over_ranks(ms, world)
@@ -270,7 +368,7 @@ def run_ours(args):
         "config": {"workload": desc, "l2": "256 MiB buffer zeroed between timed steps, outside the per-step CUDA "
                    "event pairs; ms_per_step = sum of the per-step event times / steps",
                    "graph": "whole RK4 step replayed as one CUDA graph", "parallelism": "replicas only"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "validation": validation,
     }
     if rank == 0:
         line.update(roofline_and_baseline(Q, ctx, u, (Dx, Dy, Lap), c, chi, args, ms_per_step))
@@ -281,9 +379,20 @@ def run_ours(args):
     return 0
 
 
-# dram bytes (read + write) per launch from the committed ncu --set full captures (profiles/), keyed by
-# (family, launch shape tag of qtt_diag_profile_dump)
-NCU_TRAFFIC_BYTES = {("rowjacobi", (512, 512, 4, 16)): 8.43e6}
+def ncu_traffic_table():
+    """dram bytes (read + write) per launch from the committed ncu --set full captures: profiles/ncu_traffic.csv, lines
+    `family,d0,d1,d2,d3,dram_bytes_per_launch,source` keyed by the launch shape tag of qtt_diag_profile_dump."""
+    out = {}
+    try:
+        for ln in open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")).read().splitlines()[1:]:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 7 and f[0] and not f[0].startswith("#"):
+                out[(f[0], tuple(int(x) for x in f[1:5]))] = (float(f[5]), f[6])
+    except (OSError, ValueError):
+        pass
+    return out
+
+
 KERNEL_NAMES = {"rowjacobi": "qtt_blockjacobi_kernel", "qrcp": "qtt_qrcp_reg_kernel", "gemm": "qtt_gemm_dmma_kernel",
                 "lq_panel": "qtt_lq_panel_kernel / qtt_qrcp_kernel", "lq_update": "qtt_gemm_dmma_kernel",
                 "select": "qtt_select_kernel", "move": "movement kernels"}
@@ -448,7 +557,7 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
                "no fp64 figure; nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2 TFLOP/s, DESIGN.md section 6)")
         achieved = k["work"] / (k["ms"] * 1e-3) * 1e-12
         unit = "TFLOP/s"
-    traffic = NCU_TRAFFIC_BYTES.get((dom, shape))
+    traffic, traffic_src = ncu_traffic_table().get((dom, shape), (None, None))
     roof = {"kernel": KERNEL_NAMES.get(dom, dom) + (f" launch shape (d0,d1,d2,d3)={shape}" if shape else ""),
             "bound": bound, "achieved": achieved, "peak": peak, "unit": unit,
             "frac": achieved / peak if peak else None, "traffic": traffic, "peak_source": src,
@@ -456,15 +565,52 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
             "share_of_step_kernel_time": k["ms"] / tot_ms, "family_share_of_step_kernel_time": d["ms"] / tot_ms,
             "algorithmic_work": "nominal SVD count 6ab^2+20b^3 per matrix (DESIGN.md section 6)" if dom == "rowjacobi"
             else "DESIGN.md section 6 per-family formulas",
-            "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
-            "launch shape (profiles/r1_blockjacobi_full.md)" if traffic else None}
+            "traffic_source": ("dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
+                               "launch shape (profiles/ncu_traffic.csv: " + traffic_src + ")") if traffic else None}
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        hbm_peak, hbm_src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
+    fam_bound = {"gemm": "tensor", "lq_panel": "alu", "lq_update": "tensor", "rowjacobi": "alu", "select": "hbm",
+                 "move": "hbm", "qrcp": "alu"}
+    for kf, v in fams.items():
+        sec = max(v["ms_per_step"] * 1e-3, 1e-12)
+        if fam_bound[kf] == "hbm":
+            v.update(bound="hbm", achieved=v["work_per_step"] / sec * 1e-9, peak=hbm_peak, unit="GB/s")
+        else:
+            pk = peaks["dmma"] if fam_bound[kf] == "tensor" else peaks["dfma"]
+            v.update(bound=fam_bound[kf], achieved=v["work_per_step"] / sec * 1e-12, peak=pk, unit="TFLOP/s")
+        v["frac"] = v["achieved"] / v["peak"] if v["peak"] else None
+    model = step_work_model(c["n"], chi, skew=SKEW)
+    step_sec = ms_per_step * 1e-3
+    sweep_fams = ("lq_panel", "lq_update", "rowjacobi", "select", "move", "qrcp")
+    sweep_sec = sum(fams[kf]["ms_per_step"] for kf in sweep_fams) * 1e-3
+    roofline_step = {
+        "bound": "tensor", "achieved": model["flops"] / step_sec * 1e-12, "peak": peaks["dmma"], "unit": "TFLOP/s",
+        "frac": (model["flops"] / step_sec * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,
+        "algorithmic_gflop_per_step": model["flops"] * 1e-9, "gemm_shaped_share": model["gemm_shaped_flops"] / model["flops"],
+        "qr_gflop": model["qr_flops"] * 1e-9, "svd_nominal_gflop": model["svd_nominal_flops"] * 1e-9,
+        "per_primitive_gflop": model["per_primitive_gflop"], "primitive_counts_per_step": model["counts"],
+        "ms_per_step": ms_per_step,
+        "what": "SURVEY.md section 8(d) per-site formulas (contraction + carry + absorb GEMMs, QR 4mk^2-4k^3/3, Gram-equivalent "
+                "m^2 k of the zip-up factorisation, nominal SVD 6ab^2+20b^3) summed over one step / graph-replayed step time "
+                "/ measured DMMA issue rate (fp64 tensor peak == fp64 FMA peak on this part)",
+        "rounding_sweep": {"bound": "hbm", "achieved": model["rounding_sweep_bytes"] / max(sweep_sec, 1e-12) * 1e-9,
+                           "peak": hbm_peak, "unit": "GB/s",
+                           "frac": model["rounding_sweep_bytes"] / max(sweep_sec, 1e-12) * 1e-9 / hbm_peak,
+                           "algorithmic_mbytes_per_step": model["rounding_sweep_bytes"] * 1e-6,
+                           "kernel_ms_per_step": sweep_sec * 1e3, "peak_source": hbm_src,
+                           "what": "operand cores read once + rounded cores written once (+ zip-up T written and read once) "
+                                   "over the summed kernel time of the non-GEMM families; the working set of this config is "
+                                   "L2-resident, so the HBM fraction is low by construction (SURVEY.md section 8d)"}}
     g = rep["gemm"]
     # the Hadamard site contractions proper at the bulk sites of this workload:
     # pass 1 (4 chi x chi x chi, batched over the working bond) and pass 2 (2 chi^2 x chi x chi, batched over omega)
     a2 = [r for r in per_launch if r["family"] == "gemm" and r["shape"][1] == chi and r["shape"][2] == chi
           and r["shape"][0] in (4 * chi, 2 * chi * chi)]
     a2_ms, a2_work = sum(r["ms"] for r in a2), sum(r["work"] for r in a2)
-    out = {"roofline": roof, "families": fams,
+    out = {"roofline": roof, "roofline_step": roofline_step, "families": fams,
            "contraction_a2": {"tflops": a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],
                               "frac": (a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,
                               "launches_per_step": len(a2) // nprof,
@@ -477,9 +623,10 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
            "fp64_peaks_tflops": peaks,
            "step_flop_model": {"kernel_time_sum_ms": tot_ms / nprof, "graph_ms_per_step": ms_per_step}}
     if int(os.environ.get("WORLD_SIZE", "1")) == 1 and not args.no_cpu_baseline:
-        sec, sample, _ = oracle_sample_seconds(args.config)
+        sec, sample, _ = oracle_step_seconds(args.config)
         out["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-                               "sample": sample, "seconds_per_step_extrapolated": sec}
+                               "sample": "ONE whole oracle RK4 step of this workload from the initial state ("
+                               + sample + ")", "seconds_per_step": sec}
     return out
 
 

@@ -20,6 +20,14 @@
  *  - All work is enqueued on the caller's CUDA stream given at qtt_ctx_create.  With eps == 0 every call
  *    that takes only device data is asynchronous (static shapes: rank = min(chi_max, rows, cols));
  *    with eps > 0 the rank of each bond is read back, i.e. ONE stream synchronisation per bond.
+ *  - `release` may be called while kernels that read the block are still queued on the context's stream (the library
+ *    never synchronises to free): the callback must be STREAM-ORDERED with respect to that stream, i.e. the block may
+ *    be reused only by work enqueued on the same stream afterwards (a stream-ordered pool such as torch's caching
+ *    allocator used under that stream, or cudaFreeAsync on it).  `alloc` is called on the calling thread, never
+ *    inside a graph capture.
+ *  - Jacobi SVDs that hit their sweep limit are recorded on the device.  Calls that synchronise (qtt_mps_get_core,
+ *    qtt_mps_dot, qtt_mps_norm, qtt_mps_schmidt, every call with eps > 0, qtt_ctx_jacobi_stats) return QTT_NUMERIC
+ *    once per new record, so non-convergence of an earlier asynchronous call cannot go unnoticed.
  *  - Every function returns a qtt_status; on error outputs are untouched and qtt_last_error() gives text.
  *    There is NO CPU fallback: without a usable CUDA device qtt_ctx_create fails with QTT_CUDA.
  *  - "dev" pointers are device pointers, "host" pointers are host pointers.
@@ -83,7 +91,7 @@ qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits);
 #define QTT_PROF_FAMILIES 7
 qtt_status qtt_ctx_profile(qtt_ctx* ctx, int enabled);
 qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_host, long long* launches_host);
-/* Number of kernels launched (or graph nodes replayed) by this context so far. */
+/* Number of kernels launched (or graph nodes replayed) by this context so far (per context). */
 long long qtt_ctx_launch_count(const qtt_ctx* ctx);
 
 /* PAPER.md:67-72 Eq. 4 (reading 9): right-to-left TT-SVD of the dense field dense_dev[x*N + y], N = 2^n_bits,
@@ -127,6 +135,9 @@ qtt_status qtt_axpy(qtt_ctx* ctx, double alpha, const qtt_mps* x, qtt_mps* y);
  * eps > 0: smallest r with sqrt(sum_{i>r} sigma_i^2) <= eps*||x||_F/sqrt(n-1), clamped to [1, chi_max].
  * A product handle is rounded by the zip-up (reading 8) with working bond chi_work. */
 qtt_status qtt_round(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps);
+/* The same with the working bond of the zip-up given per call; chi_work == 0: the context's
+ * setting (qtt_ctx_set_chi_work), else 2*chi_max.  Ignored for handles that are not products. */
+qtt_status qtt_round_ex(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps, int chi_work);
 /* The same for `batch` independent operands in single launches per site. */
 qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_max, double eps);
 /* PAPER.md:124-128 Eq. 11 on u = (u_1, u_2), in place: classical RK4 of
@@ -138,6 +149,11 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
 /* Inspection. */
 int qtt_mps_num_sites(const qtt_mps* x);
 qtt_status qtt_mps_bonds(const qtt_mps* x, int* bonds_out /* n+1 */);
+/* Device pointer to core k (0-based, bonds[k] x 4 x bonds[k+1] doubles, row-major) of a handle with EXPLICIT cores
+ * (from qtt_mps_from_dense / qtt_mps_from_cores / qtt_round / qtt_rk4_step / qtt_mps_clone); a lazy handle gives
+ * QTT_INVALID_ARG.  The memory is owned by the handle and valid until it is freed, rounded or stepped; reads must be
+ * ordered after the context's stream.  No copy, no synchronisation. */
+qtt_status qtt_mps_core_ptr(qtt_ctx* ctx, const qtt_mps* x, int k, const double** core_dev_out);
 /* Copy core k (0-based) to host_out (bonds[k]*4*bonds[k+1] doubles); materialises lazy handles. Synchronous. */
 qtt_status qtt_mps_get_core(qtt_ctx* ctx, const qtt_mps* x, int k, double* host_out);
 /* <a|b> by transfer matrices; result written to *out_host after a stream synchronisation. */

@@ -440,10 +440,11 @@ def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False):
 
 
 # --------------------------------------------------------------------------- O9
-def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False):
+def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False, info=None):
     """Classical RK4 (Eq. 11) on the MPS pair u = [u_1, u_2]; all
     roundings with the same (chi_max, eps); final combination as one 5-term sum
-    and one rounding (reading 10)."""
+    and one rounding (reading 10).  ``info`` (a dict), if given, receives under "final" the two
+    round_mps records (norm, singular values, discarded weight per bond) of the last rounding."""
     def stage(k, h):
         return [round_mps(lincomb([(1.0, u[i]), (h, k[i])]), chi_max, eps) for i in range(2)]
 
@@ -451,12 +452,16 @@ def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False
     k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
     k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
     k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
-    return [
+    recs = [{}, {}] if info is not None else [None, None]
+    out = [
         round_mps(
             lincomb([(1.0, u[i]), (dt / 6, k1[i]), (dt / 3, k2[i]), (dt / 3, k3[i]), (dt / 6, k4[i])]),
-            chi_max, eps)
+            chi_max, eps, recs[i])
         for i in range(2)
     ]
+    if info is not None:
+        info["final"] = recs
+    return out
 
 
 # ------------------------------------------------------------ harness utilities

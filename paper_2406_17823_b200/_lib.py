@@ -52,6 +52,8 @@ PROTOTYPES = {
     "qtt_hadamard": (C.c_int, [_P, _P, _P, _PP]),
     "qtt_axpy": (C.c_int, [_P, C.c_double, _P, _P]),
     "qtt_round": (C.c_int, [_P, _P, C.c_int, C.c_double]),
+    "qtt_round_ex": (C.c_int, [_P, _P, C.c_int, C.c_double, C.c_int]),
+    "qtt_mps_core_ptr": (C.c_int, [_P, _P, C.c_int, C.POINTER(C.c_void_p)]),
     "qtt_round_batch": (C.c_int, [_P, C.c_int, _PP, C.c_int, C.c_double]),
     "qtt_rk4_step": (C.c_int, [_P, _PP, _P, _P, _P, C.c_double, C.c_double, C.c_int, C.c_double]),
     "qtt_mps_num_sites": (C.c_int, [_P]),

@@ -34,8 +34,11 @@ class Context:
         self._blocks: dict[int, torch.Tensor] = {}
 
         def _alloc(nbytes, _user):
+            # the block is used only on self.stream and may be released with work still queued there (qtt.h): allocate
+            # it UNDER that stream, so torch's caching allocator hands it back only to later work on the same stream
             try:
-                t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device=self.device)
+                with torch.cuda.stream(self.stream):
+                    t = torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device=self.device)
             except Exception:
                 return None
             self._blocks[t.data_ptr()] = t
@@ -197,6 +200,17 @@ def qtt_axpy(ctx: Context, alpha: float, x: Mps, y: Mps) -> None:
 
 def qtt_round(ctx: Context, x: Mps, chi_max: int, eps: float = 0.0) -> None:
     ctx.check(ctx.lib.qtt_round(ctx.h, x.h, int(chi_max), float(eps)))
+
+
+def qtt_round_ex(ctx: Context, x: Mps, chi_max: int, eps: float = 0.0, chi_work: int = 0) -> None:
+    ctx.check(ctx.lib.qtt_round_ex(ctx.h, x.h, int(chi_max), float(eps), int(chi_work)))
+
+
+def qtt_mps_core_ptr(ctx: Context, x: Mps, k: int) -> int:
+    """Device address of core k of a handle with explicit cores (no copy)."""
+    p = C.c_void_p()
+    ctx.check(ctx.lib.qtt_mps_core_ptr(ctx.h, x.h, int(k), C.byref(p)))
+    return int(p.value)
 
 
 def qtt_round_batch(ctx: Context, xs: Sequence[Mps], chi_max: int, eps: float = 0.0) -> None:

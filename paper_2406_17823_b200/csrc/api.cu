@@ -141,7 +141,23 @@ int fail(qtt_ctx* ctx, const QttError& e) {
   }                                                              \
   return QTT_OK;
 
-void set_device(qtt_ctx* ctx) { QTT_CU(cudaSetDevice(ctx->device)); }
+void set_device(qtt_ctx* ctx) {
+  QTT_CU(cudaSetDevice(ctx->device));
+  qtt_stats_bind(&ctx->stats);
+}
+
+// Jacobi non-convergence is recorded on the device (jac_status[1]).  Calls that synchronise the stream anyway read it
+// back and return QTT_NUMERIC once per new hit, so a half-orthogonalised SVD of an earlier asynchronous call (eps == 0,
+// graph replay) cannot go unnoticed.  Synchronises the stream.
+void check_numeric(qtt_ctx* ctx) {
+  int h[2] = {0, 0};
+  QTT_CU(cudaMemcpyAsync(h, ctx->jac_status, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+  QTT_CU(cudaStreamSynchronize(ctx->stream));
+  if (h[1] > ctx->numeric_seen) {
+    ctx->numeric_seen = h[1];
+    QTT_THROW(QTT_NUMERIC, "a Jacobi SVD hit its sweep limit (not converged) in this or an earlier call on this context");
+  }
+}
 
 }  // namespace
 
@@ -261,6 +277,7 @@ qtt_status qtt_ctx_create(qtt_ctx** out, int device, void* cuda_stream, qtt_allo
   ctx->alloc = alloc;
   ctx->release = release;
   ctx->user = user;
+  qtt_stats_bind(&ctx->stats);
   if (workspace_bytes < ((size_t)1 << 20)) workspace_bytes = (size_t)1 << 20;
   ctx->arena.base = static_cast<char*>(alloc(workspace_bytes, user));
   if (!ctx->arena.base) {
@@ -287,12 +304,12 @@ qtt_status qtt_ctx_create(qtt_ctx** out, int device, void* cuda_stream, qtt_allo
     ctx->jac_status = reinterpret_cast<int*>(ctx->arena.keep(32));
     QTT_CU(qtt_launch_fill(ctx->ones, 32, 1.0, ctx->stream));
     QTT_CU(cudaMemsetAsync(ctx->jac_status, 0, 32 * sizeof(double), ctx->stream));
-    qtt_kernels_init();
   } catch (const QttError& e) {
     if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     release(ctx->arena.base, user);
+    qtt_stats_destroy(&ctx->stats);
     delete ctx;
     return e.status;
   }
@@ -311,6 +328,7 @@ void qtt_ctx_destroy(qtt_ctx* ctx) {
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->arena.base) ctx->release(ctx->arena.base, ctx->user);
+  qtt_stats_destroy(&ctx->stats);
   delete ctx;
 }
 
@@ -346,13 +364,14 @@ qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits) 
   QTT_CU(cudaStreamSynchronize(ctx->stream));
   if (max_sweeps) *max_sweeps = h[0];
   if (limit_hits) *limit_hits = h[1];
+  ctx->numeric_seen = 0;
   if (h[1] > 0) QTT_THROW(QTT_NUMERIC, "Jacobi sweep limit hit");
   QTT_API_END(ctx)
 }
 qtt_status qtt_ctx_profile(qtt_ctx* ctx, int enabled) {
   if (!ctx) return QTT_INVALID_ARG;
   ctx->profiling = enabled ? 1 : 0;
-  qtt_prof_enable(enabled != 0);
+  ctx->stats.prof_on = enabled != 0;
   return QTT_OK;
 }
 qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_host, long long* launches_host) {
@@ -360,10 +379,10 @@ qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_ho
   static_assert(QK_COUNT == QTT_PROF_FAMILIES, "family count");
   QTT_API_BEGIN
   set_device(ctx);
-  QTT_CU(qtt_prof_collect(ms_host, work_host, launches_host));
+  QTT_CU(qtt_prof_collect(&ctx->stats, ms_host, work_host, launches_host));
   QTT_API_END(ctx)
 }
-long long qtt_ctx_launch_count(const qtt_ctx* ctx) { return g_qtt_launch_count + (ctx ? ctx->graph_launches : 0); }
+long long qtt_ctx_launch_count(const qtt_ctx* ctx) { return ctx ? ctx->stats.launches + ctx->graph_launches : 0; }
 
 // ------------------------------------------------------------------------------------------ MPS / MPO
 qtt_status qtt_mps_from_cores(qtt_ctx* ctx, int n, const int* bonds, const double* const* cores_host, qtt_mps** out) {
@@ -454,8 +473,18 @@ qtt_status qtt_mps_get_core(qtt_ctx* ctx, const qtt_mps* x, int k, double* host_
   View v = materialize(ctx, x->body);
   QTT_CU(cudaMemcpyAsync(host_out, v.core[k], sizeof(double) * (size_t)v.r[k] * 4 * v.r[k + 1], cudaMemcpyDeviceToHost,
                          ctx->stream));
-  QTT_CU(cudaStreamSynchronize(ctx->stream));
+  check_numeric(ctx);
   QTT_API_END(ctx)
+}
+
+qtt_status qtt_mps_core_ptr(qtt_ctx* ctx, const qtt_mps* x, int k, const double** core_dev_out) {
+  if (!ctx || !x || !core_dev_out || k < 0 || k >= x->body->n) return QTT_INVALID_ARG;
+  if (x->body->kind != BODY_DENSE) {
+    ctx->err = "qtt_mps_core_ptr needs explicit cores: round the lazy handle first (or use qtt_mps_get_core)";
+    return QTT_INVALID_ARG;
+  }
+  *core_dev_out = x->body->core[k];
+  return QTT_OK;
 }
 
 qtt_status qtt_mps_from_dense(qtt_ctx* ctx, const double* dense_dev, int n_bits, int chi_max, double eps,
@@ -576,8 +605,9 @@ qtt_status qtt_axpy(qtt_ctx* ctx, double alpha, const qtt_mps* x, qtt_mps* y) {
 }
 
 // ------------------------------------------------------------------------------------------ rounding
-qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_max, double eps) {
-  if (!ctx || !xs || batch < 1 || chi_max < 1 || eps < 0.0) return QTT_INVALID_ARG;
+static qtt_status round_batch_impl(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_max, double eps,
+                                   int chi_work) {
+  if (!ctx || !xs || batch < 1 || chi_max < 1 || eps < 0.0 || chi_work < 0) return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
   ArenaScope scope(ctx);
@@ -600,7 +630,7 @@ qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_
       for (size_t j = 0; j < dense_idx.size(); ++j) body_set_bonds(fresh[dense_idx[j]], out[j].r);
     }
     if (!prod_idx.empty()) {
-      const int cw = ctx->chi_work > 0 ? ctx->chi_work : 2 * chi_max;
+      const int cw = chi_work > 0 ? chi_work : (ctx->chi_work > 0 ? ctx->chi_work : 2 * chi_max);
       std::vector<View> A, B;
       std::vector<OutMps> out;
       for (int i : prod_idx) {
@@ -622,12 +652,22 @@ qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_
     body_release(xs[i]->body);
     xs[i]->body = fresh[i];
   }
+  if (eps > 0.0) check_numeric(ctx);  // this path synchronised once per bond already
   QTT_API_END(ctx)
+}
+
+qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_max, double eps) {
+  return round_batch_impl(ctx, batch, xs, chi_max, eps, 0);
 }
 
 qtt_status qtt_round(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps) {
   qtt_mps* xs[1] = {x};
-  return qtt_round_batch(ctx, 1, xs, chi_max, eps);
+  return round_batch_impl(ctx, 1, xs, chi_max, eps, 0);
+}
+
+qtt_status qtt_round_ex(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps, int chi_work) {
+  qtt_mps* xs[1] = {x};
+  return round_batch_impl(ctx, 1, xs, chi_max, eps, chi_work);
 }
 
 // ------------------------------------------------------------------------------------------ RK4
@@ -664,6 +704,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
       body_release(u[i]->body);
       u[i]->body = fresh[i];
     }
+    if (eps > 0.0) check_numeric(ctx);
     return QTT_OK;
   }
 
@@ -696,20 +737,20 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
       }
       View pin[2] = {packed_view(plan->rin[0], plan->in_buf[0]), packed_view(plan->rin[1], plan->in_buf[1])};
       OutMps pout[2] = {packed_out(plan->rout[0], plan->out_buf[0]), packed_out(plan->rout[1], plan->out_buf[1])};
-      const long long launches_before = g_qtt_launch_count;  // captured launches run at replay, counted there
+      const long long launches_before = ctx->stats.launches;  // captured launches run at replay, counted there
       QTT_CU(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed));
       try {
         qtt_rk4_eager(ctx, pin, Dx->data, Dy->data, Lap->data, Re, dt, chi_max, 0.0, cw, ctx->skew, pout);
       } catch (...) {
         cudaGraph_t junk = nullptr;
-        g_qtt_launch_count = launches_before;
+        ctx->stats.launches = launches_before;
         cudaStreamEndCapture(ctx->stream, &junk);
         if (junk) cudaGraphDestroy(junk);
         throw;
       }
       QTT_CU(cudaStreamEndCapture(ctx->stream, &plan->graph));
-      plan->nodes = (size_t)(g_qtt_launch_count - launches_before);  // kernel nodes only
-      g_qtt_launch_count = launches_before;
+      plan->nodes = (size_t)(ctx->stats.launches - launches_before);  // kernel nodes only
+      ctx->stats.launches = launches_before;
       QTT_CU(cudaGraphInstantiate(&plan->exec, plan->graph, 0));
     } catch (...) {
       plan_free(ctx, plan);
@@ -756,7 +797,7 @@ qtt_status qtt_mps_dot(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, double*
   View va = materialize(ctx, a->body), vb = materialize(ctx, b->body);
   double* d = qtt_dot_view(ctx, va, vb);
   QTT_CU(cudaMemcpyAsync(out_host, d, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-  QTT_CU(cudaStreamSynchronize(ctx->stream));
+  check_numeric(ctx);
   QTT_API_END(ctx)
 }
 
@@ -785,7 +826,7 @@ qtt_status qtt_mps_schmidt(qtt_ctx* ctx, const qtt_mps* x, double* sigma_host, i
     QTT_CU(cudaMemcpyAsync(sigma_host + (size_t)k * cap, sc.sigma[0][k], sizeof(double) * c, cudaMemcpyDeviceToHost,
                            ctx->stream));
   }
-  QTT_CU(cudaStreamSynchronize(ctx->stream));
+  check_numeric(ctx);
   QTT_API_END(ctx)
 }
 
@@ -817,7 +858,7 @@ qtt_status qtt_mps_norm(qtt_ctx* ctx, const qtt_mps* x, double* out_host) {
   const int c = sc.count[0][n - 1];
   std::vector<double> s(c);
   QTT_CU(cudaMemcpyAsync(s.data(), sc.sigma[0][n - 1], sizeof(double) * c, cudaMemcpyDeviceToHost, ctx->stream));
-  QTT_CU(cudaStreamSynchronize(ctx->stream));
+  check_numeric(ctx);
   double t = 0.0;
   for (int i = c - 1; i >= 0; --i) t += s[i] * s[i];
   *out_host = std::sqrt(t);

@@ -141,6 +141,7 @@ struct SelProb {
 #define QTT_SEL_MAX_BATCH 16
 struct SelGroup { int nprob; SelProb p[QTT_SEL_MAX_BATCH]; };
 cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream);
+int qtt_select_max_rows();  // largest p the sort handles (shared-memory keys)
 
 // ----------------------------------------------------------------------------------------------
 // Data movement (bandwidth-bound).
@@ -173,15 +174,21 @@ cudaError_t qtt_launch_copy2d(const double* src, int rows, int cols, int lds, do
                               cudaStream_t stream);
 cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t stream);
 
-// Number of kernels enqueued by the launchers above (qtt_ctx_launch_count).
-extern long long g_qtt_launch_count;
-void qtt_kernels_init();
-
-// Per-family kernel timing (qtt_ctx_profile_*): when enabled, every launch is bracketed by a CUDA event
-// pair on its stream.  Must be off while a stream is being captured.
+// Per-context launch counter and per-kernel-family timing (qtt_ctx_launch_count, qtt_ctx_profile_*).  The launchers
+// only know a stream, so the record they write to is a thread-local pointer that every qtt_* call binds to its
+// context on entry; the handle-less diagnostic entry points (qtt_diag.h) fall back to one process-wide record.
 enum QttKernelFamily { QK_GEMM = 0, QK_LQ_PANEL, QK_LQ_UPDATE, QK_JACOBI, QK_SELECT, QK_MOVE, QK_QRCP, QK_COUNT };
+struct QttProfRec { int fam; cudaEvent_t e0, e1; double work; int d[4]; };
+struct QttStats {
+  long long launches = 0;  // kernels enqueued by the launchers above
+  bool prof_on = false;    // bracket every launch by a CUDA event pair (must be off while a stream is being captured)
+  void* recs = nullptr;    // std::vector<QttProfRec>*, owned by probe.cu
+};
+QttStats* qtt_stats_current();
+void qtt_stats_bind(QttStats* s);  // nullptr: back to the process-wide default record
+void qtt_stats_destroy(QttStats* s);
 struct QttProf {
-  int fam;
+  QttStats* stats;
   cudaStream_t st;
   bool live;
   // work: algorithmic flops (GEMM, LQ, Jacobi) or bytes (select, move) of this launch
@@ -189,6 +196,9 @@ struct QttProf {
   QttProf(int family, cudaStream_t stream, double work, int d0 = 0, int d1 = 0, int d2 = 0, int d3 = 0);
   ~QttProf();
 };
-void qtt_prof_enable(bool on);
-// Synchronises the device, sums the event pairs recorded so far and clears them.
-cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]);
+// Synchronises the device, sums the event pairs recorded in `s` so far and clears them.
+cudaError_t qtt_prof_collect(QttStats* s, double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]);
+
+// Kernel attributes (opt-in shared memory, non-portable cluster size) are per DEVICE: true the first time `key`
+// (the kernel's address) is seen on the current device.  Thread-safe.
+bool qtt_first_use_on_device(const void* key);

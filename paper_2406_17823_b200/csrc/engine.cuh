@@ -93,8 +93,10 @@ struct qtt_ctx {
   int graphs = 1;
   int skew = 0;  // 1: skew-symmetric convection (PAPER.md Eq. B2) in qtt_rk4_step
   int profiling = 0;
+  QttStats stats;           // this context's launch counter and profiler records (bound on entry of every qtt_* call)
   double* ones = nullptr;   // device: 1.0
   int* jac_status = nullptr;  // device: [max sweeps, limit hits]
+  int numeric_seen = 0;       // limit hits already reported through QTT_NUMERIC
   long long graph_launches = 0;
   std::vector<Rk4Plan*> plans;
 };

@@ -226,12 +226,9 @@ template <int BM, int BN, int WM, int WN>
 cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream, int family) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
   constexpr size_t SMEM = (size_t)STAGES * (BM + BN) * KPITCH * sizeof(double);
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_gemm_dmma_kernel<BM, BN, WM, WN>)))
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_gemm_dmma_kernel<BM, BN, WM, WN>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-    attr_done = true;
-  }
   int t = 0;
   for (int i = 0; i < grp.nprob; ++i) {
     GemmProb& p = grp.p[i];

@@ -492,12 +492,14 @@ __global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_con
 // ------------------------------------------------------------------------------------------------
 // select: sort rows by norm (bitonic in shared memory), rank rule, normalised top rows.
 constexpr int SNT = 256;
-constexpr int SEL_MAXP = 2048;
+constexpr int SEL_MAXP = 16384;  // rows whose sort keys fit the opt-in shared memory (12 bytes per padded row)
 
-__global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__ SelGroup g) {
+// dynamic shared memory: key [np] doubles | idx [np] ints, np = rows padded to a power of two
+__global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__ SelGroup g, int npmax) {
   const SelProb& P = g.p[blockIdx.x];
-  __shared__ double key[SEL_MAXP];
-  __shared__ int idx[SEL_MAXP];
+  extern __shared__ __align__(16) double sel_sm[];
+  double* key = sel_sm;
+  int* idx = reinterpret_cast<int*>(sel_sm + npmax);
   __shared__ int s_rank;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int p = P.p, q = P.q;
@@ -590,12 +592,10 @@ namespace {
 template <int EPL>
 cudaError_t launch_blockjacobi(JacGroup& grp, int pmax, int qmax, int b, int pitch, size_t smem, double flops,
                                cudaStream_t stream) {
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_blockjacobi_kernel<EPL>))) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         224 * 1024));
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    attr_done = true;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grp.cluster * grp.nprob);
@@ -688,11 +688,9 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
       if (probs[i].p >= 2 && probs[i].q >= 1 && !(probs[i].work && qtt_sbj_fits(probs[i].p, probs[i].q))) ok = false;
     if (ok) return qtt_launch_sbj(probs, n, stream);
   }
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_rowjacobi_kernel))) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_rowjacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_rowjacobi_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    attr_done = true;
   }
   for (int b0 = 0; b0 < n; b0 += QTT_JAC_MAX_BATCH) {
     JacGroup grp;
@@ -772,19 +770,27 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
   return cudaSuccess;
 }
 
+int qtt_select_max_rows() { return SEL_MAXP; }
+
 cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream) {
   for (int b0 = 0; b0 < n; b0 += QTT_SEL_MAX_BATCH) {
     SelGroup g;
     g.nprob = n - b0 < QTT_SEL_MAX_BATCH ? n - b0 : QTT_SEL_MAX_BATCH;
+    int npmax = 2;
     for (int i = 0; i < g.nprob; ++i) {
       g.p[i] = probs[b0 + i];
-      if (g.p[i].p > SEL_MAXP) return cudaErrorInvalidValue;
+      if (g.p[i].p > SEL_MAXP) return cudaErrorInvalidValue;  // callers check qtt_select_max_rows() first
+      while (npmax < g.p[i].p) npmax <<= 1;
     }
+    const size_t smem = (size_t)npmax * (sizeof(double) + sizeof(int));
+    if (smem > 48 * 1024 && qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_select_kernel)))
+      QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)((size_t)SEL_MAXP * (sizeof(double) + sizeof(int)))));
     double bytes = 0.0;
     for (int i = 0; i < g.nprob; ++i) bytes += 8.0 * ((double)g.p[i].p * g.p[i].q + (double)g.p[i].r_cap * g.p[i].q);
     {
       QttProf prof(QK_SELECT, stream, bytes, g.p[0].p, g.p[0].q, g.nprob, 0);
-      qtt_select_kernel<<<g.nprob, SNT, 0, stream>>>(g);
+      qtt_select_kernel<<<g.nprob, SNT, smem, stream>>>(g, npmax);
     }
     QTT_CHECK_CUDA(cudaGetLastError());
   }

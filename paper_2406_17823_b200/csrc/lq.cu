@@ -332,11 +332,9 @@ size_t qtt_lq_scratch_doubles(int m) { return (size_t)SP_MAX * m; }
 // at chi = 128: HBM-bound) is streamed once per 64 rows instead of once per 16.  Batches that fit the L2 (config 3: 67 MB)
 // keep one-level blocking: there the extra small updates cost more than the saved passes.
 cudaError_t qtt_launch_lq(const LqProb* probs, int n, cudaStream_t stream) {
-  static bool attr_done = false;
-  if (!attr_done) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_lq_panel_kernel))) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_lq_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_lq_panel_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    attr_done = true;
   }
   for (int b0 = 0; b0 < n; b0 += QTT_LQ_MAX_BATCH) {
     const int nb = n - b0 < QTT_LQ_MAX_BATCH ? n - b0 : QTT_LQ_MAX_BATCH;

@@ -1,7 +1,10 @@
 // fp64 issue-rate probes (include/qtt_diag.h: qtt_diag_fp64_probe) -- the measured denominators of the
-// fp64 roofline (MEASURED_PEAKS.json carries no fp64 figure), and the one-time
-// kernel attribute setup.
+// fp64 roofline (MEASURED_PEAKS.json carries no fp64 figure), the per-context launch
+// counter / profiler records and the per-device kernel-attribute bookkeeping.
 #include <cstdio>
+#include <mutex>
+#include <set>
+#include <utility>
 #include <vector>
 
 #include "../../include/qtt_diag.h"
@@ -50,38 +53,64 @@ __global__ void __launch_bounds__(256) qtt_probe_dfma_kernel(int iters, double* 
 
 }  // namespace
 
-long long g_qtt_launch_count = 0;
-
-// ------------------------------------------------------------------------------------------ profiler
+// ------------------------------------------------------------------------------------------ per-context stats
 namespace {
-struct ProfRec { int fam; cudaEvent_t e0, e1; double work; int d[4]; };
-bool g_prof_on = false;
-std::vector<ProfRec> g_prof;
+QttStats g_default_stats;
+thread_local QttStats* t_stats = nullptr;
+std::vector<QttProfRec>& recs_of(QttStats* s) {
+  if (!s->recs) s->recs = new std::vector<QttProfRec>();
+  return *static_cast<std::vector<QttProfRec>*>(s->recs);
+}
+std::mutex g_attr_mu;
+std::set<std::pair<int, const void*>> g_attr_seen;
 }  // namespace
 
+QttStats* qtt_stats_current() { return t_stats ? t_stats : &g_default_stats; }
+void qtt_stats_bind(QttStats* s) { t_stats = s; }
+void qtt_stats_destroy(QttStats* s) {
+  if (!s) return;
+  if (s->recs) {
+    for (QttProfRec& r : recs_of(s)) {
+      cudaEventDestroy(r.e0);
+      cudaEventDestroy(r.e1);
+    }
+    delete static_cast<std::vector<QttProfRec>*>(s->recs);
+    s->recs = nullptr;
+  }
+  if (t_stats == s) t_stats = nullptr;
+}
+
+bool qtt_first_use_on_device(const void* key) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  std::lock_guard<std::mutex> lock(g_attr_mu);
+  return g_attr_seen.insert({dev, key}).second;
+}
+
 QttProf::QttProf(int family, cudaStream_t stream, double work, int d0, int d1, int d2, int d3)
-    : fam(family), st(stream), live(g_prof_on) {
-  ++g_qtt_launch_count;
-  if (!live) return;
-  ProfRec r;
-  r.fam = fam;
+    : stats(qtt_stats_current()), st(stream), live(false) {
+  ++stats->launches;
+  if (!stats->prof_on) return;
+  QttProfRec r;
+  r.fam = family;
   r.work = work;
   r.d[0] = d0; r.d[1] = d1; r.d[2] = d2; r.d[3] = d3;
-  if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) {
-    live = false;
+  if (cudaEventCreate(&r.e0) != cudaSuccess) return;
+  if (cudaEventCreate(&r.e1) != cudaSuccess) {
+    cudaEventDestroy(r.e0);
     return;
   }
+  live = true;
   cudaEventRecord(r.e0, st);
-  g_prof.push_back(r);
+  recs_of(stats).push_back(r);
 }
 QttProf::~QttProf() {
-  if (live) cudaEventRecord(g_prof.back().e1, st);
+  if (live) cudaEventRecord(recs_of(stats).back().e1, st);
 }
-void qtt_prof_enable(bool on) { g_prof_on = on; }
-cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]) {
+cudaError_t qtt_prof_collect(QttStats* s, double ms[QK_COUNT], double work[QK_COUNT], long long launches[QK_COUNT]) {
   for (int i = 0; i < QK_COUNT; ++i) ms[i] = work[i] = 0.0, launches[i] = 0;
   cudaError_t e = cudaDeviceSynchronize();
-  for (ProfRec& r : g_prof) {
+  for (QttProfRec& r : recs_of(s)) {
     float t = 0.f;
     if (e == cudaSuccess && cudaEventElapsedTime(&t, r.e0, r.e1) == cudaSuccess) {
       ms[r.fam] += t;
@@ -91,12 +120,11 @@ cudaError_t qtt_prof_collect(double ms[QK_COUNT], double work[QK_COUNT], long lo
     cudaEventDestroy(r.e0);
     cudaEventDestroy(r.e1);
   }
-  g_prof.clear();
+  recs_of(s).clear();
   return e;
 }
 
-void qtt_kernels_init() {}
-
+// writes the records of the calling thread's current context (the context of its last qtt_* call)
 extern "C" int qtt_diag_profile_dump(const char* path_host) {
   if (!path_host) return (int)cudaErrorInvalidValue;
   cudaError_t e = cudaDeviceSynchronize();
@@ -105,7 +133,7 @@ extern "C" int qtt_diag_profile_dump(const char* path_host) {
   if (!f) return (int)cudaErrorInvalidValue;
   static const char* names[QK_COUNT] = {"gemm", "lq_panel", "lq_update", "rowjacobi", "select", "move", "qrcp"};
   fprintf(f, "family,d0,d1,d2,d3,ms,work\n");
-  for (ProfRec& r : g_prof) {
+  for (QttProfRec& r : recs_of(qtt_stats_current())) {
     float t = 0.f;
     if (cudaEventElapsedTime(&t, r.e0, r.e1) != cudaSuccess) continue;
     fprintf(f, "%s,%d,%d,%d,%d,%.6f,%.6g\n", names[r.fam], r.d[0], r.d[1], r.d[2], r.d[3], (double)t, r.work);

@@ -794,15 +794,9 @@ int qrcp_cluster(int q) {
 
 template <class K>
 cudaError_t launch_qrcp(K kern, const QrcpGroup& g, size_t smem, double flops, int pmax, int qmax, cudaStream_t stream) {
-  // the kernels share one function-pointer type, so remember per pointer which ones have their attributes set
-  static const void* done[8];
-  static int ndone = 0;
-  bool seen = false;
-  for (int i = 0; i < ndone; ++i) seen = seen || done[i] == reinterpret_cast<const void*>(kern);
-  if (!seen) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(kern))) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024));
     QTT_CHECK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    if (ndone < 8) done[ndone++] = reinterpret_cast<const void*>(kern);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(g.cluster * g.nprob);

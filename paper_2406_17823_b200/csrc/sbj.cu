@@ -243,12 +243,10 @@ __global__ void __launch_bounds__(SNTH) qtt_sbj_round_kernel(const __grid_consta
 bool qtt_sbj_fits(int p, int q) { return p >= 2 && q >= 1 && q <= SPITCH; }
 
 cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
-  static bool attr_done = false;
   const size_t smem = ((size_t)SB * SPITCH + SB + 2) * sizeof(double);
-  if (!attr_done) {
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_sbj_round_kernel))) {
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_intra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
   }
   for (int b0 = 0; b0 < n; b0 += QTT_JAC_MAX_BATCH) {
     SbjGroup g;
@@ -285,7 +283,7 @@ cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
       qtt_sbj_check_kernel<<<g.nprob, 32, 0, stream>>>(g);
     }
     QTT_CHECK_CUDA(cudaGetLastError());
-    g_qtt_launch_count += (long long)g.max_sweeps * (P + 1);  // + the init launch counted by QttProf
+    qtt_stats_current()->launches += (long long)g.max_sweeps * (P + 1);  // + the init launch counted by QttProf
   }
   return cudaSuccess;
 }

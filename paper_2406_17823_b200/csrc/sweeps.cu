@@ -224,6 +224,9 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
   std::vector<JacProb> jp;
   std::vector<SelProb> sp;
   for (const SvdJob& j : jobs) {
+    if (j.p > qtt_select_max_rows())
+      QTT_THROW(QTT_CAPACITY, "SVD with " + std::to_string(j.p) + " rows: the rank selection sorts at most " +
+                                  std::to_string(qtt_select_max_rows()) + " rows");
     int prow = j.p;
     const int* rank_dev = nullptr;
     if (j.p >= 2 && qtt_qrcp_fits(j.p, j.q)) {
@@ -795,11 +798,16 @@ std::vector<OutMps> alloc_outs_keep(qtt_ctx* ctx, const std::vector<std::vector<
 // Enqueue on the side stream with the side scratch region: swaps them into the context for the scope.
 struct SideScope {
   qtt_ctx* ctx;
+  size_t lo, hi;  // marks of the side scratch region, restored on exit (also when an exception unwinds the scope)
   explicit SideScope(qtt_ctx* c) : ctx(c) {
     std::swap(ctx->stream, ctx->side);
     std::swap(ctx->arena, ctx->side_arena);
+    lo = ctx->arena.lo;
+    hi = ctx->arena.hi;
   }
   ~SideScope() {
+    ctx->arena.lo = lo;
+    ctx->arena.hi = hi;
     std::swap(ctx->stream, ctx->side);
     std::swap(ctx->arena, ctx->side_arena);
   }

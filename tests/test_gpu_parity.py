@@ -282,6 +282,63 @@ def test_rk4_config2_matches_oracle(Q, ctx):
     assert Q.qtt_ctx_launch_count(ctx) > 0
 
 
+def test_round_ex_and_core_ptr(Q, ctx):
+    """qtt_round_ex (per-call working bond) == the oracle's round_product at that chi_work, for a
+    working bond that really truncates; qtt_mps_core_ptr hands out the device cores without a host copy."""
+    import torch
+    n, chi = 6, 6
+    A = O.from_dense(smooth_field(n, 3), chi_max=6)
+    B = O.from_dense(smooth_field(n, 4), chi_max=6)
+    for cw in (6, 9, 12, 36):
+        a, b = Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B)
+        c = Q.qtt_hadamard(ctx, a, b)
+        with pytest.raises(Q.QttError):
+            Q.qtt_mps_core_ptr(ctx, c, 0)          # lazy handle: no explicit cores
+        Q.qtt_round_ex(ctx, c, chi, 0.0, cw)
+        want = O.round_product(A, B, chi, chi_work=cw)
+        assert Q.qtt_mps_bonds(c) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, c), O.to_dense(want)) < TOL
+    # chi_work = 0 falls back to the default 2 * chi_max
+    c = Q.qtt_hadamard(ctx, Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B))
+    Q.qtt_round_ex(ctx, c, chi, 0.0, 0)
+    assert rel(gpu_dense(Q, ctx, c), O.to_dense(O.round_product(A, B, chi))) < TOL
+    # device pointers: read core k through torch from the raw address and compare with the host copy
+    r = Q.qtt_mps_bonds(c)
+    ctx.synchronize()
+    import ctypes as C
+    rt = None
+    for name in ("libcudart.so.12", "libcudart.so", "/usr/local/cuda/lib64/libcudart.so"):
+        try:
+            rt = C.CDLL(name)
+            break
+        except OSError:
+            continue
+    assert rt is not None, "CUDA runtime library not found"
+    for k in range(n):
+        ptr = Q.qtt_mps_core_ptr(ctx, c, k)
+        assert ptr != 0 and ptr % 8 == 0
+        host = Q.qtt_mps_get_core(ctx, c, k)
+        cnt = r[k] * 4 * r[k + 1]
+        buf = (C.c_double * cnt)()
+        assert rt.cudaMemcpy(buf, C.c_void_p(ptr), C.c_size_t(cnt * 8), 2) == 0   # cudaMemcpyDeviceToHost
+        assert np.array_equal(np.frombuffer(buf, dtype=np.float64).reshape(host.shape), host)
+
+
+def test_launch_count_is_per_context(Q, ctx):
+    """The launch counter and the profiler records belong to the context: work on one context does
+    not move the other's counter."""
+    other = Q.Context(device=0, workspace_bytes=1 << 28)
+    try:
+        a = Q.qtt_mps_from_cores(other, I.random_cores(5, 4, seed=2))
+        c0, o0 = Q.qtt_ctx_launch_count(ctx), Q.qtt_ctx_launch_count(other)
+        Q.qtt_round(other, a, 3)
+        other.synchronize()
+        assert Q.qtt_ctx_launch_count(other) > o0
+        assert Q.qtt_ctx_launch_count(ctx) == c0
+    finally:
+        other.close()
+
+
 # ---------------------------------------------------------------- error behaviour
 def test_errors_are_status_codes(Q, ctx):
     a = Q.qtt_mps_from_cores(ctx, I.random_cores(4, 3, seed=1))
@@ -311,26 +368,81 @@ def schmidt_close(Q, ctx, x, cores):
 
 
 def test_rk4_config3_full_size_matches_oracle(Q, big_ctx):
-    """BASELINE config 3 (the bench workload: 2^10 x 2^10 decaying jet, chi 64, chi_work 128, Re 2e5, dt 5e-5):
-    one graph-replayed qtt_rk4_step against one oracle step, dense 1024 x 1024 fields and Schmidt spectra."""
+    """BASELINE config 3 (the bench workload: 2^10 x 2^10 decaying jet, chi 64, chi_work 128, Re 2e5, dt 5e-5), as
+    SURVEY.md section 8d asks: steps 1-3 FREE-RUNNING (graph-replayed qtt_rk4_step against the oracle's own trajectory:
+    error growth over steps) and PER STEP with the GPU restarted from the oracle state; dense 1024 x 1024 fields and
+    Schmidt spectra."""
     import torch
     cfg = I.CONFIGS[3]
     n, chi = cfg["n"], cfg["chi"]
     ux, uy = I.config_fields(3)
     g, o = ops(Q, big_ctx, n)
     U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
-    u = [Q.qtt_mps_from_cores(big_ctx, U[0]), Q.qtt_mps_from_cores(big_ctx, U[1])]
+    free = [Q.qtt_mps_from_cores(big_ctx, U[0]), Q.qtt_mps_from_cores(big_ctx, U[1])]
     Q.qtt_ctx_set_graphs(big_ctx, True)
-    U1 = O.rk4_step(U, o[0], o[1], o[2], cfg["Re"], cfg["dt"], chi)
-    Q.qtt_rk4_step(big_ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
-    for i in range(2):
-        assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
-        assert rel(gpu_dense(Q, big_ctx, u[i]), O.to_dense(U1[i])) < TOL
-        schmidt_close(Q, big_ctx, u[i], U1[i])
+    errs = []
+    for step in range(3):
+        U1 = O.rk4_step(U, o[0], o[1], o[2], cfg["Re"], cfg["dt"], chi)
+        # restarted from the oracle state of this step (at step 0 the two coincide)
+        if step > 0:
+            u = [Q.qtt_mps_from_cores(big_ctx, U[0]), Q.qtt_mps_from_cores(big_ctx, U[1])]
+            Q.qtt_rk4_step(big_ctx, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+            for i in range(2):
+                assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+                assert rel(gpu_dense(Q, big_ctx, u[i]), O.to_dense(U1[i])) < TOL, ("restart", step)
+        Q.qtt_rk4_step(big_ctx, free, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+        for i in range(2):
+            assert Q.qtt_mps_bonds(free[i]) == O.bonds(U1[i])
+            e = rel(gpu_dense(Q, big_ctx, free[i]), O.to_dense(U1[i]))
+            errs.append(e)
+            assert e < TOL, ("free-running", step, errs)
+            if step in (0, 2):
+                schmidt_close(Q, big_ctx, free[i], U1[i])
+        U = U1
+    print("config 3 free-running relative errors (u_x, u_y per step):", ["%.2e" % e for e in errs])
     assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
     # from_dense at full size: the GPU TT-SVD of the dense field is the oracle's
     v = Q.qtt_mps_from_dense(big_ctx, torch.from_numpy(ux).cuda(), chi)
-    assert rel(gpu_dense(Q, big_ctx, v), O.to_dense(U[0])) < TOL
+    assert rel(gpu_dense(Q, big_ctx, v), O.to_dense(O.from_dense(ux, chi))) < TOL
+
+
+def test_config4_full_step_matches_stored_oracle(Q):
+    """BASELINE config 4 (2^11 x 2^11 decaying turbulence, chi 128, chi_work 256, Re 1e6, dt 0.1/2^10): ONE full
+    qtt_rk4_step in bench.py's launch configuration (graph replay, 24 GiB workspace as `bench.py --config 4`) against the
+    oracle step stored by tests/golden/make_cfg4_step.py (the oracle needs ~15 min for it; the script imports only
+    oracle/ and qtt_inputs/).  Dense 2048 x 2048 fields, bonds and Schmidt spectra.  The step runs the code paths config 3
+    never reaches: 1024 x 1024 zip-up SVDs, two-level LQ, 640 x 512 SVDs of the 5-term sum."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg4_step1.npz")
+    assert os.path.exists(path), "run tests/golden/make_cfg4_step.py"
+    z = np.load(path)
+    cfg = I.CONFIGS[4]
+    n, chi = cfg["n"], cfg["chi"]
+    assert int(z["n"]) == n and int(z["chi"]) == chi
+    U0 = [[z[f"u0_{i}_{k}"] for k in range(n)] for i in range(2)]
+    U1 = [[z[f"u1_{i}_{k}"] for k in range(n)] for i in range(2)]
+    # the stored input IS the oracle's from_dense of the seeded field (checked on the first cores only: cheap)
+    ux, _ = I.config_fields(4)
+    assert rel(O.to_dense(U0[0]), O.to_dense(O.from_dense(ux, chi))) < 1e-12
+    ctx4 = Q.Context(device=0, workspace_bytes=24 << 30)
+    try:
+        g, _ = ops(Q, ctx4, n)
+        u = [Q.qtt_mps_from_cores(ctx4, U0[0]), Q.qtt_mps_from_cores(ctx4, U0[1])]
+        Q.qtt_ctx_set_graphs(ctx4, True)
+        Q.qtt_rk4_step(ctx4, u, g[0], g[1], g[2], cfg["Re"], cfg["dt"], chi)
+        for i in range(2):
+            assert Q.qtt_mps_bonds(u[i]) == O.bonds(U1[i])
+            e = rel(gpu_dense(Q, ctx4, u[i]), O.to_dense(U1[i]))
+            print(f"config 4 full step, component {i}: relative error {e:.2e}")
+            assert e < TOL
+            sg = Q.qtt_mps_schmidt(ctx4, u[i])
+            for k in range(1, n):
+                so = z[f"sv1_{i}_{k}"]
+                m = min(len(sg[k]), len(so))
+                assert np.max(np.abs(np.asarray(sg[k][:m]) - so[:m])) <= 1e-9 * so[0]
+        assert Q.qtt_ctx_jacobi_stats(ctx4)[1] == 0
+    finally:
+        ctx4.close()
 
 
 def test_config4_size_primitives_match_oracle(Q, big_ctx):
@@ -396,14 +508,31 @@ def test_rk4_step_eps_rule_matches_oracle(Q, ctx):
     uy = -np.cos(2 * np.pi * X) * np.sin(2 * np.pi * Y) + 0.3 * smooth_field(n, 8)
     U = [O.from_dense(ux, chi, eps), O.from_dense(uy, chi, eps)]
     u = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
-    U1 = O.rk4_step(U, o[0], o[1], o[2], Re, dt, chi, eps)
+    info = {}
+    U1 = O.rk4_step(U, o[0], o[1], o[2], Re, dt, chi, eps, info=info)
     Q.qtt_rk4_step(ctx, u, g[0], g[1], g[2], Re, dt, chi, eps)
     for i in range(2):
-        # a singular value within rounding distance of the threshold may fall on either side: the fields must agree
-        # to the accuracy the threshold itself guarantees, and the ranks within one
+        # "several correct results" (reading 17): a discarded tail within rounding distance of the threshold
+        # delta may fall on either side.  The ranks must agree wherever the oracle's decision was NOT that close; where
+        # they differ (by one at most) the margin |tail - delta| / delta at that bond is logged and must be below 1e-6,
+        # and only then is the field compared at the accuracy the threshold itself guarantees.
         bg, bo = Q.qtt_mps_bonds(u[i]), O.bonds(U1[i])
-        assert all(abs(a - b) <= 1 for a, b in zip(bg, bo)), (bg, bo)
-        tol = TOL if bg == bo else 10 * eps
+        rec = info["final"][i]
+        delta = eps * rec["norm"] / np.sqrt(n - 1)
+        degenerate = False
+        for k in range(1, n):
+            if bg[k] == bo[k]:
+                continue
+            assert abs(bg[k] - bo[k]) <= 1, (bg, bo)
+            s = rec["singular_values"][k]
+            r = min(bg[k], bo[k])
+            tail = float(np.sqrt(np.sum(s[r:] ** 2)))
+            margin = abs(tail - delta) / delta
+            print(f"eps rule: component {i} bond {k}: ranks gpu {bg[k]} oracle {bo[k]}, tail {tail:.6e} delta {delta:.6e} "
+                  f"margin {margin:.2e}")
+            assert margin < 1e-6, "ranks differ at a bond whose threshold decision was not degenerate"
+            degenerate = True
+        tol = 10 * eps if degenerate else TOL
         assert rel(gpu_dense(Q, ctx, u[i]), O.to_dense(U1[i])) < tol
     assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
 
