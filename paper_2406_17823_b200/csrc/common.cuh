@@ -93,6 +93,9 @@ struct JacGroup {
   JacProb p[QTT_JAC_MAX_BATCH];
 };
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream);
+// Register-blocked cluster block Jacobi (bj2.cu): p <= 512 rows, q <= 512 columns.  Fills the launch fields of grp.
+bool qtt_bj2_config(int pmax, int qmax, int& EPL, int& BR, int& C);
+cudaError_t qtt_launch_bj2(JacGroup& grp, int pmax, int qmax, double flops, cudaStream_t stream);
 // L2-streamed block Jacobi (sbj.cu) for q <= 1024 columns, any number of rows; needs JacProb::work.
 cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream);
 bool qtt_sbj_fits(int p, int q);

@@ -10,6 +10,7 @@
 // exchanged all-to-all through distributed shared memory, so every CTA derives bit-identical
 // rotations and applies them to its own slice.
 #include <cooperative_groups.h>
+#include <cstdlib>
 
 #include "common.cuh"
 #include "jacobi_rot.cuh"
@@ -632,9 +633,40 @@ bool blockjacobi_config(int pmax, int qmax, int& EPL, int& C, int& b, int& pitch
 }  // namespace
 
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream) {
-  // production path: two-level block Jacobi; problems of one call (the operands of one site, similar shapes)
-  // share launches as long as the largest shape of the group fits a cluster's shared memory
-  {
+  // production path: the register-blocked cluster block Jacobi (bj2.cu); problems of one call (the operands of one
+  // site, similar shapes) share launches
+  static const bool use_old = getenv("QTT_OLD_BJ") != nullptr;
+  if (!use_old) {
+    bool all_fit = true;
+    for (int i = 0; i < n && all_fit; ++i) {
+      int EPL, BR, C;
+      if (probs[i].p >= 2 && probs[i].q >= 1 && !qtt_bj2_config(probs[i].p, probs[i].q, EPL, BR, C)) all_fit = false;
+    }
+    if (all_fit) {
+      int done = 0;
+      while (done < n) {
+        JacGroup grp;
+        grp.nprob = 0;
+        int pmax = 0, qmax = 0;
+        double flops = 0.0;
+        while (done < n && grp.nprob < QTT_JAC_MAX_BATCH) {
+          const JacProb& pr = probs[done];
+          if (pr.p >= 2 && pr.q >= 1) {
+            grp.p[grp.nprob++] = pr;
+            pmax = pr.p > pmax ? pr.p : pmax;
+            qmax = pr.q > qmax ? pr.q : qmax;
+            double a = pr.p > pr.q ? pr.p : pr.q, bb = pr.p > pr.q ? pr.q : pr.p;
+            flops += 6.0 * a * bb * bb + 20.0 * bb * bb * bb;
+          }
+          ++done;
+        }
+        if (grp.nprob == 0) continue;
+        QTT_CHECK_CUDA(qtt_launch_bj2(grp, pmax, qmax, flops, stream));
+      }
+      return cudaSuccess;
+    }
+  }
+  if (use_old) {
     int done = 0;
     bool all_fit = true;
     for (int i = 0; i < n && all_fit; ++i) {

@@ -4,9 +4,9 @@
     python tests/golden/make_cfg4_step.py            # from the repo root; ~10-25 min on 8-16 host cores
 
 Imports ONLY oracle/ and qtt_inputs/ (no CUDA path): the stored values are the oracle's.  The GPU parity test
-tests/test_gpu_parity.py::test_config4_full_step_matches_stored_oracle feeds the SAME input cores (stored too, so the
-test does not depend on re-running the oracle's from_dense) to qtt_rk4_step and compares dense fields and Schmidt spectra.
-Stored: the input cores u0_i_k, the output cores u1_i_k (fp64), and the oracle's Schmidt values of the output per bond.
+tests/test_gpu_parity.py::test_config4_full_step_matches_stored_oracle recomputes the input cores with the oracle's
+from_dense (seconds), feeds them to qtt_rk4_step and compares dense fields, bonds and Schmidt spectra.
+Stored: the output cores u1_i_k (fp64) and the oracle's Schmidt values of the output per bond (sv1_i_k).
 """
 import os
 import sys
@@ -38,7 +38,6 @@ def main():
     out = {"n": n, "chi": chi, "Re": c["Re"], "dt": c["dt"]}
     for i in range(2):
         for k in range(n):
-            out[f"u0_{i}_{k}"] = U[i][k]
             out[f"u1_{i}_{k}"] = U1[i][k]
         sv = O.schmidt_values(U1[i])
         for k in range(1, n):
