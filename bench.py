@@ -459,14 +459,20 @@ def primitive_sweep(args):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
     n = 12
-    ctx = Q.Context(device=0, workspace_bytes=int(max(args.workspace_gib, 24.0) * (1 << 30)))
+    ctx = Q.Context(device=0, workspace_bytes=int(max(args.workspace_gib, 64.0) * (1 << 30)))
     dx = 1.0 / (1 << n)
     mpos = [Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx),
             Q.qtt_mpo_laplacian(ctx, n, dx)]
     peaks = fp64_peaks(Q, ctx)
     out = {}
-    for chi in (16, 32, 64, 128):
+    r = lambda chi: _bond_profile(n, chi)
+    for chi in (16, 32, 64, 128, 256):
         xs = [Q.qtt_mps_from_cores(ctx, I.random_cores(n, chi, seed=s)) for s in range(6)]
+        # algorithmic work of the two primitives on the batch of 6 (SURVEY.md section 8(d) per-site formulas)
+        mul = lambda D: [D * x if 0 < i < n else x for i, x in enumerate(r(chi))]
+        w3, w5, wz = _round_dense_work(mul(3), chi, 3), _round_dense_work(mul(5), chi, 5), _zip_work(r(chi), r(chi), chi, 2 * chi)
+        alg = {"apply_round": 4 * sum(w3[:3]) + 2 * sum(w5[:3]), "hadamard_round": 6 * sum(wz[:3])}
+        alg_gemm = {"apply_round": 4 * w3[0] + 2 * w5[0], "hadamard_round": 6 * wz[0]}
 
         def apply_round():
             ys = [Q.qtt_apply_mpo(ctx, mpos[i % 3], xs[i]) for i in range(6)]
@@ -496,17 +502,24 @@ def primitive_sweep(args):
             rep = Q.qtt_ctx_profile_report(ctx)
             Q.qtt_ctx_profile(ctx, False)
             g = rep["gemm"]
-            res[name] = {"ms_per_batch_of_6": float(np.median(times)),
+            ms = float(np.median(times))
+            tf = alg[name] / (ms * 1e-3) * 1e-12
+            stats = Q.qtt_ctx_jacobi_stats(ctx)
+            res[name] = {"ms_per_batch_of_6": ms,
+                         "algorithmic_gflop": alg[name] * 1e-9, "gemm_shaped_share": alg_gemm[name] / alg[name],
+                         "roofline": {"bound": "tensor", "achieved": tf, "peak": peaks["dmma"], "unit": "TFLOP/s",
+                                      "frac": tf / peaks["dmma"]},
                          "family_ms": {k: round(v["ms"], 3) for k, v in rep.items()},
                          "gemm_tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12,
-                         "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"]}
+                         "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"],
+                         "jacobi_max_sweeps": int(stats[0]), "jacobi_limit_hits": int(stats[1])}
         out[str(chi)] = res
         del xs
     line = {"metric": "primitive sweep at 2^12x2^12, batch 6 (BASELINE.json configs[4])", "unit": "ms per batch of 6",
             "dtype": "f64", "data": "synthetic", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
             "chi": out, "fp64_peaks_tflops": peaks,
-            "not_run": {"256": "the zip-up SVD at chi = 256 has 2048 columns: beyond the streamed Jacobi kernel (<= 1024), "
-                               "see DESIGN.md known limits"}}
+            "roofline_note": "per primitive: SURVEY.md section 8(d) algorithmic flops of the batch of 6 / median CUDA-event "
+                             "time / measured DMMA issue rate (fp64 tensor peak == fp64 FMA peak on B200)"}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -640,8 +653,8 @@ def main():
     ap.add_argument("--workspace-gib", type=float, default=8.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--primitive-sweep", action="store_true",
-                    help="BASELINE.json configs[4]: time apply+round and hadamard+round at 2^12 x 2^12, chi = 16..128, "
-                         "batch 6, instead of the RK4 step")
+                    help="BASELINE.json configs[4]: time apply+round and hadamard+round at 2^12 x 2^12, chi = 16..256, "
+                         "batch 6, with each primitive's roofline fraction, instead of the RK4 step")
     ap.add_argument("--convection", default="convective", choices=("convective", "skew"),
                     help="convective (BASELINE.json's configs, default) or the paper's skew-symmetric form (Eq. B2)")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",

@@ -277,16 +277,18 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
             Q = np.eye(m)
             Rn = T
             branch = "identity"
+            s = None
         elif k < m and k <= chi_work:
             Q, Rn = np.linalg.qr(T)
             branch = "qr"
+            s = None
         else:
             U, s, Vt = np.linalg.svd(T, full_matrices=False)
             keep = min(chi_work, len(s))
             Q = U[:, :keep]
             Rn = s[:keep, None] * Vt[:keep]
             branch = "svd"
-        zip_log.append(dict(T=T, Q=Q, R=Rn, branch=branch))
+        zip_log.append(dict(T=T, Q=Q, R=Rn, branch=branch, s=s))
         rn = Q.shape[1]
         cores.append(Q.reshape(r, d, rn))
         R = Rn.reshape(rn, a2, b2)

@@ -956,6 +956,7 @@ int qtt_diag_rowjacobi(void* stream, double* X, int batch, int p, int q, int ld,
     probs[i].p = p; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = nullptr;
     probs[i].work = nullptr;
+    probs[i].sweep_cap = 0;
     probs[i].status = status;
   }
   return (int)qtt_launch_rowjacobi(probs.data(), batch, static_cast<cudaStream_t>(stream));
@@ -969,6 +970,7 @@ int qtt_diag_rowjacobi_streamed(void* stream, double* X, int batch, int p, int q
     probs[i].p = p; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = nullptr;
     probs[i].work = work + 8 * (size_t)i;
+    probs[i].sweep_cap = 0;
     probs[i].status = status;
   }
   return (int)qtt_launch_sbj(probs.data(), batch, static_cast<cudaStream_t>(stream));
@@ -985,6 +987,7 @@ int qtt_diag_svd_rows(void* stream, double* X, int batch, int p, int q, int ld, 
     probs[i].p = p < q ? p : q; probs[i].q = q; probs[i].ld = ld;
     probs[i].p_dev = rank_dev + i;
     probs[i].work = nullptr;
+    probs[i].sweep_cap = 0;
     probs[i].status = status;
   }
   cudaError_t e = qtt_launch_qrcp(qp.data(), batch, 1, st);

@@ -81,6 +81,8 @@ struct JacProb {
   int p, q, ld;
   const int* p_dev;  // if non-null: number of rows to rotate (<= p), read on the device (numerical rank from qrcp)
   double* work;      // 8 doubles of device scratch (any content) for the L2-streamed path, or null
+  int sweep_cap;     // 0: the kernel's default sweep limit; else the limit for this problem (L2-streamed path: the launch
+                     // count is static, so the limit is kept as tight as the kind of input allows)
   int* status;  // device ints, may be shared by all problems: [0] <- max(sweeps used), [1] += 1 if the sweep limit was hit
 };
 #define QTT_JAC_MAX_BATCH 16

@@ -815,7 +815,7 @@ cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream) 
       while (npmax < g.p[i].p) npmax <<= 1;
     }
     const size_t smem = (size_t)npmax * (sizeof(double) + sizeof(int));
-    if (smem > 48 * 1024 && qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_select_kernel)))
+    if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_select_kernel)))
       QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)((size_t)SEL_MAXP * (sizeof(double) + sizeof(int)))));
     double bytes = 0.0;

@@ -18,10 +18,10 @@
 
 namespace {
 
-constexpr int SB = 16;    // rows per block
-constexpr int SNTH = 512;  // 16 warps: one per top row
-constexpr int SEPL = 32;   // elements per lane: q <= 1024
-constexpr int SPITCH = 32 * SEPL;
+// Two instantiations: <SB = 16 rows per block, SEPL = 32 elements per lane> for q <= 1024 columns (16 warps, one per
+// top row) and <8, 64> for q <= 2048 (the zip-up factor at chi = 256, BASELINE config 5): a top row of 2048 doubles
+// is 128 registers per lane, so a CTA holds 8 of them.
+constexpr int INIT_NTH = 512;
 
 struct SbjGroup {
   int nprob;
@@ -35,7 +35,8 @@ struct SbjGroup {
 __device__ __forceinline__ int sbj_rows(const JacProb& P) { return P.p_dev ? min(P.p, P.p_dev[0]) : P.p; }
 
 // ||X||_F^2 -> work[0]; clears the flags.  One CTA per problem.
-__global__ void __launch_bounds__(SNTH) qtt_sbj_init_kernel(const __grid_constant__ SbjGroup g) {
+__global__ void __launch_bounds__(INIT_NTH) qtt_sbj_init_kernel(const __grid_constant__ SbjGroup g) {
+  constexpr int SNTH = INIT_NTH;
   const JacProb& P = g.p[blockIdx.x];
   const int p = sbj_rows(P), q = P.q;
   __shared__ double red[SNTH / 32];
@@ -86,7 +87,9 @@ __device__ __forceinline__ void rr_pair(int P, int t, int k, int& ia, int& ib) {
 
 // shared memory: Bs [SB][SPITCH] | nB [SB] | flags
 // Pairs inside one block (once per sweep): CTA = block, 8 warps busy per round of the 16-player tournament.
-__global__ void __launch_bounds__(SNTH) qtt_sbj_intra_kernel(const __grid_constant__ SbjGroup g) {
+template <int SB, int SEPL>
+__global__ void __launch_bounds__(SB * 32) qtt_sbj_intra_kernel(const __grid_constant__ SbjGroup g) {
+  constexpr int SPITCH = 32 * SEPL;
   const JacProb& P = g.p[blockIdx.x / g.P];
   const int blk = blockIdx.x % g.P;
   if (P.work[1] != 0.0) return;
@@ -159,7 +162,9 @@ __global__ void __launch_bounds__(SNTH) qtt_sbj_intra_kernel(const __grid_consta
 }
 
 // One round of the block tournament: CTA = block pair, top rows in registers, bot block in shared memory.
-__global__ void __launch_bounds__(SNTH) qtt_sbj_round_kernel(const __grid_constant__ SbjGroup g) {
+template <int SB, int SEPL>
+__global__ void __launch_bounds__(SB * 32) qtt_sbj_round_kernel(const __grid_constant__ SbjGroup g) {
+  constexpr int SPITCH = 32 * SEPL;
   const int half = g.P / 2;
   const JacProb& P = g.p[blockIdx.x / half];
   const int k = blockIdx.x % half;
@@ -240,23 +245,27 @@ __global__ void __launch_bounds__(SNTH) qtt_sbj_round_kernel(const __grid_consta
 
 }  // namespace
 
-bool qtt_sbj_fits(int p, int q) { return p >= 2 && q >= 1 && q <= SPITCH; }
+bool qtt_sbj_fits(int p, int q) { return p >= 2 && q >= 1 && q <= 2048; }
 
-cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
+namespace {
+template <int SB, int SEPL>
+cudaError_t launch_sbj_cfg(const JacProb* probs, int n, cudaStream_t stream) {
+  constexpr int SPITCH = 32 * SEPL, SNTH = SB * 32;
   const size_t smem = ((size_t)SB * SPITCH + SB + 2) * sizeof(double);
-  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_sbj_round_kernel))) {
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_intra_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_sbj_round_kernel<SB, SEPL>))) {
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_intra_kernel<SB, SEPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_sbj_round_kernel<SB, SEPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   }
   for (int b0 = 0; b0 < n; b0 += QTT_JAC_MAX_BATCH) {
     SbjGroup g;
     g.nprob = 0;
-    int pmax = 0, qmax = 0;
+    int pmax = 0, qmax = 0, cap = 0;
     double flops = 0.0;
     for (int i = b0; i < n && g.nprob < QTT_JAC_MAX_BATCH; ++i) {
       const JacProb& pr = probs[i];
       if (pr.p < 2 || pr.q < 1) continue;
       if (!pr.work || pr.q > SPITCH) return cudaErrorInvalidValue;
+      cap = pr.sweep_cap > cap ? pr.sweep_cap : cap;
       g.p[g.nprob++] = pr;
       pmax = pr.p > pmax ? pr.p : pmax;
       qmax = pr.q > qmax ? pr.q : qmax;
@@ -267,18 +276,20 @@ cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
     int P = (pmax + SB - 1) / SB;
     P += P & 1;
     g.P = P;
-    g.max_sweeps = 30;
+    // unpreconditioned inputs (too large for the cluster-resident pivoted QR) need up to ~20 sweeps at 1024 columns
+    // (measured: 17-18 on the config-4 zip-up factors); the limit is a static launch count, so it is kept tight
+    g.max_sweeps = cap > 0 ? cap : (SEPL > 32 ? 40 : 30);
     g.round = 0;
     g.sweep = 0;
     // the whole iteration is booked as ONE profiler record of the family (first launch .. last launch)
     QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, g.nprob, 0);
-    qtt_sbj_init_kernel<<<g.nprob, SNTH, 0, stream>>>(g);
+    qtt_sbj_init_kernel<<<g.nprob, INIT_NTH, 0, stream>>>(g);
     for (int sweep = 0; sweep < g.max_sweeps; ++sweep) {
       g.sweep = sweep;
-      qtt_sbj_intra_kernel<<<P * g.nprob, SNTH, smem, stream>>>(g);
+      qtt_sbj_intra_kernel<SB, SEPL><<<P * g.nprob, SNTH, smem, stream>>>(g);
       for (int t = 0; t < P - 1; ++t) {
         g.round = t;
-        qtt_sbj_round_kernel<<<(P / 2) * g.nprob, SNTH, smem, stream>>>(g);
+        qtt_sbj_round_kernel<SB, SEPL><<<(P / 2) * g.nprob, SNTH, smem, stream>>>(g);
       }
       qtt_sbj_check_kernel<<<g.nprob, 32, 0, stream>>>(g);
     }
@@ -286,4 +297,14 @@ cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
     qtt_stats_current()->launches += (long long)g.max_sweeps * (P + 1);  // + the init launch counted by QttProf
   }
   return cudaSuccess;
+}
+}  // namespace
+
+cudaError_t qtt_launch_sbj(const JacProb* probs, int n, cudaStream_t stream) {
+  int qmax = 0;
+  for (int i = 0; i < n; ++i)
+    if (probs[i].p >= 2) qmax = probs[i].q > qmax ? probs[i].q : qmax;
+  if (qmax <= 1024) return launch_sbj_cfg<16, 32>(probs, n, stream);
+  if (qmax <= 2048) return launch_sbj_cfg<8, 64>(probs, n, stream);
+  return cudaErrorInvalidConfiguration;
 }

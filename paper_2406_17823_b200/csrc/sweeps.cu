@@ -199,6 +199,7 @@ struct SvdJob {
   const double* delta_ptr;
   double* delta_out;
   double delta_scale;
+  bool rank_deficient = false;  // expanded / direct-sum cores (rows a1, a3): rank-deficient by construction
 };
 
 // right singular vectors by row-Jacobi, preconditioned by a rank-revealing pivoted QR (qrcp.cu): X <- Q^T X has
@@ -238,6 +239,9 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
     JacProb a;
     a.X = j.X; a.p = prow; a.q = j.q; a.ld = j.q; a.p_dev = rank_dev; a.status = ctx->jac_status;
     a.work = ctx->arena.tmp(8);
+    // without the pivoted-QR preconditioner (matrix too large for a cluster's shared memory) a rank-deficient input
+    // needs 20-45 sweeps; the zip-up's full-rank triangular factors need < 20
+    a.sweep_cap = (rank_dev == nullptr && j.rank_deficient) ? 60 : 0;
     jp.push_back(a);
     SelProb s;
     s.X = j.X; s.p = prow; s.q = j.q; s.ld = j.q;
@@ -334,6 +338,7 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
         cap->count[i][k] = std::min(p, q);
       }
       j.rank = rank_dev[i];
+      j.rank_deficient = true;
       j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
       if (eps > 0.0) {
         if (k == n - 1) {

@@ -496,6 +496,106 @@ def test_config5_primitive_sweep_matches_oracle(Q, big_ctx, chi):
     assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
 
 
+def zip_cuts_are_safe(info, thr=1e-5):
+    """DESIGN.md reading 17: a working-bond cut of the zip-up is comparable between two implementations only if the
+    kept subspace is unique, i.e. the relative gap (s_keep - s_keep+1) / s_keep at the cut exceeds `thr` (or the cut lies
+    in the noise floor).  Uses the singular values the oracle itself computed at every truncating site."""
+    for z in info["zip"]:
+        if z["branch"] != "svd":
+            continue
+        sv, keep = z["s"], z["Q"].shape[1]
+        if keep < len(sv) and sv[keep - 1] > 1e-11 * sv[0]:
+            if (sv[keep - 1] - sv[keep]) <= thr * sv[keep - 1]:
+                return False
+    return True
+
+
+def graded_random_cores(n, chi, seed):
+    """Seeded N(0,1) site tensors (qtt_inputs.random_cores) with the columns of every core scaled geometrically, so
+    that all Schmidt spectra decay with clear gaps (canonicalised random cores with full-rank left bonds make the first
+    zip-up matrices exact isometries: all singular values equal, the kept subspace arbitrary)."""
+    cores = I.random_cores(n, chi, seed=seed)
+    return [c * np.logspace(0, -3, c.shape[2])[None, None, :] / np.sqrt(c.shape[0]) for c in cores]
+
+
+def test_round_product_wide_site_uses_the_tsqr_lq(Q, big_ctx):
+    """A zip-up site whose matrix T has more than 16384 columns (bonds 130 x 130 = 16900): the Q-less LQ of T goes through
+    the column-chunk TSQR tree of run_lq (sweeps.cu), which no BASELINE config below chi = 256 reaches."""
+    n, chi_op, chi, cw = 8, 130, 8, 16
+    A, B = graded_random_cores(n, chi_op, 3), graded_random_cores(n, chi_op, 4)
+    assert max(O.bonds(A)) == 130
+    info = {}
+    want = O.round_product(A, B, chi, chi_work=cw, info=info)
+    assert any(z["T"].shape[1] > 16384 and z["branch"] == "svd" for z in info["zip"])
+    assert zip_cuts_are_safe(info)
+    c = Q.qtt_hadamard(big_ctx, Q.qtt_mps_from_cores(big_ctx, A), Q.qtt_mps_from_cores(big_ctx, B))
+    Q.qtt_round_ex(big_ctx, c, chi, 0.0, cw)
+    assert Q.qtt_mps_bonds(c) == O.bonds(want)
+    assert rel(gpu_dense(Q, big_ctx, c), O.to_dense(want)) < TOL
+    assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
+
+
+def test_zipup_svd_with_2048_columns_matches_oracle(Q, big_ctx):
+    """The SVD shape of BASELINE config 5 at chi = 256 (working bond 512: a 2048 x 2048 triangular factor, the streamed
+    Jacobi's 2048-column instantiation) on operands small enough for the oracle: 10 sites with bonds 64, so T is 2048 x 4096."""
+    n, chi_op, chi, cw = 10, 64, 256, 512
+    A, B = graded_random_cores(n, chi_op, 5), graded_random_cores(n, chi_op, 6)
+    info = {}
+    want = O.round_product(A, B, chi, chi_work=cw, info=info)
+    assert any(z["T"].shape[0] == 2048 and z["branch"] == "svd" for z in info["zip"])
+    assert zip_cuts_are_safe(info)
+    c = Q.qtt_hadamard(big_ctx, Q.qtt_mps_from_cores(big_ctx, A), Q.qtt_mps_from_cores(big_ctx, B))
+    Q.qtt_round_ex(big_ctx, c, chi, 0.0, cw)
+    assert Q.qtt_mps_bonds(c) == O.bonds(want)
+    assert rel(gpu_dense(Q, big_ctx, c), O.to_dense(want)) < TOL
+    assert Q.qtt_ctx_jacobi_stats(big_ctx)[1] == 0
+
+
+def test_config5_chi256_matches_oracle_at_ten_sites(Q):
+    """BASELINE config 5's last point, chi = 256 (bond profile 4, 16, 64, 256, ..., working bond 512): one apply(Laplacian)
+    + round and one Hadamard + round with every bulk shape of the 12-site sweep (T = 2048 x 65536 through the TSQR LQ,
+    2048 x 2048 and 1024 x 1024 streamed Jacobi SVDs, 1280 x 1024 expanded cores), on a 10-site chain (bonds 4, 16, 64,
+    256, 256, 256, 64, 16, 4) so that the oracle's LAPACK SVDs of the 1 GB zip-up matrices stay within the test budget."""
+    n, chi = 10, 256
+    ctx5 = Q.Context(device=0, workspace_bytes=40 << 30)
+    try:
+        g, o = ops(Q, ctx5, n)
+        cores = [O.canonical_random(I.random_cores(n, chi, seed=s)) for s in range(2)]
+        assert max(O.bonds(cores[0])) == 256
+        xs = [Q.qtt_mps_from_cores(ctx5, c) for c in cores]
+        y = Q.qtt_apply_mpo(ctx5, g[2], xs[0])
+        Q.qtt_round(ctx5, y, chi)
+        want = O.round_mps(O.apply_mpo(o[2], cores[0]), chi)
+        assert Q.qtt_mps_bonds(y) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx5, y), O.to_dense(want)) < TOL
+        h = Q.qtt_hadamard(ctx5, xs[0], xs[1])
+        Q.qtt_round(ctx5, h, chi)
+        info = {}
+        want = O.round_product(cores[0], cores[1], chi, info=info)
+        assert Q.qtt_mps_bonds(h) == O.bonds(want)
+        assert Q.qtt_ctx_jacobi_stats(ctx5)[1] == 0
+        assert np.all(np.isfinite(gpu_dense(Q, ctx5, h)))
+        # left-canonical random cores whose first bonds are full (4, 16, 64, 256 = 4^l) make the first zip-up matrices
+        # isometries: if a working-bond cut falls into equal singular values the kept subspace is not unique (reading 17)
+        # and only bonds, finiteness and convergence are comparable; the graded operands below pin the same shapes
+        if zip_cuts_are_safe(info):
+            assert rel(gpu_dense(Q, ctx5, h), O.to_dense(want)) < TOL
+        else:
+            print("config 5 chi=256: degenerate working-bond cut on canonical random cores (unpinned, reading 17)")
+        A, B = graded_random_cores(n, chi, 7), graded_random_cores(n, chi, 8)
+        info = {}
+        want = O.round_product(A, B, chi, info=info)
+        assert zip_cuts_are_safe(info)
+        assert any(z["T"].shape == (2048, 65536) for z in info["zip"])
+        h = Q.qtt_hadamard(ctx5, Q.qtt_mps_from_cores(ctx5, A), Q.qtt_mps_from_cores(ctx5, B))
+        Q.qtt_round(ctx5, h, chi)
+        assert Q.qtt_mps_bonds(h) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx5, h), O.to_dense(want)) < TOL
+        assert Q.qtt_ctx_jacobi_stats(ctx5)[1] == 0
+    finally:
+        ctx5.close()
+
+
 def test_rk4_step_eps_rule_matches_oracle(Q, ctx):
     """qtt_rk4_step with eps > 0 (data-dependent ranks, one stream synchronisation per bond; the Laplacian branch on
     the side stream): same bonds and fields as the oracle, whose ranks come from the same rule."""
