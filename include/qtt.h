@@ -170,6 +170,13 @@ qtt_status qtt_mps_fidelity(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, do
  * truncation error sqrt(sum_{i > chi_l} sigma_i^2) / ||x|| <= eps, written to chi_host[l] (n+1 ints, ends = 1), and
  * chi = max_l chi_l to *chi_max_host (may be NULL).  Synchronous. */
 qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_host, int* chi_max_host);
+/* PAPER.md:173-184 Eq. 13-15: turbulent-kinetic-energy spectrum.  With u_i' = u_i - mean_i (mean_i == NULL: zero mean; Eq. 14)
+ * and the Fourier coefficients u_i'^(k) = (1/N^2) sum_x u_i'(x) exp(-2 pi i k.x), k in [-N/2, N/2)^2 (Eq. 13):
+ *   E_host[b] = 1/2 sum over the shell round(|k|) = b of (|u_1'^(k)|^2 + |u_2'^(k)|^2),  b = 0 .. nbins-1  (Eq. 15),
+ * so that sum_b E[b] = 1/2 mean(u_1'^2 + u_2'^2) (Parseval).  nbins >= floor(N / sqrt(2) + 1/2) + 1.  A diagnostic on
+ * dense fields (qtt_to_dense + an FFT kernel); needs ~10 N^2 doubles of workspace.  Synchronous. */
+qtt_status qtt_tke_spectrum(qtt_ctx* ctx, const qtt_mps* u1, const qtt_mps* u2, const qtt_mps* mean1, const qtt_mps* mean2,
+                            int nbins, double* E_host);
 qtt_status qtt_mps_clone(qtt_ctx* ctx, const qtt_mps* x, qtt_mps** out);
 void qtt_mps_free(qtt_mps* x);
 

@@ -35,6 +35,7 @@ where the paper is silent/garbled and the reading taken):
   O10 mpo_d1 / mpo_d2 / mpo_laplacian   PAPER.md:391-424 App. A, Eq. A1-A3, Table II
       mpo_stencil (any order)   PAPER.md:98, same construction
   O11 fidelity, chi_eps         PAPER.md:160 Eq. 12; Eq. 16-17 (diagnostics)
+      tke_spectrum              PAPER.md:173-184 Eq. 13-15
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
 grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
@@ -517,6 +518,27 @@ def fidelity(A, B) -> float:
     if na == 0.0 or nb == 0.0:
         return 0.0
     return dot(A, B) ** 2 / (na * na * nb * nb)
+
+
+def tke_spectrum(u1, u2, mean1=None, mean2=None):
+    """Turbulent-kinetic-energy spectrum (Eq. 13-15) of the velocity MPS pair (u1, u2):
+    u_i' = u_i - mean_i (Eq. 14; mean_i = None: zero), Fourier coefficients u_i'^(k) = (1/N^2) sum_x u_i'(x) exp(-2 pi i k.x)
+    on the N x N periodic grid, E(k1, k2) = 1/2 (|u_1'^|^2 + |u_2'^|^2) (Eq. 13), and E(kappa) = the sum of E(k1, k2) over the
+    shell round(sqrt(k1^2 + k2^2)) = kappa (Eq. 15, the integral over the circle discretised to integer shells).
+    Returns E[0 .. floor(N / sqrt(2) + 1/2)]; sum(E) = 1/2 mean(u_1'^2 + u_2'^2) (Parseval)."""
+    f = []
+    for u, m in ((u1, mean1), (u2, mean2)):
+        F = to_dense(u)
+        if m is not None:
+            F = F - to_dense(m)
+        f.append(F)
+    N = f[0].shape[0]
+    k = np.fft.fftfreq(N, d=1.0 / N)  # integer wave numbers -N/2 .. N/2-1
+    K1, K2 = np.meshgrid(k, k, indexing="ij")
+    shell = np.floor(np.sqrt(K1 * K1 + K2 * K2) + 0.5).astype(np.int64)
+    E2 = 0.5 * sum(np.abs(np.fft.fft2(F) / (N * N)) ** 2 for F in f)
+    nb = int(math.floor(math.sqrt(2.0) * (N // 2) + 0.5)) + 1
+    return np.bincount(shell.reshape(-1), weights=E2.reshape(-1), minlength=nb)[:nb]
 
 
 def chi_eps(cores, eps: float):

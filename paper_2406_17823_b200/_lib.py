@@ -64,6 +64,7 @@ PROTOTYPES = {
     "qtt_mps_schmidt": (C.c_int, [_P, _P, _DP, C.c_int, _IP]),
     "qtt_mps_fidelity": (C.c_int, [_P, _P, _P, _DP]),
     "qtt_mps_chi_eps": (C.c_int, [_P, _P, C.c_double, _IP, _IP]),
+    "qtt_tke_spectrum": (C.c_int, [_P, _P, _P, _P, _P, C.c_int, _DP]),
     "qtt_mps_clone": (C.c_int, [_P, _P, _PP]),
     "qtt_mps_free": (None, [_P]),
     # include/qtt_diag.h

@@ -288,6 +288,17 @@ def qtt_mps_chi_eps(ctx: Context, x: Mps, eps: float) -> tuple[list[int], int]:
     return list(out), mx.value
 
 
+def qtt_tke_spectrum(ctx: Context, u1: Mps, u2: Mps, mean1: "Mps | None" = None, mean2: "Mps | None" = None) -> np.ndarray:
+    """E(kappa) of PAPER.md Eq. 13-15 for shells kappa = 0 .. floor(N / sqrt(2) + 1/2)."""
+    n = ctx.lib.qtt_mps_num_sites(u1.h)
+    nbins = int(np.floor(np.sqrt(2.0) * (1 << n) / 2 + 0.5)) + 1
+    out = np.zeros(nbins, dtype=np.float64)
+    ctx.check(ctx.lib.qtt_tke_spectrum(ctx.h, u1.h, u2.h, mean1.h if mean1 is not None else None,
+                                       mean2.h if mean2 is not None else None, nbins,
+                                       out.ctypes.data_as(C.POINTER(C.c_double))))
+    return out
+
+
 def qtt_mps_clone(ctx: Context, x: Mps) -> Mps:
     h = C.c_void_p()
     ctx.check(ctx.lib.qtt_mps_clone(ctx.h, x.h, C.byref(h)))

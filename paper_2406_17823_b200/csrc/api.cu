@@ -878,6 +878,47 @@ qtt_status qtt_mps_fidelity(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, do
   return QTT_OK;
 }
 
+qtt_status qtt_tke_spectrum(qtt_ctx* ctx, const qtt_mps* u1, const qtt_mps* u2, const qtt_mps* mean1, const qtt_mps* mean2,
+                            int nbins, double* E_host) {
+  if (!ctx || !u1 || !u2 || !E_host || nbins < 1) return QTT_INVALID_ARG;
+  QTT_API_BEGIN
+  set_device(ctx);
+  ArenaScope scope(ctx);
+  const int n = u1->body->n;
+  if (u2->body->n != n || (mean1 && mean1->body->n != n) || (mean2 && mean2->body->n != n))
+    QTT_THROW(QTT_SHAPE_MISMATCH, "velocity components differ in length");
+  if (n < 1 || n > 12) QTT_THROW(QTT_CAPACITY, "TKE spectrum: grids up to 2^12 x 2^12");
+  const i64 N = 1ll << n;
+  const int max_shell = (int)std::floor(std::sqrt(2.0) * (double)(N / 2) + 0.5);
+  if (nbins < max_shell + 1) QTT_THROW(QTT_INVALID_ARG, "nbins must be at least floor(N / sqrt(2) + 1/2) + 1");
+  double* spec[2];
+  const qtt_mps* us[2] = {u1, u2};
+  const qtt_mps* ms[2] = {mean1, mean2};
+  for (int i = 0; i < 2; ++i) {
+    spec[i] = ctx->arena.keep((size_t)2 * N * N);
+    const size_t mark = ctx->arena.hi;
+    View v = materialize(ctx, us[i]->body);
+    if (ms[i]) {  // u' = u - u_mean (Eq. 14) as an exact direct sum
+      if (n < 2) QTT_THROW(QTT_INVALID_ARG, "a mean field needs at least two sites");
+      View m = materialize(ctx, ms[i]->body);
+      std::vector<View> o;
+      qtt_concat_batch(ctx, {{{1.0, v}, {-1.0, m}}}, o);
+      v = o[0];
+    }
+    double* dense = ctx->arena.tmp((size_t)N * N);
+    qtt_to_dense_view(ctx, v, dense);
+    double* tmp = ctx->arena.tmp((size_t)2 * N * N);
+    QTT_CU(qtt_launch_fft2_real(dense, spec[i], tmp, n, ctx->stream));
+    ctx->arena.hi = mark;
+  }
+  double* partial = ctx->arena.tmp((size_t)N * nbins);
+  double* E = ctx->arena.tmp((size_t)nbins);
+  QTT_CU(qtt_launch_tke_shells(spec[0], spec[1], n, nbins, partial, E, ctx->stream));
+  QTT_CU(cudaMemcpyAsync(E_host, E, sizeof(double) * nbins, cudaMemcpyDeviceToHost, ctx->stream));
+  check_numeric(ctx);
+  QTT_API_END(ctx)
+}
+
 qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_host, int* chi_max_host) {
   if (!ctx || !x || !chi_host || !(eps >= 0.0)) return QTT_INVALID_ARG;
   const int n = qtt_mps_num_sites(x);

@@ -178,6 +178,11 @@ cudaError_t qtt_launch_transpose(const double* src, int rows, int cols, int lds,
 cudaError_t qtt_launch_copy2d(const double* src, int rows, int cols, int lds, double* dst, int ldd,
                               cudaStream_t stream);
 cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t stream);
+// Diagnostics (spectrum.cu): unnormalised 2-D DFT of a real N x N field (complex output, interleaved re/im, transposed
+// wave-number order; tmp_c: 2 N^2 doubles) and the shell sums of the TKE spectrum (Eq. 13-15).
+cudaError_t qtt_launch_fft2_real(const double* F, double* out_c, double* tmp_c, int nbits, cudaStream_t stream);
+cudaError_t qtt_launch_tke_shells(const double* U1_c, const double* U2_c, int nbits, int nbins, double* partial,
+                                  double* E_dev, cudaStream_t stream);
 
 // Per-context launch counter and per-kernel-family timing (qtt_ctx_launch_count, qtt_ctx_profile_*).  The launchers
 // only know a stream, so the record they write to is a thread-local pointer that every qtt_* call binds to its

@@ -230,6 +230,8 @@ void run_svd(qtt_ctx* ctx, std::vector<SvdJob>& jobs) {
                                   std::to_string(qtt_select_max_rows()) + " rows");
     int prow = j.p;
     const int* rank_dev = nullptr;
+    // (the zip-up's triangular factors are preconditioned too: measured on the config-3 step, skipping the pivoted QR
+    // for them raises the Jacobi sweep count from 11 to 20)
     if (j.p >= 2 && qtt_qrcp_fits(j.p, j.q)) {
       int* rk = reinterpret_cast<int*>(ctx->arena.tmp(1));
       qp.push_back(QrcpProb{j.X, j.p, j.q, j.q, rk, 0, nullptr});

@@ -673,6 +673,32 @@ def test_diagnostics_match_oracle(Q, ctx):
         assert got == want and gmax == wmax
 
 
+@pytest.mark.parametrize("n", [3, 6, 10])
+def test_tke_spectrum_matches_oracle(Q, big_ctx, n):
+    """qtt_tke_spectrum (Eq. 13-15: the library's own FFT + shell sums) against the oracle's definition, with and
+    without the mean-flow subtraction of Eq. 14, on a turbulence-shaped field; Parseval; bitwise reproducibility."""
+    N = 1 << n
+    ux, uy = I.decaying_turbulence(n, seed=1, k0=min(16.0, N / 4))
+    ux = ux + 0.3  # a mean flow for shell 0
+    chi = min(32, 4 ** (n // 2))
+    A, B = O.from_dense(ux, chi), O.from_dense(uy, chi)
+    a, b = Q.qtt_mps_from_cores(big_ctx, A), Q.qtt_mps_from_cores(big_ctx, B)
+    want = O.tke_spectrum(A, B)
+    got = Q.qtt_tke_spectrum(big_ctx, a, b)
+    assert got.shape == want.shape
+    assert np.max(np.abs(got - want)) <= 1e-12 * want.max()
+    fa, fb = O.to_dense(A), O.to_dense(B)
+    assert abs(got.sum() - 0.5 * np.mean(fa * fa + fb * fb)) <= 1e-12 * got.sum()
+    assert np.array_equal(got, Q.qtt_tke_spectrum(big_ctx, a, b))
+    if n >= 2:
+        M = O.from_dense(np.full((N, N), 0.3))
+        m = Q.qtt_mps_from_cores(big_ctx, M)
+        want = O.tke_spectrum(A, B, M, None)
+        got = Q.qtt_tke_spectrum(big_ctx, a, b, m, None)
+        assert np.max(np.abs(got - want)) <= 1e-12 * want.max()
+        assert got[0] < 1e-3 * Q.qtt_tke_spectrum(big_ctx, a, b)[0]   # the mean flow is gone (up to the chi truncation)
+
+
 @pytest.mark.parametrize("graphs", [False, True])
 def test_rk4_step_skew_symmetric_matches_oracle(Q, ctx, graphs):
     """qtt_ctx_set_convection(1): the paper's skew-symmetric convection (PAPER.md Eq. B2, section 8f next-2), two steps

@@ -356,3 +356,45 @@ def test_skew_convection_conserves_discrete_energy():
     assert abs(work) < 1e-12 * scale
     g = O.rhs(u, Dx, Dy, Lap, Re, chi, chi_work=10**6)
     assert abs(O.dot(u[0], g[0]) + O.dot(u[1], g[1])) > 1e-4 * scale
+
+
+# ---------------------------------------------------------------- TKE spectrum (Eq. 13-15)
+def test_tke_spectrum_closed_forms_parseval_and_brute_force():
+    n = 5
+    N = 1 << n
+    X, Y = I.grid(n)
+    A_, B_ = 0.7, 1.3
+    u1 = O.from_dense(A_ * np.sin(2 * np.pi * (3 * X + 4 * Y)))      # |k| = 5: coefficients -+ A/(2i) at +-(3,4)
+    u2 = O.from_dense(B_ * np.cos(2 * np.pi * 7 * Y) + 0.25)         # |k| = 7, plus a mean flow in shell 0
+    E = O.tke_spectrum(u1, u2)
+    assert len(E) == int(np.floor(np.sqrt(2.0) * N / 2 + 0.5)) + 1
+    want = np.zeros_like(E)
+    want[5], want[7], want[0] = A_**2 / 4, B_**2 / 4, 0.25**2 / 2
+    assert np.max(np.abs(E - want)) < 1e-14
+    # Eq. 14: subtracting the mean flow empties shell 0 and nothing else
+    mean2 = O.from_dense(np.full((N, N), 0.25))
+    E2 = O.tke_spectrum(u1, u2, None, mean2)
+    want[0] = 0.0
+    assert np.max(np.abs(E2 - want)) < 1e-14
+    assert np.max(np.abs(O.tke_spectrum(u1, u2, u1, u2))) < 1e-28
+    # Parseval on a generic field: sum_k E(k) = 1/2 mean(u1^2 + u2^2)
+    F, G = smooth_field(n, 31), smooth_field(n, 32)
+    E = O.tke_spectrum(O.from_dense(F), O.from_dense(G))
+    assert abs(E.sum() - 0.5 * np.mean(F * F + G * G)) < 1e-13 * E.sum()
+    # brute force on an 8 x 8 grid: the DFT written as plain loops (no FFT), integer shells by rounding
+    n = 3
+    N = 8
+    F, G = rand_field(n, 41), rand_field(n, 42)
+    got = O.tke_spectrum(O.from_dense(F), O.from_dense(G))
+    bf = np.zeros(len(got))
+    for k1 in range(-N // 2, N // 2):
+        for k2 in range(-N // 2, N // 2):
+            c1 = c2 = 0.0 + 0.0j
+            for x in range(N):
+                for y in range(N):
+                    ph = np.exp(-2j * np.pi * (k1 * x + k2 * y) / N)
+                    c1 += F[x, y] * ph
+                    c2 += G[x, y] * ph
+            e = 0.5 * (abs(c1 / N**2) ** 2 + abs(c2 / N**2) ** 2)
+            bf[int(np.floor(np.hypot(k1, k2) + 0.5))] += e
+    assert np.max(np.abs(got - bf)) < 1e-13 * bf.max()
