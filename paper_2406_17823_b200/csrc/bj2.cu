@@ -364,6 +364,8 @@ bool qtt_bj2_config(int pmax, int qmax, int& EPL, int& BR, int& C) {
   else if (qmax <= 256) EPL = 8;
   else if (qmax <= 512) EPL = 16;
   else return false;
+  // 8-row blocks on up to 16 CTAs for p <= 256 (measured 10-15 % faster than 16-row blocks on half as many CTAs),
+  // 16-row blocks beyond
   BR = pmax <= 256 ? 8 : 16;
   C = (pmax + 2 * BR - 1) / (2 * BR);
   C = C < 1 ? 1 : C;

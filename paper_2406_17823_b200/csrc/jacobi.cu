@@ -1,5 +1,7 @@
 // Batched one-sided (Hestenes) Jacobi on the ROWS of X (the truncated-SVD
-// step of the R->L rounding sweep; row a6: the SVD of the zip-up's triangular factor).
+// step of the R->L rounding sweep; row a6: the SVD of the zip-up's triangular factor): the dispatcher
+// (qtt_launch_rowjacobi: bj2.cu for p, q <= 512, sbj.cu up to 2048 columns, the column-sliced kernel below as the
+// last resort) and the rank selection.
 //
 //   X (p x q)  <-  J X,   J orthogonal, rows of the result mutually orthogonal:  J X = Sigma V^T.
 //
@@ -10,7 +12,6 @@
 // exchanged all-to-all through distributed shared memory, so every CTA derives bit-identical
 // rotations and applies them to its own slice.
 #include <cooperative_groups.h>
-#include <cstdlib>
 
 #include "common.cuh"
 #include "jacobi_rot.cuh"
@@ -198,299 +199,6 @@ __global__ void __launch_bounds__(JNT) qtt_rowjacobi_kernel(const __grid_constan
 }
 
 // ------------------------------------------------------------------------------------------------
-// Two-level block Jacobi, the production path for every matrix whose row blocks fit in a cluster's shared
-// memory.  The p rows are cut into 2C blocks of b rows; every CTA of the cluster (C CTAs) holds two blocks
-// with their FULL rows, so a rotation needs no cross-CTA reduction at all:
-//   sweep = intra-block pairs of the two resident blocks (b-1 rounds)
-//         + 2C-1 outer rounds of a round-robin tournament over the blocks; in each, the CTA meets
-//           every row of its "top" block with every row of its "bot" block (b inner rounds of b
-//           disjoint pairs, one warp per pair, the top row kept in registers), then the blocks
-//           move one seat through distributed shared memory (pull into a spare slot, two
-//           cluster.syncs, relabel the slots -- no copy inside a CTA).
-// Every pair of rows meets exactly once per sweep, as in the cyclic one-sided Jacobi method.
-//  * Squared row norms travel with the rows and are updated in closed form after a rotation
-//    (aa' = aa - t ab, bb' = bb + t ab), so a pair costs ONE inner product (a.b) and one warp reduction; they
-//    are recomputed from the data once per sweep.
-//  * The number of rows is read on the device (numerical rank from the pivoted-QR preconditioner); only
-//    Ce = ceil(p / (2 bmax)) CTAs of the cluster take part, the others exit at once (cluster barriers wait
-//    for non-exited threads only).
-//  * Convergence: a sweep in which no pair had cos^2 > 1e-15 ends the iteration -- Jacobi converges
-//    quadratically, so after such a sweep the remaining cosines are O(1e-15).
-constexpr int BJ_NT = 512;
-constexpr int BJ_G = 32;
-constexpr int BJ_NGRP = BJ_NT / BJ_G;
-
-// shared memory: 3 slots of [bmax * pitchmax data | bme norms] | xch [2][MAXC] counts | fro [MAXC] | ints
-template <int EPL>
-__global__ void __launch_bounds__(BJ_NT) qtt_blockjacobi_kernel(const __grid_constant__ JacGroup g, int bmax,
-                                                                 int pitchmax) {
-  cg::cluster_group cluster = cg::this_cluster();
-  const int C = g.cluster;
-  const int rank = (C > 1) ? (int)cluster.block_rank() : 0;
-  const JacProb& P = g.p[blockIdx.x / C];
-  const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
-  // rows to rotate: the numerical rank found by the pivoted-QR preconditioner, if there is one
-  int p = P.p;
-  if (P.p_dev) p = min(p, P.p_dev[0]);
-  if (p < 2) return;  // uniform over the cluster: nothing to orthogonalise
-  const int Ce = max(1, (p + 2 * bmax - 1) / (2 * bmax));  // CTAs that take part (<= C)
-  if (rank >= Ce) return;
-  const int q = P.q;
-  constexpr int pitch = BJ_G * EPL;  // every row is zero-padded to the full lane footprint (== pitchmax)
-  const int b = (p + 2 * Ce - 1) / (2 * Ce);         // <= bmax
-
-  extern __shared__ __align__(16) double sm[];
-  const int bme = (bmax + 1) & ~1;
-  const size_t data_sz = (size_t)bmax * pitchmax;
-  const size_t slot_sz = data_sz + bme;
-  double* xch = sm + 3 * slot_sz;  // [2][MAXC] "big rotation" counts from peers
-  double* xfro = xch + 2 * MAXC;   // [MAXC]
-  int* cnt = reinterpret_cast<int*>(xfro + MAXC);
-  int top_s = 0, bot_s = 1, spare_s = 2;
-  auto slot = [&](int sidx) { return sm + (size_t)sidx * slot_sz; };
-
-  // ---- load: block k holds rows [k b, (k+1) b); CTA c starts with top = block c, bot = block 2Ce-1-c
-  double fro = 0.0;
-  for (int which = 0; which < 2; ++which) {
-    const int blk = which == 0 ? rank : 2 * Ce - 1 - rank;
-    double* S = slot(which == 0 ? top_s : bot_s);
-    for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
-      const int r = idx / pitch, x = idx - r * pitch;
-      const int gr = blk * b + r;
-      double v = 0.0;
-      if (gr < p && x < q) v = P.X[(i64)gr * P.ld + x];
-      S[idx] = v;
-      fro += v * v;
-    }
-  }
-  // Frobenius norm^2 over the cluster -> noise floor (rows below eps * ||X||_F / sqrt(p) are zero to
-  // working accuracy; they cannot all be made mutually orthogonal when p > rank)
-  fro = warp_sum1(fro);
-  if (tid == 0) cnt[0] = 0;
-  if (tid < MAXC) xfro[tid] = 0.0;
-  __syncthreads();
-  if (lane == 0) atomicAdd(&xfro[rank], fro);
-  __syncthreads();
-  if (Ce > 1) {
-    cluster.sync();  // peers have zeroed their xfro
-    if (tid < Ce && tid != rank) {
-      double* remote = cluster.map_shared_rank(xfro, tid);
-      remote[rank] = xfro[rank];
-    }
-    cluster.sync();
-  }
-  double fro2 = 0.0;
-  for (int c2 = 0; c2 < Ce; ++c2) fro2 += xfro[c2];
-  const double floor2 = 4.930380657631324e-32 * fro2 / (double)p;
-  const double tol = 2.220446049250313e-16 * sqrt((double)q);
-  const double tol2 = tol * tol;
-  __syncthreads();
-
-  const int be = b + (b & 1);  // players of the intra-block tournament
-  int sweep = 0, hit_limit = 0;
-  int mybig = 0;
-  for (; sweep < g.max_sweeps; ++sweep) {
-    // ---- fresh squared norms of the resident rows
-    for (int which = 0; which < 2; ++which) {
-      double* S = slot(which == 0 ? top_s : bot_s);
-      for (int r = grp; r < b; r += BJ_NGRP) {
-        const double* row = S + (size_t)r * pitch + lane;
-        double sq = 0.0;
-#pragma unroll
-        for (int e = 0; e < EPL; ++e)
-          sq += row[e * BJ_G] * row[e * BJ_G];
-        sq = warp_sum1(sq);
-        if (lane == 0) S[data_sz + r] = sq;
-      }
-    }
-    __syncthreads();
-    // ---- intra-block pairs of both resident blocks
-    for (int round = 0; round < be - 1; ++round) {
-      for (int k0 = 0; k0 < be; k0 += BJ_NGRP) {  // be pairs in all: be/2 per block
-        const int kk = k0 + grp;
-        int ia = b, ib = b;
-        double* S = slot(top_s);
-        if (kk < be) {
-          const int k = kk % (be / 2);
-          S = slot(kk < be / 2 ? top_s : bot_s);
-          if (k == 0) {
-            ia = be - 1;
-            ib = round;
-          } else {
-            ia = (round + k) % (be - 1);
-            ib = (round - k + (be - 1)) % (be - 1);
-          }
-        }
-        const bool live = ia < b && ib < b;
-        double a[EPL], v[EPL];
-        double ab = 0.0, ab2 = 0.0;
-        double* ra = S + (size_t)(live ? ia : 0) * pitch + lane;
-        double* rb = S + (size_t)(live ? ib : 0) * pitch + lane;
-        if (live) {
-#pragma unroll
-          for (int e = 0; e < EPL; ++e) {
-            a[e] = ra[e * BJ_G];
-            v[e] = rb[e * BJ_G];
-            if (e & 1) ab2 += a[e] * v[e];
-            else ab += a[e] * v[e];
-          }
-          ab += ab2;
-        }
-        ab = warp_sum1(ab);
-        if (live) {
-          const double aa = S[data_sz + ia], bb = S[data_sz + ib];
-          const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
-          if (R.apply) {
-#pragma unroll
-            for (int e = 0; e < EPL; ++e) {
-              ra[e * BJ_G] = R.c * a[e] - R.s * v[e];
-              rb[e * BJ_G] = R.s * a[e] + R.c * v[e];
-            }
-            if (lane == 0) {
-              S[data_sz + ia] = fmax(aa - R.t * ab, 0.0);
-              S[data_sz + ib] = fmax(bb + R.t * ab, 0.0);
-              if (R.big) ++mybig;
-            }
-          }
-        }
-      }
-      __syncthreads();
-    }
-    // ---- tournament over the 2Ce blocks
-    for (int t = 0; t < 2 * Ce - 1; ++t) {
-      double* T = slot(top_s);
-      double* B = slot(bot_s);
-      for (int i0 = 0; i0 < b; i0 += BJ_NGRP) {
-        const int i = i0 + grp;
-        const bool have = i < b;
-        double a[EPL];
-        double aa = 0.0;
-        double* rt = T + (have ? i : 0) * pitch + lane;
-        if (have) {
-#pragma unroll
-          for (int e = 0; e < EPL; ++e) a[e] = rt[e * BJ_G];
-          aa = T[data_sz + i];
-        }
-        int j = have ? i : 0;
-        for (int r = 0; r < b; ++r) {
-          double ab = 0.0, ab2 = 0.0, bb = 0.0;
-          double* rb = B + j * pitch + lane;
-          if (have) {
-            bb = B[data_sz + j];
-#pragma unroll
-            for (int e = 0; e < EPL; ++e) {
-              const double ve = rb[e * BJ_G];
-              if (e & 1) ab2 += a[e] * ve;
-              else ab += a[e] * ve;
-            }
-          }
-          ab = warp_sum1(ab + ab2);
-          if (have) {
-            const Rot R = jacobi_rotation(aa, bb, ab, tol2, floor2);
-            if (R.apply) {
-#pragma unroll
-              for (int e = 0; e < EPL; ++e) {  // the bottom row is read again: keeping it live costs spills
-                const double ve = rb[e * BJ_G];
-                const double an = R.c * a[e] - R.s * ve;
-                rb[e * BJ_G] = R.s * a[e] + R.c * ve;
-                a[e] = an;
-              }
-              aa = fmax(aa - R.t * ab, 0.0);
-              if (lane == 0) {
-                B[data_sz + j] = fmax(bb + R.t * ab, 0.0);
-                if (R.big) ++mybig;
-              }
-            }
-          }
-          j = (j + 1 == b) ? 0 : j + 1;
-          __syncthreads();
-        }
-        if (have) {
-#pragma unroll
-          for (int e = 0; e < EPL; ++e) rt[e * BJ_G] = a[e];
-          if (lane == 0) T[data_sz + i] = aa;
-        }
-      }
-      __syncthreads();
-      if (Ce == 1) break;
-      // ---- move the blocks one seat (labels of every peer are a function of the round number only)
-      const int tt = sweep * (2 * Ce - 1) + t;  // exchanges done so far
-      // peer labelling after tt relabels: CTA 0: top fixed at slot 0, (bot, spare) = tt even ? (1, 2) : (2, 1);
-      // CTA c >= 1: (top, bot, spare) = cyclic shifts of (0, 1, 2)
-      auto peer_top = [&](int c2) { return c2 == 0 ? 0 : (2 * tt) % 3; };
-      auto peer_bot = [&](int c2) { return c2 == 0 ? ((tt & 1) ? 2 : 1) : (2 * tt + 1) % 3; };
-      auto pull = [&](double* dst, const double* remote) {
-        for (int idx = tid * 2; idx < b * pitch; idx += BJ_NT * 2)
-          *reinterpret_cast<double2*>(dst + idx) = *reinterpret_cast<const double2*>(remote + idx);
-        for (int idx = tid; idx < b; idx += BJ_NT) dst[data_sz + idx] = remote[data_sz + idx];
-      };
-      cluster.sync();  // every CTA has finished rotating its blocks
-      // phase 1: new top <- old top of the left neighbour (CTA 1: old bot of CTA 0) into my spare slot
-      if (rank >= 1) {
-        const int src = rank - 1;
-        const int ss = (rank == 1) ? peer_bot(0) : peer_top(src);
-        pull(slot(spare_s), cluster.map_shared_rank(sm + (size_t)ss * slot_sz, src));
-      }
-      cluster.sync();
-      // phase 2: new bot <- old bot of the right neighbour (last CTA: its own old top, a relabel)
-      if (rank <= Ce - 2) {
-        const int src = rank + 1;
-        pull(slot(rank == 0 ? spare_s : top_s), cluster.map_shared_rank(sm + (size_t)peer_bot(src) * slot_sz, src));
-      }
-      cluster.sync();
-      if (rank == 0) {
-        const int ob = bot_s;
-        bot_s = spare_s;
-        spare_s = ob;
-      } else {
-        const int ot = top_s, ob = bot_s;
-        top_s = spare_s;
-        bot_s = ot;
-        spare_s = ob;
-      }
-    }
-    // ---- "big" rotations of this sweep over the whole cluster
-    if (lane == 0 && mybig) atomicAdd(&cnt[0], mybig);
-    mybig = 0;
-    __syncthreads();
-    int total = cnt[0];
-    if (Ce > 1) {
-      const int par = sweep & 1;
-      if (tid < Ce) {
-        double* remote = cluster.map_shared_rank(xch, tid);
-        remote[par * MAXC + rank] = (double)cnt[0];
-      }
-      cluster.sync();
-      total = 0;
-      for (int c2 = 0; c2 < Ce; ++c2) total += (int)xch[par * MAXC + c2];
-    }
-    __syncthreads();
-    if (tid == 0) cnt[0] = 0;
-    __syncthreads();
-    if (total == 0) {
-      ++sweep;
-      break;
-    }
-    if (sweep + 1 == g.max_sweeps) hit_limit = 1;
-  }
-  // ---- after whole sweeps every block is back in its first seat
-  for (int which = 0; which < 2; ++which) {
-    const int blk = which == 0 ? rank : 2 * Ce - 1 - rank;
-    const double* S = slot(which == 0 ? top_s : bot_s);
-    for (int idx = tid; idx < b * pitch; idx += BJ_NT) {
-      const int r = idx / pitch, x = idx - r * pitch;
-      const int gr = blk * b + r;
-      if (gr < p && x < q) P.X[(i64)gr * P.ld + x] = S[idx];
-    }
-  }
-  if (rank == 0 && tid == 0 && P.status) {
-    atomicMax(&P.status[0], sweep);
-    if (hit_limit) atomicAdd(&P.status[1], 1);
-  }
-  if (Ce > 1) cluster.sync();
-}
-
-// ------------------------------------------------------------------------------------------------
 // select: sort rows by norm (bitonic in shared memory), rank rule, normalised top rows.
 constexpr int SNT = 256;
 constexpr int SEL_MAXP = 16384;  // rows whose sort keys fit the opt-in shared memory (12 bytes per padded row)
@@ -589,54 +297,10 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
 
 }  // namespace
 
-namespace {
-template <int EPL>
-cudaError_t launch_blockjacobi(JacGroup& grp, int pmax, int qmax, int b, int pitch, size_t smem, double flops,
-                               cudaStream_t stream) {
-  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_blockjacobi_kernel<EPL>))) {
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        224 * 1024));
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_blockjacobi_kernel<EPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-  }
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grp.cluster * grp.nprob);
-  cfg.blockDim = dim3(BJ_NT);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = stream;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeClusterDimension;
-  at[0].val.clusterDim.x = grp.cluster;
-  at[0].val.clusterDim.y = 1;
-  at[0].val.clusterDim.z = 1;
-  cfg.attrs = at;
-  cfg.numAttrs = 1;
-  QttProf prof(QK_JACOBI, stream, flops, pmax, qmax, grp.nprob, grp.cluster);
-  return cudaLaunchKernelEx(&cfg, qtt_blockjacobi_kernel<EPL>, grp, b, pitch);
-}
-
-// Block-Jacobi configuration for a group with largest shape pmax x qmax; false if it does not fit.
-// One warp per row pair (EPL = elements per lane); C = ceil(p / 16) CTAs (at most 16) of two blocks of 8 rows each
-// for p <= 256 (measured ~10 % faster than 16-row blocks on half as many CTAs: two instead of four warps share an
-// fp64 pipe), 16-row blocks on 16 CTAs for p = 512.
-bool blockjacobi_config(int pmax, int qmax, int& EPL, int& C, int& b, int& pitch, size_t& smem) {
-  if (qmax <= 128) EPL = 4;
-  else if (qmax <= 256) EPL = 8;
-  else if (qmax <= 512) EPL = 16;
-  else return false;
-  pitch = BJ_G * EPL;
-  C = (pmax + 15) / 16;
-  C = C < 1 ? 1 : (C > MAXC ? MAXC : C);
-  b = (pmax + 2 * C - 1) / (2 * C);
-  smem = ((size_t)3 * ((size_t)b * pitch + ((b + 1) & ~1)) + 3 * MAXC + 2) * sizeof(double);
-  return smem <= 220 * 1024;
-}
-}  // namespace
-
 cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t stream) {
   // production path: the register-blocked cluster block Jacobi (bj2.cu); problems of one call (the operands of one
   // site, similar shapes) share launches
-  static const bool use_old = getenv("QTT_OLD_BJ") != nullptr;
-  if (!use_old) {
+  {
     bool all_fit = true;
     for (int i = 0; i < n && all_fit; ++i) {
       int EPL, BR, C;
@@ -662,53 +326,6 @@ cudaError_t qtt_launch_rowjacobi(const JacProb* probs, int n, cudaStream_t strea
         }
         if (grp.nprob == 0) continue;
         QTT_CHECK_CUDA(qtt_launch_bj2(grp, pmax, qmax, flops, stream));
-      }
-      return cudaSuccess;
-    }
-  }
-  if (use_old) {
-    int done = 0;
-    bool all_fit = true;
-    for (int i = 0; i < n && all_fit; ++i) {
-      int EPL, C, b, pitch;
-      size_t smem;
-      if (probs[i].p >= 2 && probs[i].q >= 1 && !blockjacobi_config(probs[i].p, probs[i].q, EPL, C, b, pitch, smem))
-        all_fit = false;
-    }
-    if (all_fit) {
-      while (done < n) {
-        JacGroup grp;
-        grp.nprob = 0;
-        int pmax = 0, qmax = 0;
-        double flops = 0.0;
-        while (done < n && grp.nprob < QTT_JAC_MAX_BATCH) {
-          const JacProb& pr = probs[done];
-          if (pr.p >= 2 && pr.q >= 1) {
-            const int pm = pr.p > pmax ? pr.p : pmax, qm = pr.q > qmax ? pr.q : qmax;
-            int EPL, C, b, pitch;
-            size_t smem;
-            if (grp.nprob > 0 && !blockjacobi_config(pm, qm, EPL, C, b, pitch, smem)) break;
-            grp.p[grp.nprob++] = pr;
-            pmax = pm;
-            qmax = qm;
-            double a = pr.p > pr.q ? pr.p : pr.q, bb = pr.p > pr.q ? pr.q : pr.p;
-            flops += 6.0 * a * bb * bb + 20.0 * bb * bb * bb;
-          }
-          ++done;
-        }
-        if (grp.nprob == 0) continue;
-        int EPL, C, b, pitch;
-        size_t smem;
-        blockjacobi_config(pmax, qmax, EPL, C, b, pitch, smem);
-        grp.cluster = C;
-        grp.use_smem = 1;
-        grp.wslice = 0;
-        grp.max_sweeps = 60;
-        cudaError_t e;
-        if (EPL == 4) e = launch_blockjacobi<4>(grp, pmax, qmax, b, pitch, smem, flops, stream);
-        else if (EPL == 8) e = launch_blockjacobi<8>(grp, pmax, qmax, b, pitch, smem, flops, stream);
-        else e = launch_blockjacobi<16>(grp, pmax, qmax, b, pitch, smem, flops, stream);
-        if (e != cudaSuccess) return e;
       }
       return cudaSuccess;
     }
