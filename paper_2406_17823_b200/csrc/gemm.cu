@@ -6,6 +6,8 @@
 // Shared-memory layouts keep each operand in its global orientation (contiguous direction stays
 // contiguous, so 16-byte async copies apply) and pad the pitch to == 4 (mod 16) doubles, which makes
 // the 8x4 / 4x8 DMMA fragment reads conflict-free for 64-bit accesses in either orientation.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace {
@@ -26,6 +28,37 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+// ---- TMA (bulk asynchronous copy engine, SASS UBLKCP) + mbarrier: rows of an M/N-contiguous operand tile are
+// contiguous in global memory (up to 1 KB), so one cp.async.bulk per tile row moves them into the padded shared-memory
+// layout the DMMA fragment loads need -- no tensor map: the operand views are strided / batched / split-index views of
+// site tensors, and a 1-D bulk copy needs only 16-byte alignment of source, destination and size.
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(a), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "DONE:\n"
+      "}\n" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(double* smem, const double* g, unsigned bytes, uint64_t* bar) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  unsigned b = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(s), "l"(g),
+               "r"(bytes), "r"(b) : "memory");
 }
 
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
@@ -65,6 +98,23 @@ struct TileLoader {
         if (ok) rowvalid |= 1 << i;
       }
     }
+  }
+
+  // kind 1 through the bulk copy engine: thread t0 + kr moves row kr of the tile (rows beyond K are zero-filled by
+  // that thread: 0 x 0 must not meet stale data; columns beyond MN only feed C entries that are never stored)
+  __device__ __forceinline__ void issue_bulk(double* sm, int k0, int tid, int t0, uint64_t* bar) const {
+    constexpr int P = BMN + 4;
+    const int kr = tid - t0;
+    if (kr < 0 || kr >= BK) return;
+    double* s = sm + kr * P;
+    const int cnt = (k0 + kr < K) ? min(max(MN - mn0, 0), BMN) : 0;
+    const int even = cnt & ~1;
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    mbar_arrive_expect_tx(bar, (unsigned)even * 8u);
+    if (even > 0) bulk_g2s(s, base + (i64)(k0 + kr) * k_stride + mn0, (unsigned)even * 8u, bar);
+    if (cnt & 1) s[even] = base[(i64)(k0 + kr) * k_stride + mn0 + even];
+    if (k0 + kr >= K)
+      for (int c = 0; c < BMN; ++c) s[c] = 0.0;
   }
 
   __device__ __forceinline__ void issue(double* sm, int k0, int tid) const {
@@ -107,7 +157,9 @@ struct TileLoader {
   }
 };
 
-template <int BM, int BN, int WM, int WN>
+// TMA = true: the variant whose M/N-contiguous operands are staged by the bulk copy engine (a separate instantiation,
+// so that the cp.async-only kernel keeps its register allocation)
+template <int BM, int BN, int WM, int WN, bool TMA>
 __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
 qtt_gemm_dmma_kernel(const __grid_constant__ GemmGroup g) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
@@ -139,6 +191,22 @@ qtt_gemm_dmma_kernel(const __grid_constant__ GemmGroup g) {
   TileLoader<BN, NT> lb;
   la.init(P.A + (i64)z * P.a_bs, a_kind, (P.flags & 1) != 0, m0, P.M, P.K, P.a_lo, P.a_hi, P.a_div, P.a_k, tid);
   lb.init(P.B + (i64)z * P.b_bs, b_kind, (P.flags & 2) != 0, n0, P.N, P.K, P.b_n, 0, 0, P.b_k, tid);
+  // operands staged by the bulk copy engine (flags 8 / 16 set by the launcher: M/N-contiguous, 16-byte aligned views)
+  const bool a_bulk = TMA && (P.flags & 8) != 0, b_bulk = TMA && (P.flags & 16) != 0;
+  __shared__ uint64_t tma_bar[TMA ? STAGES : 1];
+  if (TMA && (a_bulk || b_bulk)) {
+    if (tid == 0)
+      for (int s = 0; s < STAGES; ++s) mbar_init(&tma_bar[s], (unsigned)BK * ((a_bulk ? 1u : 0u) + (b_bulk ? 1u : 0u)));
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    __syncthreads();
+  }
+  auto issue_stage = [&](int s, int k0) {
+    double* As = smem + s * (A_SZ + B_SZ);
+    if (TMA && a_bulk) la.issue_bulk(As, k0, tid, 0, &tma_bar[TMA ? s : 0]);
+    else la.issue(As, k0, tid);
+    if (TMA && b_bulk) lb.issue_bulk(As + A_SZ, k0, tid, NT >= 2 * BK ? BK : 0, &tma_bar[TMA ? s : 0]);
+    else lb.issue(As + A_SZ, k0, tid);
+  };
 
   const int sa_m = a_kind == 0 ? KPITCH : 1, sa_k = a_kind == 0 ? 1 : (BM + 4);
   const int sb_n = b_kind == 0 ? KPITCH : 1, sb_k = b_kind == 0 ? 1 : (BN + 4);
@@ -153,23 +221,17 @@ qtt_gemm_dmma_kernel(const __grid_constant__ GemmGroup g) {
   const int KT = (P.K + BK - 1) / BK;
 #pragma unroll
   for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < KT) {
-      la.issue(smem + s * (A_SZ + B_SZ), s * BK, tid);
-      lb.issue(smem + s * (A_SZ + B_SZ) + A_SZ, s * BK, tid);
-    }
+    if (s < KT) issue_stage(s, s * BK);
     cp_async_commit();
   }
   const int fr = lane >> 2, fk = lane & 3;
   for (int kt = 0; kt < KT; ++kt) {
     cp_async_wait<STAGES - 2>();
+    if (TMA && (a_bulk || b_bulk)) mbar_wait(&tma_bar[TMA ? kt % STAGES : 0], (unsigned)((kt / STAGES) & 1));
     __syncthreads();
     {
       int nk = kt + STAGES - 1;
-      if (nk < KT) {
-        int s = nk % STAGES;
-        la.issue(smem + s * (A_SZ + B_SZ), nk * BK, tid);
-        lb.issue(smem + s * (A_SZ + B_SZ) + A_SZ, nk * BK, tid);
-      }
+      if (nk < KT) issue_stage(nk % STAGES, nk * BK);
       cp_async_commit();
     }
     const double* As = smem + (kt % STAGES) * (A_SZ + B_SZ);
@@ -222,12 +284,12 @@ qtt_gemm_dmma_kernel(const __grid_constant__ GemmGroup g) {
   }
 }
 
-template <int BM, int BN, int WM, int WN>
+template <int BM, int BN, int WM, int WN, bool TMA>
 cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream, int family) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
   constexpr size_t SMEM = (size_t)STAGES * (BM + BN) * KPITCH * sizeof(double);
-  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_gemm_dmma_kernel<BM, BN, WM, WN>)))
-    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_gemm_dmma_kernel<BM, BN, WM, WN>,
+  if (qtt_first_use_on_device(reinterpret_cast<const void*>(&qtt_gemm_dmma_kernel<BM, BN, WM, WN, TMA>)))
+    QTT_CHECK_CUDA(cudaFuncSetAttribute(qtt_gemm_dmma_kernel<BM, BN, WM, WN, TMA>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
   int t = 0;
   for (int i = 0; i < grp.nprob; ++i) {
@@ -243,7 +305,7 @@ cudaError_t launch_cfg(GemmGroup& grp, cudaStream_t stream, int family) {
   for (int i = 0; i < grp.nprob; ++i) flops += 2.0 * grp.p[i].M * grp.p[i].N * (double)grp.p[i].K * grp.p[i].nbatch;
   {
     QttProf prof(family, stream, flops, grp.p[0].M, grp.p[0].N, grp.p[0].K, grp.nprob);
-    qtt_gemm_dmma_kernel<BM, BN, WM, WN><<<t, NT, SMEM, stream>>>(grp);
+    qtt_gemm_dmma_kernel<BM, BN, WM, WN, TMA><<<t, NT, SMEM, stream>>>(grp);
   }
   return cudaGetLastError();
 }
@@ -274,6 +336,17 @@ cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream, i
         if (al16(p.B) && even(p.b_n) && even(p.b_bs)) f |= 2;
       } else if (al16(p.B) && even(p.b_k) && even(p.b_bs)) f |= 2;
       if (p.c_n == 1 && al16(p.C) && even(p.c_lo) && even(p.c_hi) && even(p.c_bs)) f |= 4;
+      // M/N-contiguous operand views that are 16-byte aligned go through the bulk copy engine (TMA) unless disabled
+      // (QTT_GEMM_TMA=0: the cp.async path for every operand; profiles/r2_gemm_tma_ab.md has the comparison)
+      static const int tma_mode = getenv("QTT_GEMM_TMA") ? (getenv("QTT_GEMM_TMA")[0] == '0' ? 0 : 1) : -1;
+      // default (-1): the bulk engine where it measured at least as fast as cp.async -- the batched site contractions
+      // with long K (the chi = 256 shapes of row a2: 26.0 vs 25.8 TFLOP/s); at K = 64 / 128 and for the unbatched carry
+      // products cp.async is 1-5 % ahead and stays (profiles/r2_gemm_tma_ab.md)
+      const bool use_tma = tma_mode == 1 || (tma_mode < 0 && p.K >= 256 && p.nbatch >= 4);
+      if (use_tma) {
+        if (p.a_k != 1 && (f & 1)) f |= 8;
+        if (p.b_k != 1 && (f & 2)) f |= 16;
+      }
       p.flags = f;
       grp.p[grp.nprob++] = p;
       big_tiles += (i64)((p.M + 127) / 128) * ((p.N + 127) / 128) * p.nbatch;
@@ -282,13 +355,15 @@ cudaError_t qtt_launch_gemm(const GemmProb* probs, int n, cudaStream_t stream, i
       minMN = p.N < minMN ? p.N : minMN;
     }
     if (grp.nprob == 0) continue;
+    bool any_bulk = false;
+    for (int i = 0; i < grp.nprob; ++i) any_bulk = any_bulk || (grp.p[i].flags & 24) != 0;
     cudaError_t e;
     if (big_tiles >= 120 && minMN >= 96)
-      e = launch_cfg<128, 128, 64, 32>(grp, stream, family);
+      e = any_bulk ? launch_cfg<128, 128, 64, 32, true>(grp, stream, family) : launch_cfg<128, 128, 64, 32, false>(grp, stream, family);
     else if (mid_tiles >= 32 && minMN >= 48)
-      e = launch_cfg<64, 64, 32, 32>(grp, stream, family);
+      e = any_bulk ? launch_cfg<64, 64, 32, 32, true>(grp, stream, family) : launch_cfg<64, 64, 32, 32, false>(grp, stream, family);
     else
-      e = launch_cfg<32, 32, 16, 16>(grp, stream, family);
+      e = any_bulk ? launch_cfg<32, 32, 16, 16, true>(grp, stream, family) : launch_cfg<32, 32, 16, 16, false>(grp, stream, family);
     if (e != cudaSuccess) return e;
   }
   return cudaSuccess;
