@@ -36,6 +36,7 @@ where the paper is silent/garbled and the reading taken):
       mpo_stencil (any order)   PAPER.md:98, same construction
   O11 fidelity, chi_eps         PAPER.md:160 Eq. 12; Eq. 16-17 (diagnostics)
       tke_spectrum              PAPER.md:173-184 Eq. 13-15
+  O12 variational_cost / variational_stage   PAPER.md:107-132 Sec. II.C; 437-452 Eq. B3-B6; 522-544 Eq. B20-B24
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
 grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
@@ -49,6 +50,8 @@ R' = Q^T T, ||T - Q R'||_F = the tail of an independent svdvals(T) beyond keep =
 (Eckart-Young), T_l = (Phi_{<l}^T (x) I_4) X_l with X_l from the explicit hadamard() cores, a planted spectrum
 with a gap at chi_work, and the projected dense product as the state handed to the R->L sweep; the eps rank
 rule by hand-computed tails, brute-force minimality and a case where the 1/sqrt(n-1) split decides the rank.
+O12 (variational stage) is pinned in tests/test_oracle_variational.py by the dense normal equations of Theta,
+finite-difference stationarity at truncating bonds and the dense operator product.
 """
 from __future__ import annotations
 
@@ -560,3 +563,155 @@ def chi_eps(cores, eps: float):
                 break
         out[k] = max(1, chi)
     return out, max(out)
+
+
+# ------------------------------------------- variational stage (Sec. II.C, App. B)
+def mpo_product(W1, W2):
+    """MPO of the operator product W1 W2 (W1 acts after W2): cores [(m1,m2)][w][w''][(m1',m2')]."""
+    out = []
+    for A, B in zip(W1, W2):
+        C = np.einsum("aopb,cpqd->acoqbd", A, B)
+        a, c, o, q, b, d = C.shape
+        out.append(C.reshape(a * c, o, q, b * d))
+    return out
+
+
+def variational_cost(v, a, Bm, D1, D2, h, mu):
+    """Theta of PAPER.md:452 Eq. B6 with the nonlinear part given as the MPS pair B (Eq. B21):
+    mu ||D1 v1 + D2 v2||^2 + sum_i ||(v_i - a_i)/h + B_i||^2, evaluated with exact MPS sums (no rounding)."""
+    div = lincomb([(1.0, apply_mpo(D1, v[0])), (1.0, apply_mpo(D2, v[1]))])
+    th = mu * float(np.linalg.norm(_sweep_lr(div)[-1])) ** 2
+    for i in range(2):
+        res = lincomb([(1.0 / h, v[i]), (-1.0 / h, a[i]), (1.0, Bm[i])])
+        th += float(np.linalg.norm(_sweep_lr(res)[-1])) ** 2
+    return th
+
+
+def _canonicalize_right(cores):
+    """Right-canonical form with the centre on site 1 (PAPER.md:498-518 Eq. B15-B19): QR sweeps only, bonds kept."""
+    C = [c.copy() for c in cores]
+    for k in range(len(C) - 1, 0, -1):
+        r0, d, r1 = C[k].shape
+        Q, R = np.linalg.qr(C[k].reshape(r0, d * r1).T)       # M^T = Q R  ->  M = R^T Q^T
+        C[k] = Q.T.reshape(-1, d, r1)
+        p0 = C[k - 1].shape[0]
+        C[k - 1] = (C[k - 1].reshape(p0 * d, r0) @ R.T).reshape(p0, d, -1)
+    return C
+
+
+def variational_stage(v0, a, Bm, D1, D2, h, mu, max_sweeps=20, sweep_tol=1e-5, cg_maxit=100, cg_tol=1e-5, info=None):
+    """One Euler-type stage of the paper's DMRG-like solver (Sec. II.C; App. B): minimise Theta (Eq. B6)
+    over the trial MPS pair v (bonds of v0 kept) by one-site sweeps.  At the canonical centre d the stationarity condition
+    Eq. B22 is the coupled linear system Eq. B23-B24,
+        C_i - mu h^2 sum_j <basis_i| D_i D_j |basis_j> C_j = <basis_i| a_i - h B_i>,     i = 1, 2,
+    (D^T = -D, so the operator is I + mu h^2 P^T (D^T D) P: symmetric positive definite), solved by
+    conjugate gradients from the current centre tensors, at most cg_maxit iterations or until ||r|| <= cg_tol ||rhs||
+    (100 iterations, 1e-5); the centre is then shifted by a QR factorisation and the environments are
+    updated.  A sweep runs the centre from site 1 to site n and back; the iteration stops when the
+    relative change of sum_i <v_i|v_i> between sweeps is below sweep_tol (1e-5 in the paper) or after max_sweeps.
+    Reading: the nonlinear part B_i of Eq. B21 enters as an MPS (formed by the hot-path primitives: -rhs with
+    the skew-symmetric convection), so its projection is a two-layer overlap instead of the paper's four-layer network."""
+    n = len(v0[0])
+    V = [_canonicalize_right(v0[0]), _canonicalize_right(v0[1])]
+    Dm = (D1, D2)
+    Wij = [[mpo_product(Dm[i], Dm[j]) for j in range(2)] for i in range(2)]
+    g = [lincomb([(1.0, a[i]), (-h, Bm[i])]) for i in range(2)]
+    # environments: LH[i][j][k] (r^i_k, m_k, r^j_k) of <v_i| D_i D_j |v_j> left of site k+1 / RH right of site k;
+    # LG[i][k] (r^i_k, rg_k) of <v_i| g_i>
+    one3, one2 = np.ones((1, 1, 1)), np.ones((1, 1))
+    LH = [[[None] * (n + 1) for _ in range(2)] for _ in range(2)]
+    RH = [[[None] * (n + 1) for _ in range(2)] for _ in range(2)]
+    LG = [[None] * (n + 1) for _ in range(2)]
+    RG = [[None] * (n + 1) for _ in range(2)]
+
+    def upd_left(k):
+        for i in range(2):
+            for j in range(2):
+                LH[i][j][k + 1] = np.einsum("amc,awb,mwxn,cxd->bnd", LH[i][j][k], V[i][k], Wij[i][j][k], V[j][k], optimize=True)
+            LG[i][k + 1] = np.einsum("ac,awb,cwd->bd", LG[i][k], V[i][k], g[i][k], optimize=True)
+
+    def upd_right(k):
+        for i in range(2):
+            for j in range(2):
+                RH[i][j][k] = np.einsum("bnd,awb,mwxn,cxd->amc", RH[i][j][k + 1], V[i][k], Wij[i][j][k], V[j][k], optimize=True)
+            RG[i][k] = np.einsum("bd,awb,cwd->ac", RG[i][k + 1], V[i][k], g[i][k], optimize=True)
+
+    for i in range(2):
+        for j in range(2):
+            LH[i][j][0], RH[i][j][n] = one3, one3
+        LG[i][0], RG[i][n] = one2, one2
+    for k in range(n - 1, 0, -1):
+        upd_right(k)
+
+    cg_its = []
+
+    def solve_site(d):
+        def op(x):
+            y = [x[0].copy(), x[1].copy()]
+            for i in range(2):
+                for j in range(2):
+                    y[i] = y[i] - mu * h * h * np.einsum("amc,mwxn,bnd,cxd->awb", LH[i][j][d], Wij[i][j][d], RH[i][j][d + 1],
+                                                         x[j], optimize=True)
+            return y
+        rhs_ = [np.einsum("ac,cwd,bd->awb", LG[i][d], g[i][d], RG[i][d + 1], optimize=True) for i in range(2)]
+        dot2 = lambda p, q: float(np.sum(p[0] * q[0]) + np.sum(p[1] * q[1]))
+        x = [V[0][d].copy(), V[1][d].copy()]
+        Ax = op(x)
+        r = [rhs_[i] - Ax[i] for i in range(2)]
+        p = [r[0].copy(), r[1].copy()]
+        rr = dot2(r, r)
+        bnorm = math.sqrt(dot2(rhs_, rhs_))
+        its = 0
+        while its < cg_maxit and math.sqrt(rr) > cg_tol * bnorm:
+            Ap = op(p)
+            alpha = rr / dot2(p, Ap)
+            for i in range(2):
+                x[i] = x[i] + alpha * p[i]
+                r[i] = r[i] - alpha * Ap[i]
+            rr_new = dot2(r, r)
+            beta = rr_new / rr
+            for i in range(2):
+                p[i] = r[i] + beta * p[i]
+            rr = rr_new
+            its += 1
+        cg_its.append(its)
+        V[0][d], V[1][d] = x[0], x[1]
+
+    def shift_right(d):
+        for i in range(2):
+            r0, dd, r1 = V[i][d].shape
+            Q, R = np.linalg.qr(V[i][d].reshape(r0 * dd, r1))
+            V[i][d] = Q.reshape(r0, dd, -1)
+            nr0, _, nr1 = V[i][d + 1].shape
+            V[i][d + 1] = (R @ V[i][d + 1].reshape(nr0, dd * nr1)).reshape(-1, dd, nr1)
+
+    def shift_left(d):
+        for i in range(2):
+            r0, dd, r1 = V[i][d].shape
+            Q, R = np.linalg.qr(V[i][d].reshape(r0, dd * r1).T)
+            V[i][d] = Q.T.reshape(-1, dd, r1)
+            p0 = V[i][d - 1].shape[0]
+            V[i][d - 1] = (V[i][d - 1].reshape(p0 * dd, r0) @ R.T).reshape(p0, dd, -1)
+
+    norm2 = lambda: float(np.sum(V[0][0] ** 2) + np.sum(V[1][0] ** 2))
+    prev = norm2()
+    sweeps = 0
+    for sweeps in range(1, max_sweeps + 1):
+        for d in range(n - 1):
+            solve_site(d)
+            shift_right(d)
+            upd_left(d)
+        solve_site(n - 1)
+        for d in range(n - 1, 0, -1):
+            shift_left(d)
+            upd_right(d)
+            solve_site(d - 1)
+        cur = norm2()
+        change = abs(cur - prev) / max(cur, 1e-300)
+        prev = cur
+        if change < sweep_tol:
+            break
+    if info is not None:
+        info["sweeps"] = sweeps
+        info["cg_iterations"] = cg_its
+    return V
