@@ -2,6 +2,7 @@
 // sweeps that sequence the kernels of common.cuh.  Everything here only ENQUEUES work on the context's
 // stream; with eps == 0 no call synchronises, so a whole RK4 step can be stream-captured.
 #pragma once
+#include <cstring>
 #include <string>
 #include <utility>
 #include <vector>
@@ -145,3 +146,37 @@ double* qtt_dot_view(qtt_ctx* ctx, const View& a, const View& b);  // device sca
 
 
 
+
+// ------------------------------------------------------------------------------------------ GEMM views (row-major)
+inline GemmProb gemm_base(const double* A, const double* B, double* C, int M, int N, int K) {
+  GemmProb p;
+  std::memset(&p, 0, sizeof(p));
+  p.A = A; p.B = B; p.C = C;
+  p.M = M; p.N = N; p.K = K;
+  p.nbatch = 1;
+  p.alpha = 1.0; p.beta = 0.0;
+  return p;
+}
+// plain row-major C(MxN, ldc) = A(MxK, lda) * B(KxN, ldb)
+inline GemmProb gemm_nn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_base(A, B, C, M, N, K);
+  p.a_lo = lda; p.a_k = 1;
+  p.b_k = ldb; p.b_n = 1;
+  p.c_lo = ldc; p.c_n = 1;
+  return p;
+}
+// C = A * B^T with B stored N x K (ldb)
+inline GemmProb gemm_nt(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_nn(A, lda, B, 0, C, ldc, M, N, K);
+  p.b_k = 1; p.b_n = ldb;
+  return p;
+}
+// C = A^T * B with A stored K x M (lda)
+inline GemmProb gemm_tn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
+  GemmProb p = gemm_nn(A, 0, B, ldb, C, ldc, M, N, K);
+  p.a_lo = 1; p.a_k = lda;
+  return p;
+}
+
+
+void qtt_row_space_basis(qtt_ctx* ctx, double* X, int p, int q, double* out);

@@ -204,8 +204,13 @@ constexpr int SNT = 256;
 constexpr int SEL_MAXP = 16384;  // rows whose sort keys fit the opt-in shared memory (12 bytes per padded row)
 
 // dynamic shared memory: key [np] doubles | idx [np] ints, np = rows padded to a power of two
-__global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__ SelGroup g, int npmax) {
-  const SelProb& P = g.p[blockIdx.x];
+// One cluster of S CTAs per matrix (S = 1 for small ones): the squared row norms are computed by slices of rows, one
+// slice per CTA, and all-gathered through distributed shared memory (a single CTA reading a 2 MB matrix out of L2 was
+// most of this kernel's time); every CTA then sorts the keys itself and writes its share of the output rows.
+__global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__ SelGroup g, int npmax, int S) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int crank = S > 1 ? (int)cluster.block_rank() : 0;
+  const SelProb& P = g.p[blockIdx.x / S];
   extern __shared__ __align__(16) double sel_sm[];
   double* key = sel_sm;
   int* idx = reinterpret_cast<int*>(sel_sm + npmax);
@@ -214,7 +219,10 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
   const int p = P.p, q = P.q;
   int np = 1;
   while (np < p) np <<= 1;
-  for (int r = warp; r < np; r += SNT / 32) {
+  for (int r = tid; r < np; r += SNT) idx[r] = r;
+  const int per = (np + S - 1) / S;
+  const int r_end = min(np, (crank + 1) * per);
+  for (int r = crank * per + warp; r < r_end; r += SNT / 32) {
     double s = 0.0;
     if (r < p)
       for (int x = lane; x < q; x += 32) {
@@ -222,11 +230,14 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
         s += v * v;
       }
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == 0) {
-      key[r] = (r < p) ? s : -1.0;
-      idx[r] = r;
+    const double kv = (r < p) ? s : -1.0;
+    if (S > 1) {
+      if (lane < S) cluster.map_shared_rank(key, lane)[r] = kv;
+    } else if (lane == 0) {
+      key[r] = kv;
     }
   }
+  if (S > 1) cluster.sync();
   __syncthreads();
   // bitonic sort, descending by key (ties: lower row index first, for determinism)
   for (int k2 = 2; k2 <= np; k2 <<= 1)
@@ -250,8 +261,9 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
     const int mn = p < q ? p : q;
     int r = P.chi_max < mn ? P.chi_max : mn;
     double tot = 0.0;
-    for (int i = p - 1; i >= 0; --i) tot += key[i];
-    if (P.delta_out) *P.delta_out = P.delta_scale * sqrt(tot);
+    if (P.delta_out)  // (only the first SVD of an eps > 0 sweep needs ||X||_F)
+      for (int i = p - 1; i >= 0; --i) tot += key[i];
+    if (P.delta_out && crank == 0) *P.delta_out = P.delta_scale * sqrt(tot);
     double delta = -1.0;
     if (P.delta_ptr) delta = *P.delta_ptr;
     else if (P.delta_out) delta = P.delta_scale * sqrt(tot);
@@ -273,13 +285,13 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
     if (r > P.r_cap) r = P.r_cap;
     if (r < 1) r = 1;
     s_rank = r;
-    if (P.rank) P.rank[0] = r;
+    if (P.rank && crank == 0) P.rank[0] = r;
   }
   __syncthreads();
   const int r = s_rank;
-  if (P.sigma)
+  if (P.sigma && crank == 0)
     for (int i = tid; i < p; i += SNT) P.sigma[i] = sqrt(fmax(key[i], 0.0));
-  for (int j = warp; j < P.r_cap; j += SNT / 32) {
+  for (int j = crank * (SNT / 32) + warp; j < P.r_cap; j += S * (SNT / 32)) {
     double inv = 0.0;
     int src = 0;
     if (j < r) {
@@ -437,11 +449,25 @@ cudaError_t qtt_launch_select(const SelProb* probs, int n, cudaStream_t stream) 
                                           (int)((size_t)SEL_MAXP * (sizeof(double) + sizeof(int)))));
     double bytes = 0.0;
     for (int i = 0; i < g.nprob; ++i) bytes += 8.0 * ((double)g.p[i].p * g.p[i].q + (double)g.p[i].r_cap * g.p[i].q);
+    int pmaxrows = 0;
+    for (int i = 0; i < g.nprob; ++i) pmaxrows = g.p[i].p > pmaxrows ? g.p[i].p : pmaxrows;
+    const int S = pmaxrows >= 64 ? 8 : 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(g.nprob * S);
+    cfg.blockDim = dim3(SNT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = S;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
     {
       QttProf prof(QK_SELECT, stream, bytes, g.p[0].p, g.p[0].q, g.nprob, 0);
-      qtt_select_kernel<<<g.nprob, SNT, smem, stream>>>(g, npmax);
+      QTT_CHECK_CUDA(cudaLaunchKernelEx(&cfg, qtt_select_kernel, g, npmax, S));
     }
-    QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;
 }

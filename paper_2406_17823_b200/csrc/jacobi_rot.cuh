@@ -20,37 +20,44 @@ __device__ __forceinline__ double rsqrt_pos(double x) {
 }
 
 // Rotation that orthogonalises two rows with Gram entries (aa, bb, ab):  a' = c a - s b,  b' = s a + c b, the small
-// angle (|tan| <= 1).  With D = bb - aa and H = sqrt(D^2 + 4 ab^2):  cos 2theta = |D| / H, sin 2theta = 2 |ab| / H,
-// c^2 = (1 + cos 2theta) / 2, s = sign(D ab) sin 2theta / (2 c), t = s / c.  Only two reciprocal square roots, no
-// divide; the operands are first scaled by a power of two so that the fourth powers of the row norms neither
-// overflow nor underflow.  c^2 + s^2 = 1 to rounding (what backward stability needs); the angle itself is accurate
-// to a few ulps.
+// angle (|t| <= 1, t = tan theta).  With D = bb - aa, X = 2 ab and H = sqrt(D^2 + X^2):
+//     t = sign(D ab) |X| / (H + |D|)      (= sin 2theta / (1 + cos 2theta)),      c = 1 / sqrt(1 + t^2),      s = c t.
+// Orthogonality (c^2 + s^2 = 1 to rounding, what backward stability needs) rests on the ONE full-accuracy reciprocal
+// square root that gives c; t itself only has to be a good angle -- an error of 1e-13 in it leaves a residual inner
+// product of that relative size, which the quadratically convergent iteration removes in the next sweep -- so H and the
+// reciprocal take one Newton step from the hardware seeds.  The Gram entries are first multiplied by an approximate
+// 1 / max(aa, bb) (hardware seed, any scale factor would do) so that no square over- or underflows.  Straight-line code:
+// two rotations computed back to back interleave in the instruction stream.
 __device__ __forceinline__ Rot jacobi_rotation(double aa, double bb, double ab, double tol2, double floor2) {
-  // straight-line code (no early exit): two rotations computed back to back interleave in the instruction stream
   Rot r;
-  const double ab2 = ab * ab, nn = aa * bb;
-  // power-of-two scale 2^-e, e = exponent of max(aa, bb): exact, keeps D^2 + 4 ab^2 in range
   const double m = fmax(aa, bb);
-  const int hi = __double2hiint(m) & 0x7ff00000;
-  // pairs already orthogonal to working accuracy, rows in the noise floor, subnormal / huge / inf / nan norms: skip
-  const bool ok = (ab2 > tol2 * nn) && (aa > floor2) && (bb > floor2) && hi != 0 && hi < 0x7fe00000;
-  const double sc = __hiloint2double(0x7fe00000 - hi, 0);
-  const double a1 = aa * sc, b1 = bb * sc, x1 = ab * sc;
+  double rm;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rm) : "d"(m));
+  const double a1 = aa * rm, b1 = bb * rm, x1 = ab * rm;
+  const double x2 = x1 * x1;
+  // pairs already orthogonal to working accuracy, rows in the noise floor, zero / inf / nan norms: skip
+  const bool ok = (x2 > tol2 * (a1 * b1)) && (aa > floor2) && (bb > floor2);
   const double d = b1 - a1;
-  const double h2 = fma(d, d, 4.0 * x1 * x1);
-  const double rh = rsqrt_pos(h2);
-  const double cos2 = fabs(d) * rh, sin2 = 2.0 * fabs(x1) * rh;
-  const double c2 = fma(0.5, cos2, 0.5);  // in [1/2, 1]
-  const double rc = rsqrt_pos(c2);
-  const double sg = copysign(0.5, d) * copysign(1.0, ab);
-  const double hs = sg * sin2 * rc;  // s = sin 2theta / (2 c)
-  const double c = c2 * rc;
-  const bool fin = ok && (c == c) && (hs == hs) && hs != 0.0;
-  r.c = fin ? c : 1.0;
-  r.s = fin ? hs : 0.0;
-  r.t = fin ? hs * rc : 0.0;
+  const double h2 = fma(d, d, 4.0 * x2);
+  double rh;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(rh) : "d"(h2));
+  rh = rh * fma(-(0.5 * h2 * rh), rh, 1.5);
+  const double den = fma(h2, rh, fabs(d));  // H + |D|
+  double rd;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rd) : "d"(den));
+  rd = fma(rd, fma(-den, rd, 1.0), rd);
+  // sign(D ab) 2 |x1| / den
+  const double ta = (fabs(x1) + fabs(x1)) * rd;
+  const int sgn = (__double2hiint(d) ^ __double2hiint(ab)) & 0x80000000;
+  const double t = __hiloint2double(__double2hiint(ta) | sgn, __double2loint(ta));
+  const double c = rsqrt_pos(fma(t, t, 1.0));
+  const double sn = c * t;
+  const bool fin = ok && (sn == sn) && (c == c) && sn != 0.0;
+  r.c = c;
+  r.s = sn;
+  r.t = t;
   r.apply = fin;
-  r.big = fin && ab2 > 1e-15 * nn;
+  r.big = fin && x2 > 1e-15 * (a1 * b1);
   return r;
 }
 __device__ __forceinline__ double warp_sum1(double v) {

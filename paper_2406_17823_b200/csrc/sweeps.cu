@@ -54,36 +54,6 @@ void qtt_zip_caps(const std::vector<int>& ra, const std::vector<int>& rb, int ch
 // ------------------------------------------------------------------------------------------ helpers
 namespace {
 
-GemmProb gemm_base(const double* A, const double* B, double* C, int M, int N, int K) {
-  GemmProb p;
-  std::memset(&p, 0, sizeof(p));
-  p.A = A; p.B = B; p.C = C;
-  p.M = M; p.N = N; p.K = K;
-  p.nbatch = 1;
-  p.alpha = 1.0; p.beta = 0.0;
-  return p;
-}
-// plain row-major C(MxN, ldc) = A(MxK, lda) * B(KxN, ldb)
-GemmProb gemm_nn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
-  GemmProb p = gemm_base(A, B, C, M, N, K);
-  p.a_lo = lda; p.a_k = 1;
-  p.b_k = ldb; p.b_n = 1;
-  p.c_lo = ldc; p.c_n = 1;
-  return p;
-}
-// C = A * B^T with B stored N x K (ldb)
-GemmProb gemm_nt(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
-  GemmProb p = gemm_nn(A, lda, B, 0, C, ldc, M, N, K);
-  p.b_k = 1; p.b_n = ldb;
-  return p;
-}
-// C = A^T * B with A stored K x M (lda)
-GemmProb gemm_tn(const double* A, i64 lda, const double* B, i64 ldb, double* C, i64 ldc, int M, int N, int K) {
-  GemmProb p = gemm_nn(A, 0, B, ldb, C, ldc, M, N, K);
-  p.a_lo = 1; p.a_k = lda;
-  return p;
-}
-
 void run_gemms(qtt_ctx* ctx, std::vector<GemmProb>& v) {
   if (v.empty()) return;
   QTT_CU(qtt_launch_gemm(v.data(), (int)v.size(), ctx->stream));
@@ -393,6 +363,23 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
 }
 
 }  // namespace
+
+// Orthonormal basis of the row space of X (p x q, ld = q, destroyed): out (min(p, q) x q, ld = q) <- the right singular
+// vectors of X as rows, in the order of decreasing singular value (rows belonging to singular values in the noise floor
+// are zeros).  The SVD step of the sweeps on its own, for callers that move a canonical centre (variational.cu).
+void qtt_row_space_basis(qtt_ctx* ctx, double* X, int p, int q, double* out) {
+  std::vector<SvdJob> svd(1);
+  SvdJob& j = svd[0];
+  j.X = X; j.p = p; j.q = q;
+  j.out = out;
+  j.r_cap = std::min(p, q);
+  j.chi_max = j.r_cap;
+  j.sigma = nullptr;
+  j.rank = reinterpret_cast<int*>(ctx->arena.tmp(1));
+  j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
+  j.rank_deficient = true;
+  run_svd(ctx, svd);
+}
 
 // ------------------------------------------------------------------------------------------ O6
 void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, double eps, std::vector<OutMps>& out,
