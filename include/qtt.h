@@ -170,6 +170,26 @@ qtt_status qtt_mps_fidelity(qtt_ctx* ctx, const qtt_mps* a, const qtt_mps* b, do
  * truncation error sqrt(sum_{i > chi_l} sigma_i^2) / ||x|| <= eps, written to chi_host[l] (n+1 ints, ends = 1), and
  * chi = max_l chi_l to *chi_max_host (may be NULL).  Synchronous. */
 qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_host, int* chi_max_host);
+/* ---- The variational stage of the paper's own solver (Sec. II.C, App. B).
+ * Theta(v) = mu ||D1 v_1 + D2 v_2||^2 + sum_i ||(v_i - a_i) / h + B_i||^2   (PAPER.md:452 Eq. B6; mu: the
+ * incompressibility penalty; a: the state the stage starts from, h: the stage's time increment, B: the
+ * nonlinear part Eq. B21 given as an MPS pair, e.g. minus the right-hand side formed by the hot-path primitives),
+ * evaluated with exact MPS sums and overlaps.  Handles of any kind; *theta_host is written after a synchronisation. */
+qtt_status qtt_variational_cost(qtt_ctx* ctx, const qtt_mps* const v[2], const qtt_mps* const a[2], const qtt_mps* const B[2],
+                                const qtt_mpo* D1, const qtt_mpo* D2, double h, double mu, double* theta_host);
+/* Minimises Theta over the MPS pair v (in-out; its bonds are kept, or shrink where a bond exceeds what its neighbours
+ * allow) by one-site sweeps, site 1 -> n -> 1 per sweep: at the canonical centre the stationarity condition
+ * Eq. B22 is the symmetric positive definite system Eq. B23-B24, C_i - mu h^2 sum_j <basis_i|D_i D_j|basis_j> C_j =
+ * <basis_i|a_i - h B_i>, solved by conjugate gradients from the current centre tensors until ||r|| <= cg_tol ||rhs|| or
+ * cg_maxit iterations (the paper: 1e-5, 100); the iteration stops when sum_i <v_i|v_i> changes by less than sweep_tol
+ * (relative) between sweeps, or after max_sweeps.  D1, D2 must be antisymmetric first-derivative MPOs.
+ * Environments and the local operator are DMMA GEMMs; the CG loop is driven from the host (synchronous call, two scalar
+ * read-backs per iteration; not captured into a graph).  Host outputs (each may be NULL): sweeps done, CG iterations in
+ * total, most CG iterations of one local solve.  On error v is untouched. */
+qtt_status qtt_variational_stage(qtt_ctx* ctx, qtt_mps* const v[2], const qtt_mps* const a[2], const qtt_mps* const B[2],
+                                 const qtt_mpo* D1, const qtt_mpo* D2, double h, double mu, int max_sweeps, double sweep_tol,
+                                 int cg_maxit, double cg_tol, int* sweeps_host, long long* cg_iterations_host,
+                                 int* cg_max_host);
 /* PAPER.md:173-184 Eq. 13-15: turbulent-kinetic-energy spectrum.  With u_i' = u_i - mean_i (mean_i == NULL: zero mean; Eq. 14)
  * and the Fourier coefficients u_i'^(k) = (1/N^2) sum_x u_i'(x) exp(-2 pi i k.x), k in [-N/2, N/2)^2 (Eq. 13):
  *   E_host[b] = 1/2 sum over the shell round(|k|) = b of (|u_1'^(k)|^2 + |u_2'^(k)|^2),  b = 0 .. nbins-1  (Eq. 15),

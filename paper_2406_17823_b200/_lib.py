@@ -65,6 +65,9 @@ PROTOTYPES = {
     "qtt_mps_fidelity": (C.c_int, [_P, _P, _P, _DP]),
     "qtt_mps_chi_eps": (C.c_int, [_P, _P, C.c_double, _IP, _IP]),
     "qtt_tke_spectrum": (C.c_int, [_P, _P, _P, _P, _P, C.c_int, _DP]),
+    "qtt_variational_cost": (C.c_int, [_P, _PP, _PP, _PP, _P, _P, C.c_double, C.c_double, _DP]),
+    "qtt_variational_stage": (C.c_int, [_P, _PP, _PP, _PP, _P, _P, C.c_double, C.c_double, C.c_int, C.c_double, C.c_int,
+                                        C.c_double, _IP, C.POINTER(C.c_longlong), _IP]),
     "qtt_mps_clone": (C.c_int, [_P, _P, _PP]),
     "qtt_mps_free": (None, [_P]),
     # include/qtt_diag.h

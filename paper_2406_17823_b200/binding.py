@@ -224,6 +224,28 @@ def qtt_rk4_step(ctx: Context, u: Sequence[Mps], Dx: Mpo, Dy: Mpo, Lap: Mpo, Re:
     ctx.check(ctx.lib.qtt_rk4_step(ctx.h, arr, Dx.h, Dy.h, Lap.h, float(Re), float(dt), int(chi_max), float(eps)))
 
 
+def qtt_variational_cost(ctx: Context, v: Sequence[Mps], a: Sequence[Mps], B: Sequence[Mps], D1: Mpo, D2: Mpo, h: float,
+                         mu: float) -> float:
+    """Theta of PAPER.md Eq. B6."""
+    out = C.c_double()
+    pair = lambda x: (C.c_void_p * 2)(x[0].h, x[1].h)
+    ctx.check(ctx.lib.qtt_variational_cost(ctx.h, pair(v), pair(a), pair(B), D1.h, D2.h, float(h), float(mu), C.byref(out)))
+    return out.value
+
+
+def qtt_variational_stage(ctx: Context, v: Sequence[Mps], a: Sequence[Mps], B: Sequence[Mps], D1: Mpo, D2: Mpo, h: float,
+                          mu: float, max_sweeps: int = 20, sweep_tol: float = 1e-5, cg_maxit: int = 100,
+                          cg_tol: float = 1e-5) -> dict:
+    """One stage of the paper's variational solver (Sec. II.C, App. B); v is updated in place.  Returns the
+    counters the library reports: sweeps, CG iterations in total, most CG iterations of one local solve."""
+    sw, mx, tot = C.c_int(), C.c_int(), C.c_longlong()
+    pair = lambda x: (C.c_void_p * 2)(x[0].h, x[1].h)
+    ctx.check(ctx.lib.qtt_variational_stage(ctx.h, pair(v), pair(a), pair(B), D1.h, D2.h, float(h), float(mu), int(max_sweeps),
+                                            float(sweep_tol), int(cg_maxit), float(cg_tol), C.byref(sw), C.byref(tot),
+                                            C.byref(mx)))
+    return {"sweeps": sw.value, "cg_iterations": tot.value, "cg_max": mx.value}
+
+
 # ------------------------------------------------------------------ inspection
 def qtt_mps_bonds(x: Mps) -> list[int]:
     n = x.ctx.lib.qtt_mps_num_sites(x.h)

@@ -951,6 +951,67 @@ qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_
   return QTT_OK;
 }
 
+// ------------------------------------------------------------------------------------------ variational stage
+qtt_status qtt_variational_cost(qtt_ctx* ctx, const qtt_mps* const v[2], const qtt_mps* const a[2], const qtt_mps* const B[2],
+                                const qtt_mpo* D1, const qtt_mpo* D2, double h, double mu, double* theta_host) {
+  if (!ctx || !v || !a || !B || !D1 || !D2 || !theta_host || !(h > 0.0) || mu < 0.0) return QTT_INVALID_ARG;
+  for (int i = 0; i < 2; ++i)
+    if (!v[i] || !a[i] || !B[i]) return QTT_INVALID_ARG;
+  QTT_API_BEGIN
+  set_device(ctx);
+  ArenaScope scope(ctx);
+  View vv[2], va[2], vb[2];
+  for (int i = 0; i < 2; ++i) {
+    vv[i] = materialize(ctx, v[i]->body);
+    va[i] = materialize(ctx, a[i]->body);
+    vb[i] = materialize(ctx, B[i]->body);
+    if (vv[i].n != D1->data->n || va[i].n != vv[i].n || vb[i].n != vv[i].n || D2->data->n != vv[i].n)
+      QTT_THROW(QTT_SHAPE_MISMATCH, "operands differ in length");
+  }
+  *theta_host = qtt_variational_cost_impl(ctx, vv, va, vb, D1->data, D2->data, h, mu);
+  QTT_API_END(ctx)
+}
+
+qtt_status qtt_variational_stage(qtt_ctx* ctx, qtt_mps* const v[2], const qtt_mps* const a[2], const qtt_mps* const B[2],
+                                 const qtt_mpo* D1, const qtt_mpo* D2, double h, double mu, int max_sweeps, double sweep_tol,
+                                 int cg_maxit, double cg_tol, int* sweeps_host, long long* cg_iterations_host,
+                                 int* cg_max_host) {
+  if (!ctx || !v || !a || !B || !D1 || !D2 || !(h > 0.0) || mu < 0.0 || max_sweeps < 1 || cg_maxit < 0 || sweep_tol < 0.0 ||
+      cg_tol < 0.0)
+    return QTT_INVALID_ARG;
+  for (int i = 0; i < 2; ++i)
+    if (!v[i] || !a[i] || !B[i]) return QTT_INVALID_ARG;
+  QTT_API_BEGIN
+  set_device(ctx);
+  ArenaScope scope(ctx);
+  View vv[2], va[2], vb[2];
+  for (int i = 0; i < 2; ++i) {
+    vv[i] = materialize(ctx, v[i]->body);
+    va[i] = materialize(ctx, a[i]->body);
+    vb[i] = materialize(ctx, B[i]->body);
+  }
+  Body* fresh[2] = {nullptr, nullptr};
+  try {
+    OutMps out[2];
+    for (int i = 0; i < 2; ++i) {
+      fresh[i] = body_new_dense(ctx, vv[i].r);
+      out[i] = out_of_body(fresh[i]);
+    }
+    qtt_variational_stage_impl(ctx, vv, va, vb, D1->data, D2->data, h, mu, max_sweeps, sweep_tol, cg_maxit, cg_tol, out,
+                               sweeps_host, cg_iterations_host, cg_max_host);
+    for (int i = 0; i < 2; ++i) body_set_bonds(fresh[i], out[i].r);
+  } catch (...) {
+    for (Body* b : fresh) body_release(b);
+    throw;
+  }
+  for (int i = 0; i < 2; ++i) {
+    body_release(v[i]->body);
+    v[i]->body = fresh[i];
+  }
+  check_numeric(ctx);
+  QTT_API_END(ctx)
+}
+
 // ------------------------------------------------------------------------------------------ diagnostics
 int qtt_diag_gemm(void* stream, const double* A, const double* B, double* C, int M, int N, int K, int transA,
                   int transB, long long lda, long long ldb, long long ldc, double alpha, double beta, int nbatch,

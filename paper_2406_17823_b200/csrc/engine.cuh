@@ -180,3 +180,11 @@ inline GemmProb gemm_tn(const double* A, i64 lda, const double* B, i64 ldb, doub
 
 
 void qtt_row_space_basis(qtt_ctx* ctx, double* X, int p, int q, double* out);
+
+// The variational stage (variational.cu; Sec. II.C, App. B): out[i].core slots sized for the bonds of v0[i].
+void qtt_variational_stage_impl(qtt_ctx* ctx, const View v0[2], const View a[2], const View Bm[2], const MpoData* D1,
+                                const MpoData* D2, double h, double mu, int max_sweeps, double sweep_tol, int cg_maxit,
+                                double cg_tol, OutMps out[2], int* sweeps_out, long long* cg_total, int* cg_max);
+double qtt_variational_cost_impl(qtt_ctx* ctx, const View v[2], const View a[2], const View Bm[2], const MpoData* D1,
+                                 const MpoData* D2, double h, double mu);
+
