@@ -524,6 +524,76 @@ def primitive_sweep(args):
     return 0
 
 
+def variational_bench(args):
+    """one stage of the paper's variational solver (Sec. II.C, App. B) at the bench
+    workload's shape (config 3: 2^10 x 2^10, chi = 64) with the paper's settings (mu = 25e4, <= 20 sweeps, CG <= 100
+    iterations / 1e-5): a = the initial state, B = the convective right-hand side formed by the hot-path primitives,
+    v0 = a (plus a 2 % compressible disturbance of u_y).  The stage is host-driven (scalar read-backs inside CG), so it is timed by wall clock around the synchronous
+    call, after one warm-up stage.  Prints ONE JSON line."""
+    import torch
+    import paper_2406_17823_b200 as Q
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    c, desc = workload(args.config)
+    n, chi = c["n"], c["chi"]
+    ctx = Q.Context(device=0, workspace_bytes=int(args.workspace_gib * (1 << 30)))
+    dx = 1.0 / (1 << n)
+    Dx, Dy = Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx)
+    ux, uy = I.config_fields(args.config)
+    # the bench state is divergence-free by construction (the penalty would have nothing to do: zero CG iterations at the
+    # paper's tolerance); a compressible disturbance of 2 % gives the stage the work it has inside a real time step
+    X, Y = I.grid(n)
+    uy = uy + 0.02 * np.sin(2 * np.pi * X) * np.cos(4 * np.pi * Y)
+    a = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
+    # B_i = sum_j u_j (.) D_j u_i, rounded to chi (the nonlinear part of Eq. B21 in convective form)
+    B = []
+    for i in range(2):
+        terms = []
+        for j, D in enumerate((Dx, Dy)):
+            g = Q.qtt_apply_mpo(ctx, D, a[i])
+            Q.qtt_round(ctx, g, chi)
+            prod = Q.qtt_hadamard(ctx, a[j], g)
+            Q.qtt_round(ctx, prod, chi)
+            terms.append(prod)
+        Q.qtt_axpy(ctx, 1.0, terms[0], terms[1])
+        Q.qtt_round(ctx, terms[1], chi)
+        B.append(terms[1])
+    mu, h = 25e4, c["dt"]
+    peaks = fp64_peaks(Q, ctx)
+    times, infos = [], []
+    th0 = Q.qtt_variational_cost(ctx, a, a, B, Dx, Dy, h, mu)
+    for rep in range(1 + max(args.steps, 1)):
+        v = [Q.qtt_mps_clone(ctx, x) for x in a]
+        if rep == 1:
+            Q.qtt_ctx_profile(ctx, True)
+            Q.qtt_ctx_profile_report(ctx)
+        ctx.synchronize()
+        t0 = time.perf_counter()
+        info = Q.qtt_variational_stage(ctx, v, a, B, Dx, Dy, h, mu)
+        ctx.synchronize()
+        if rep >= 1:
+            times.append(time.perf_counter() - t0)
+            infos.append(info)
+        if rep == 1:
+            rep1 = Q.qtt_ctx_profile_report(ctx)
+            Q.qtt_ctx_profile(ctx, False)
+            th1 = Q.qtt_variational_cost(ctx, v, a, B, Dx, Dy, h, mu)
+    sec = float(np.median(times))
+    g = rep1["gemm"]
+    line = {"metric": "variational stage (PAPER.md Sec. II.C) at 2^%d x 2^%d, chi=%d fp64" % (n, n, chi), "value": 1.0 / sec,
+            "unit": "stages/s", "ms_per_stage": sec * 1e3, "n_gpus": 1, "steps": len(times), "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "mu": mu, "h": h, "max_sweeps": 20, "sweep_tol": 1e-5, "cg_maxit": 100, "cg_tol": 1e-5,
+                       "timing": "wall clock around the synchronous call (profiled repetition excluded from nothing: event "
+                                 "pairs per launch are on during the first timed repetition only)"},
+            "solver": infos[-1], "theta_before": th0, "theta_after": th1,
+            "family_ms": {k: round(vv["ms"], 3) for k, vv in rep1.items()},
+            "gemm_tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12,
+            "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"],
+            "launches_per_stage": int(sum(vv["launches"] for vv in rep1.values())), "fp64_peaks_tflops": peaks}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     """Per-kernel-family device times of one more (eagerly launched, event-bracketed) step -> roofline of the
     dominant family; the site-contraction TFLOP/s; and the CPU oracle timed on a bounded sample."""
@@ -657,6 +727,8 @@ def main():
                          "batch 6, with each primitive's roofline fraction, instead of the RK4 step")
     ap.add_argument("--convection", default="convective", choices=("convective", "skew"),
                     help="convective (BASELINE.json's configs, default) or the paper's skew-symmetric form (Eq. B2)")
+    ap.add_argument("--variational", action="store_true",
+                    help="time one stage of the paper's variational solver (SURVEY.md section 8f next-1) at the workload's shape")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
                     help="only run the row-a2 site-contraction GEMM passes at the bulk-site shapes of bond CHI and "
                          "print their TFLOP/s (the command the ncu capture in profiles/ is taken on)")
@@ -667,6 +739,8 @@ def main():
         return run_reference(args)
     if args.primitive_sweep:
         return primitive_sweep(args)
+    if args.variational:
+        return variational_bench(args)
     if args.probe_contraction:
         import torch
         import paper_2406_17823_b200 as Q

@@ -174,7 +174,9 @@ qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_
  * Theta(v) = mu ||D1 v_1 + D2 v_2||^2 + sum_i ||(v_i - a_i) / h + B_i||^2   (PAPER.md:452 Eq. B6; mu: the
  * incompressibility penalty; a: the state the stage starts from, h: the stage's time increment, B: the
  * nonlinear part Eq. B21 given as an MPS pair, e.g. minus the right-hand side formed by the hot-path primitives),
- * evaluated with exact MPS sums and overlaps.  Handles of any kind; *theta_host is written after a synchronisation. */
+ * evaluated with exact MPS sums; the three norms come from an orthogonalisation sweep, not from overlaps (with v close to
+ * a the residual is a difference of terms 1/h times larger than itself, which <s|s> by transfer matrices cannot resolve).
+ * Handles of any kind; *theta_host is written after a synchronisation. */
 qtt_status qtt_variational_cost(qtt_ctx* ctx, const qtt_mps* const v[2], const qtt_mps* const a[2], const qtt_mps* const B[2],
                                 const qtt_mpo* D1, const qtt_mpo* D2, double h, double mu, double* theta_host);
 /* Minimises Theta over the MPS pair v (in-out; its bonds are kept, or shrink where a bond exceeds what its neighbours

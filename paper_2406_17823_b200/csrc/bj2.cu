@@ -183,6 +183,7 @@ __global__ void __launch_bounds__(BR * 16) qtt_bj2_kernel(const __grid_constant_
   for (int r = warp; r < 2 * BR; r += NW) {
     const int gr = rank * 2 * BR + r;
     if (gr < p)
+#pragma unroll 4
       for (int x = lane; x < q; x += 32) {
         const double v = __ldcg(X + (i64)gr * ld + x);
         fro += v * v;

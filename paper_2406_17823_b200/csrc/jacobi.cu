@@ -225,6 +225,7 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
   for (int r = crank * per + warp; r < r_end; r += SNT / 32) {
     double s = 0.0;
     if (r < p)
+#pragma unroll 4
       for (int x = lane; x < q; x += 32) {
         double v = P.X[(i64)r * P.ld + x];
         s += v * v;
@@ -302,6 +303,7 @@ __global__ void __launch_bounds__(SNT) qtt_select_kernel(const __grid_constant__
       // one Newton step: rsqrt() is accurate to ~1 ulp in fp64, keep the normalisation at full precision
       inv = inv * (1.5 - 0.5 * s2 * inv * inv);
     }
+#pragma unroll 4
     for (int x = lane; x < q; x += 32)
       P.out[(i64)j * P.out_ld + x] = (inv != 0.0) ? P.X[(i64)src * P.ld + x] * inv : 0.0;
   }

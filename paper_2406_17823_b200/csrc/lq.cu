@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(PANEL_NT) qtt_lq_panel_kernel(const __grid_con
     // partial inner products of row j with rows j..nbp-1 over this slice's tail columns
     for (int i = j + warp; i < nbp; i += NW) {
       double s = 0.0;
+#pragma unroll 4
       for (int x = xj + lane; x < wc; x += 32) s += Ps[j * wp + x] * Ps[i * wp + x];
       s = warp_sum(s);
       if (lane == 0) {
@@ -120,6 +121,7 @@ __global__ void __launch_bounds__(PANEL_NT) qtt_lq_panel_kernel(const __grid_con
         const double si = yij + sc * (gji - yjj * yij);  // v_j . y_i
         const double f = ta * si;
         const double fs = f * sc;
+#pragma unroll 4
         for (int x = xj + lane; x < wc; x += 32) {
           int col = cs + x;
           if (col == colj)
@@ -155,6 +157,7 @@ __global__ void __launch_bounds__(PANEL_NT) qtt_lq_panel_kernel(const __grid_con
     int a = pr / NB, b = pr - a * NB;
     if (a < b && b < nbp) {
       double s = 0.0;
+#pragma unroll 4
       for (int x = lane; x < wc; x += 32) s += Ps[a * wp + x] * Ps[b * wp + x];
       s = warp_sum(s);
       if (lane == 0) st[pr] = s;

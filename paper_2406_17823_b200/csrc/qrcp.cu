@@ -110,6 +110,7 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_kernel(const __grid_constant__ Q
     double fro = 0.0;
     for (int c = warp; c < wc; c += QNW) {
       double s = 0.0;
+#pragma unroll 4
       for (int i = lane; i < p; i += 32) {
         const double v = Xs[(size_t)c * pp + i];
         s += v * v;
@@ -351,6 +352,7 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_kernel(const __grid_constant__ Q
           }
         } else {
           double dot0 = 0.0, dot1 = 0.0;
+#pragma unroll 4
           for (int i = j + 1 + lane; i < p; i += 32) {
             const double v = vb[i];
             dot0 += v * col0[i];
@@ -375,6 +377,7 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_kernel(const __grid_constant__ Q
           }
           double s0 = 0.0, s1 = 0.0;
           if (on0 && on1) {
+#pragma unroll 4
             for (int i = j + 1 + lane; i < p; i += 32) {
               const double v = vb[i];
               const double y0 = col0[i] - ds0 * v, y1 = col1[i] - ds1 * v;
@@ -386,6 +389,7 @@ __global__ void __launch_bounds__(QNT) qtt_qrcp_kernel(const __grid_constant__ Q
           } else {  // one live column (col0 and col1 alias it)
             const double dsa = on0 ? ds0 : ds1;
             double* cola = on0 ? col0 : col1;
+#pragma unroll 4
             for (int i = j + 1 + lane; i < p; i += 32) {
               const double y = cola[i] - dsa * vb[i];
               cola[i] = y;

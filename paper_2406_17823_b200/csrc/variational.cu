@@ -535,7 +535,9 @@ void qtt_variational_stage_impl(qtt_ctx* ctx, const View v0[2], const View a[2],
   if (cg_max) *cg_max = mx;
 }
 
-// Theta (Eq. B6) by exact MPS sums and overlaps
+// Theta (Eq. B6): exact MPS sums, norms from an orthogonalisation sweep.  (The overlap formula <s|s> is no use here: with
+// v close to a, the residual (v - a) / h + B is a difference of terms 1 / h times larger than itself and the transfer-matrix
+// contraction cancels catastrophically -- measured: a relative 4e-5 of Theta at h = 5e-5; reading 19.)
 double qtt_variational_cost_impl(qtt_ctx* ctx, const View v[2], const View a[2], const View Bm[2], const MpoData* D1,
                                  const MpoData* D2, double h, double mu) {
   std::vector<const MpoData*> W{D1, D2};
@@ -546,11 +548,26 @@ double qtt_variational_cost_impl(qtt_ctx* ctx, const View v[2], const View a[2],
   for (int i = 0; i < 2; ++i) terms.push_back({{1.0 / h, v[i]}, {-1.0 / h, a[i]}, {1.0, Bm[i]}});
   std::vector<View> s;
   qtt_concat_batch(ctx, terms, s);
-  double hv[3];
+  const int n = s[0].n;
+  const int big = 1 << 30;
+  std::vector<OutMps> outs(3);
   for (int t = 0; t < 3; ++t) {
-    double* d = qtt_dot_view(ctx, s[t], s[t]);
-    QTT_CU(cudaMemcpyAsync(&hv[t], d, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    outs[t].n = n;
+    outs[t].rcap = qtt_round_caps(s[t].r, big);
+    outs[t].core.resize(n);
+    for (int k = 0; k < n; ++k) outs[t].core[k] = ctx->arena.keep((size_t)outs[t].rcap[k] * 4 * outs[t].rcap[k + 1]);
   }
-  QTT_CU(cudaStreamSynchronize(ctx->stream));
-  return mu * hv[0] + hv[1] + hv[2];
+  SigmaCapture sc;
+  qtt_round_dense_batch(ctx, s, big, 0.0, outs, &sc);
+  double nrm2[3];
+  for (int t = 0; t < 3; ++t) {
+    const int c = sc.count[t][n - 1];
+    std::vector<double> sv(c);
+    QTT_CU(cudaMemcpyAsync(sv.data(), sc.sigma[t][n - 1], sizeof(double) * c, cudaMemcpyDeviceToHost, ctx->stream));
+    QTT_CU(cudaStreamSynchronize(ctx->stream));
+    double acc = 0.0;
+    for (int i = c - 1; i >= 0; --i) acc += sv[i] * sv[i];
+    nrm2[t] = acc;
+  }
+  return mu * nrm2[0] + nrm2[1] + nrm2[2];
 }

@@ -80,7 +80,7 @@ def test_gemm_odd_leading_dimensions(env):
 
 
 LQ_CASES = [(4, 4, 1), (12, 16, 2), (16, 48, 3), (48, 64, 1), (192, 768, 2), (100, 333, 2), (320, 1280, 1),
-            (64, 4096, 2), (256, 9000, 1),
+            (64, 4096, 2), (256, 9000, 1), (512, 4096, 4), (100, 5000, 2), (40, 300, 2), (330, 4100, 2),
             (500, 8192, 3)]  # > 96 MB per batch: the two-level (64-row super-panel) blocking
 
 
