@@ -34,6 +34,7 @@ METRICS = {2: "QTT RK4 steps/sec at 2^8x2^8, chi=32 fp64", 3: METRIC, 4: "QTT RK
 UNIT = "steps/s"
 
 
+EPS = 0.0     # --eps: truncation tolerance of every rounding (Eq. 16); 0 = pure chi_max cap, the BASELINE configs
 SKEW = False  # --convection skew: the paper's skew-symmetric convection (PAPER.md Eq. B2) instead of the convective form
 
 
@@ -41,7 +42,7 @@ def workload(cfg: int):
     c = I.CONFIGS[cfg]
     name = {2: "config2 double shear layer", 3: "config3 decaying jet", 4: "config4 decaying turbulence"}[cfg]
     desc = (f"{name}: 2^{c['n']}x2^{c['n']} grid ({c['n']} sites, d=4), chi_max={c['chi']}, chi_work={2 * c['chi']}, "
-            f"Re={c['Re']:g}, dt={c['dt']:g}, eps=0, "
+            f"Re={c['Re']:g}, dt={c['dt']:g}, eps={EPS:g}, "
             f"{'skew-symmetric convection (PAPER.md Eq. B2)' if SKEW else 'convective form'}, one qtt_rk4_step per step")
     return c, desc
 
@@ -111,7 +112,7 @@ def oracle_step_seconds(cfg: int, state=None):
         state = dict(U=[O.from_dense(ux, chi), O.from_dense(uy, chi)], Dx=O.mpo_d1(n, dx), Dy=O.mpo_d2(n, dx),
                      Lap=O.mpo_laplacian(n, dx))
     t0 = time.perf_counter()
-    state["U"] = O.rk4_step(state["U"], state["Dx"], state["Dy"], state["Lap"], c["Re"], c["dt"], chi, skew=SKEW)
+    state["U"] = O.rk4_step(state["U"], state["Dx"], state["Dy"], state["Lap"], c["Re"], c["dt"], chi, eps=EPS, skew=SKEW)
     t = time.perf_counter() - t0
     return t, "one whole oracle RK4 step per timed step (no extrapolation)", state
 
@@ -305,7 +306,7 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
     def step():
-        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi, EPS)
 
     def barrier():
         if world > 1:
@@ -352,7 +353,7 @@ def run_ours(args):
     d2h = 0
     for _ in range(e2e_steps):
         v = [Q.qtt_mps_from_cores(ctx, cs) for cs in host]
-        Q.qtt_rk4_step(ctx, v, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+        Q.qtt_rk4_step(ctx, v, Dx, Dy, Lap, c["Re"], c["dt"], chi, EPS)
         host = [Q.qtt_mps_get_cores(ctx, x, pinned=True) for x in v]
         d2h = sum(a.nbytes for cs in host for a in cs)
     torch.cuda.synchronize()
@@ -367,7 +368,9 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": desc, "l2": "256 MiB buffer zeroed between timed steps, outside the per-step CUDA "
                    "event pairs; ms_per_step = sum of the per-step event times / steps",
-                   "graph": "whole RK4 step replayed as one CUDA graph", "parallelism": "replicas only"},
+                   "graph": "whole RK4 step replayed as one CUDA graph" if EPS == 0.0 else
+                   "eps > 0: ranks are data dependent, the step runs eagerly with one stream synchronisation per bond and batch",
+                   "parallelism": "replicas only"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "validation": validation,
     }
     if rank == 0:
@@ -393,7 +396,8 @@ def ncu_traffic_table():
     return out
 
 
-KERNEL_NAMES = {"rowjacobi": "qtt_blockjacobi_kernel", "qrcp": "qtt_qrcp_reg_kernel", "gemm": "qtt_gemm_dmma_kernel",
+KERNEL_NAMES = {"rowjacobi": "qtt_bj2_kernel (q <= 512) / qtt_sbj_round_kernel (q <= 2048)", "qrcp": "qtt_qrcp_reg_kernel",
+                "gemm": "qtt_gemm_dmma_kernel",
                 "lq_panel": "qtt_lq_panel_kernel / qtt_qrcp_kernel", "lq_update": "qtt_gemm_dmma_kernel",
                 "select": "qtt_select_kernel", "move": "movement kernels"}
 
@@ -603,7 +607,7 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     Q.qtt_ctx_profile_report(ctx)  # clear
     nprof = 2
     for _ in range(nprof):
-        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi)
+        Q.qtt_rk4_step(ctx, u, Dx, Dy, Lap, c["Re"], c["dt"], chi, EPS)
     per_launch = launch_records(ctx)  # before the report clears them
     rep = Q.qtt_ctx_profile_report(ctx)
     Q.qtt_ctx_profile(ctx, False)
@@ -727,14 +731,18 @@ def main():
                          "batch 6, with each primitive's roofline fraction, instead of the RK4 step")
     ap.add_argument("--convection", default="convective", choices=("convective", "skew"),
                     help="convective (BASELINE.json's configs, default) or the paper's skew-symmetric form (Eq. B2)")
+    ap.add_argument("--eps", type=float, default=0.0,
+                    help="truncation tolerance of every rounding (PAPER.md Eq. 16-17) on top of the chi_max cap; 0 (default) = the "
+                         "BASELINE configs.  eps > 0 runs eagerly (data-dependent ranks: one stream synchronisation per bond)")
     ap.add_argument("--variational", action="store_true",
                     help="time one stage of the paper's variational solver (SURVEY.md section 8f next-1) at the workload's shape")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
                     help="only run the row-a2 site-contraction GEMM passes at the bulk-site shapes of bond CHI and "
                          "print their TFLOP/s (the command the ncu capture in profiles/ is taken on)")
     args = ap.parse_args()
-    global SKEW
+    global SKEW, EPS
     SKEW = args.convection == "skew"
+    EPS = args.eps
     if args.impl == "reference":
         return run_reference(args)
     if args.primitive_sweep:

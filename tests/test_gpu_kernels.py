@@ -126,7 +126,8 @@ def test_lq_rank_deficient(env):
 
 
 JAC_CASES = [(2, 8, 1), (4, 4, 2), (12, 4, 1), (16, 48, 3), (48, 16, 1), (64, 256, 2), (192, 256, 2), (37, 101, 2),
-             (256, 256, 1), (384, 512, 1)]
+             (256, 256, 1), (384, 512, 1),
+             (24, 700, 2), (6, 2500, 1)]  # rows too long for bj2 and no work buffer for sbj: the column-sliced last-resort kernel
 
 
 @pytest.mark.parametrize("p,q,batch", JAC_CASES)
