@@ -253,7 +253,37 @@ def round_mps(cores, chi_max: int = 1 << 30, eps: float = 0.0, info=None):
 
 
 # --------------------------------------------------------------------------- O7
-def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None):
+_M64 = (1 << 64) - 1
+
+
+def sketch_signs(seed: int, site: int, rows: int, cols: int) -> np.ndarray:
+    """Random signs Omega[c, t] in {+1, -1} of the sketched zip-up (reading 25), a counter-based generator both
+    sides implement: z = seed * 0x9E3779B97F4A7C15 + site * 0xD1B54A32D192ED03 + c * 2^20 + t (mod 2^64), mixed by the
+    splitmix64 finaliser z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31;
+    Omega = -1 if the top bit of z is set, else +1.  (cols < 2^20.)"""
+    base = (int(seed) * 0x9E3779B97F4A7C15 + int(site) * 0xD1B54A32D192ED03) & _M64
+    c = np.arange(rows, dtype=np.uint64)[:, None]
+    t = np.arange(cols, dtype=np.uint64)[None, :]
+    with np.errstate(over="ignore"):
+        z = np.uint64(base) + (c << np.uint64(20)) + t
+        z ^= z >> np.uint64(30)
+        z *= np.uint64(0xBF58476D1CE4E5B9)
+        z ^= z >> np.uint64(27)
+        z *= np.uint64(0x94D049BB133111EB)
+        z ^= z >> np.uint64(31)
+    return np.where((z >> np.uint64(63)) == 1, -1.0, 1.0)
+
+
+def sketch_factor(T: np.ndarray, keep: int, seed: int, site: int):
+    """The truncating step of the sketched zip-up: Q = an orthonormal basis of range(T Omega), Omega = sketch_signs(seed,
+    site, columns of T, keep), and R' = Q^T T, so that Q R' is the projection of T on the sketched range
+    (randomised range finder; SURVEY.md section 8f next-4 "cheaper product compression")."""
+    Om = sketch_signs(seed, site, T.shape[1], keep)
+    Q, _ = np.linalg.qr(T @ Om)
+    return Q, Q.T @ T
+
+
+def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None, sketch_seed=None):
     """Fused Hadamard + round ("zip-up" with working bond chi_work; reading 8).
 
     carry R_0 = [1]; for l = 1..n-1:
@@ -265,7 +295,10 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
         core_l = Q.
     Last site: core_n = contract(R, A_n, B_n).  Then step (ii) of O6 with (chi_max, eps).
     Default chi_work = 2*chi_max.  With chi_work >= every intermediate rank this IS
-    round_mps(hadamard(A, B))."""
+    round_mps(hadamard(A, B)).
+    sketch_seed (an int): the cheaper compression of reading 25 -- wherever the line above takes a truncated SVD that
+    really truncates (chi_work < min(4r, a'b')), take instead Q = orth(T Omega), R' = Q^T T with chi_work random sign
+    probes (sketch_factor)."""
     if chi_work is None:
         chi_work = 2 * int(chi_max)
     n = len(A)
@@ -285,6 +318,10 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
         elif k < m and k <= chi_work:
             Q, Rn = np.linalg.qr(T)
             branch = "qr"
+            s = None
+        elif sketch_seed is not None and chi_work < min(m, k):
+            Q, Rn = sketch_factor(T, chi_work, sketch_seed, l)
+            branch = "sketch"
             s = None
         else:
             U, s, Vt = np.linalg.svd(T, full_matrices=False)
@@ -416,7 +453,7 @@ def mpo_to_dense(W) -> np.ndarray:
 
 
 # --------------------------------------------------------------------------- O8
-def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False):
+def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False, sketch_seed=None):
     """f_i = -(u_1 (.) D_1 u_i + u_2 (.) D_2 u_i) + (1/Re) Lap u_i, i = 1,2 (PAPER.md:49-53
     Eq. 2 without the pressure term; convective form, reading 4), with one rounding
     after every apply, product and sum (reading 7).
@@ -427,15 +464,15 @@ def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False):
     f_i = round(-1/2 c_i1 - 1/2 c_i2 - 1/2 d_i1 - 1/2 d_i2 + (1/Re) Lap u_i) (one 5-term sum)."""
     Dj = (Dx, Dy)
     if skew:
-        p11 = round_product(u[0], u[0], chi_max, eps, chi_work)
-        p12 = round_product(u[0], u[1], chi_max, eps, chi_work)
-        p22 = round_product(u[1], u[1], chi_max, eps, chi_work)
+        p11 = round_product(u[0], u[0], chi_max, eps, chi_work, sketch_seed=sketch_seed)
+        p12 = round_product(u[0], u[1], chi_max, eps, chi_work, sketch_seed=sketch_seed)
+        p22 = round_product(u[1], u[1], chi_max, eps, chi_work, sketch_seed=sketch_seed)
         pij = [[p11, p12], [p12, p22]]
     f = []
     for i in range(2):
         g = [round_mps(apply_mpo(Dj[j], u[i]), chi_max, eps) for j in range(2)]
         lap = round_mps(apply_mpo(Lap, u[i]), chi_max, eps)
-        c = [round_product(u[j], g[j], chi_max, eps, chi_work) for j in range(2)]
+        c = [round_product(u[j], g[j], chi_max, eps, chi_work, sketch_seed=sketch_seed) for j in range(2)]
         if skew:
             d = [round_mps(apply_mpo(Dj[j], pij[i][j]), chi_max, eps) for j in range(2)]
             terms = [(-0.5, c[0]), (-0.5, c[1]), (-0.5, d[0]), (-0.5, d[1]), (1.0 / Re, lap)]
@@ -446,7 +483,7 @@ def rhs(u, Dx, Dy, Lap, Re, chi_max, eps=0.0, chi_work=None, skew=False):
 
 
 # --------------------------------------------------------------------------- O9
-def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False, info=None):
+def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False, info=None, sketch_seed=None):
     """Classical RK4 (Eq. 11) on the MPS pair u = [u_1, u_2]; all
     roundings with the same (chi_max, eps); final combination as one 5-term sum
     and one rounding (reading 10).  ``info`` (a dict), if given, receives under "final" the two
@@ -454,10 +491,10 @@ def rk4_step(u, Dx, Dy, Lap, Re, dt, chi_max, eps=0.0, chi_work=None, skew=False
     def stage(k, h):
         return [round_mps(lincomb([(1.0, u[i]), (h, k[i])]), chi_max, eps) for i in range(2)]
 
-    k1 = rhs(u, Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
-    k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
-    k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
-    k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew)
+    k1 = rhs(u, Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew, sketch_seed)
+    k2 = rhs(stage(k1, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew, sketch_seed)
+    k3 = rhs(stage(k2, dt / 2), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew, sketch_seed)
+    k4 = rhs(stage(k3, dt), Dx, Dy, Lap, Re, chi_max, eps, chi_work, skew, sketch_seed)
     recs = [{}, {}] if info is not None else [None, None]
     out = [
         round_mps(
