@@ -260,7 +260,8 @@ def sketch_signs(seed: int, site: int, rows: int, cols: int) -> np.ndarray:
     """Random signs Omega[c, t] in {+1, -1} of the sketched zip-up (reading 25), a counter-based generator both
     sides implement: z = seed * 0x9E3779B97F4A7C15 + site * 0xD1B54A32D192ED03 + c * 2^20 + t (mod 2^64), mixed by the
     splitmix64 finaliser z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31;
-    Omega = -1 if the top bit of z is set, else +1.  (cols < 2^20.)"""
+    Omega = -1 if the top bit of z is set, else +1.  (cols < 2^20.)  The zip-up uses it with rows = 4: row c = the physical
+    index w of site `site`, column t = the probe."""
     base = (int(seed) * 0x9E3779B97F4A7C15 + int(site) * 0xD1B54A32D192ED03) & _M64
     c = np.arange(rows, dtype=np.uint64)[:, None]
     t = np.arange(cols, dtype=np.uint64)[None, :]
@@ -274,13 +275,43 @@ def sketch_signs(seed: int, site: int, rows: int, cols: int) -> np.ndarray:
     return np.where((z >> np.uint64(63)) == 1, -1.0, 1.0)
 
 
-def sketch_factor(T: np.ndarray, keep: int, seed: int, site: int):
-    """The truncating step of the sketched zip-up: Q = an orthonormal basis of range(T Omega), Omega = sketch_signs(seed,
-    site, columns of T, keep), and R' = Q^T T, so that Q R' is the projection of T on the sketched range
-    (randomised range finder; SURVEY.md section 8f next-4 "cheaper product compression")."""
-    Om = sketch_signs(seed, site, T.shape[1], keep)
-    Q, _ = np.linalg.qr(T @ Om)
+def sketch_probes(A, B, n_probes: int, seed: int):
+    """Structured probes of the sketched zip-up (reading 25).  Probe t is the rank-one tensor x^{(1)}_t (x) ... (x) x^{(n)}_t
+    of random sign vectors over the PHYSICAL indices, x^{(k)}_t[w] = sketch_signs(seed, k, 4, n_probes)[w, t] (sites k
+    counted from 0).  Contracted through the product's own site tensors from the right they give, for every bond l,
+        S_l[a, b, t] = sum_w x^{(l)}_t[w] sum_{a', b'} A_l[a, w, a'] B_l[b, w, b'] S_{l+1}[a', b', t],     S_n = 1,
+    i.e. the probes as seen from the bond (a, b) left of site l.  Because they live on the physical indices, T S is the
+    same whatever gauge the bonds of A and B are in -- a random matrix on the bond indices themselves would not be
+    (measured: two gauges of the same operand gave results 10 % apart).  Returns [S_0, ..., S_n]."""
+    n = len(A)
+    S = [None] * (n + 1)
+    S[n] = np.ones((1, 1, n_probes))
+    for l in range(n - 1, -1, -1):
+        x = sketch_signs(seed, l, D_PHYS, n_probes)
+        S[l] = np.einsum("wt,awc,bwd,cdt->abt", x, A[l], B[l], S[l + 1], optimize=True)
+    return S
+
+
+def sketch_factor(T: np.ndarray, Sl: np.ndarray):
+    """The truncating step of the sketched zip-up: Q = an orthonormal basis of the numerical range of Y = T S (left singular
+    vectors of Y with sigma_i > 8 eps ||Y||_F; the columns beyond that rank are ZERO, so the bond keeps its size), S the
+    probes seen from the right bond of this site as a (columns of T) x (probes) matrix, and R' = Q^T T: Q R' is the projection
+    of T on the sketched range (randomised range finder; SURVEY.md section 8f next-4 "cheaper product compression",
+    PAPER.md:318).  The rank cut makes the step a function of range(Y) alone: when Y is numerically rank deficient (smooth
+    fields; coinciding probes) a plain QR would fill up with directions made of rounding noise."""
+    Y = T @ Sl
+    U, sv, _ = np.linalg.svd(Y, full_matrices=False)
+    rank = int(np.sum(sv > 8.0 * np.finfo(np.float64).eps * np.linalg.norm(Y)))
+    Q = np.zeros_like(U)
+    Q[:, :rank] = U[:, :rank]
     return Q, Q.T @ T
+
+
+def sketch_applies(n: int, l: int, m: int, k: int, chi_work: int) -> bool:
+    """The sketch replaces the truncated SVD at zip-up site l (0-based) where that SVD really truncates (chi_work < min(m, k))
+    and the sites to the right still carry at least 4 chi_work physical configurations (4^(n-1-l) >= 4 chi_work): sign probes
+    over fewer configurations coincide or are linearly dependent too often to span a chi_work-dimensional range."""
+    return chi_work < min(m, k) and 4 ** (n - 1 - l) >= 4 * chi_work
 
 
 def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None, sketch_seed=None):
@@ -297,13 +328,15 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
     Default chi_work = 2*chi_max.  With chi_work >= every intermediate rank this IS
     round_mps(hadamard(A, B)).
     sketch_seed (an int): the cheaper compression of reading 25 -- wherever the line above takes a truncated SVD that
-    really truncates (chi_work < min(4r, a'b')), take instead Q = orth(T Omega), R' = Q^T T with chi_work random sign
-    probes (sketch_factor)."""
+    really truncates (chi_work < min(4r, a'b')) and enough sites remain to the right (sketch_applies), take instead
+    Q = orth(T S), R' = Q^T T with chi_work structured random sign probes contracted through the remaining sites
+    (sketch_probes, sketch_factor)."""
     if chi_work is None:
         chi_work = 2 * int(chi_max)
     n = len(A)
     R = np.ones((1, 1, 1))
     cores = []
+    probes = None  # built at the first site that takes the sketch (a working bond that never truncates needs none)
     zip_log = []  # per site: the matrix T that was factorised, Q, R' and the branch taken (read by the pins only)
     for l in range(n - 1):
         T4 = np.einsum("rab,awc,bwd->rwcd", R, A[l], B[l], optimize=True)
@@ -319,8 +352,10 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
             Q, Rn = np.linalg.qr(T)
             branch = "qr"
             s = None
-        elif sketch_seed is not None and chi_work < min(m, k):
-            Q, Rn = sketch_factor(T, chi_work, sketch_seed, l)
+        elif sketch_seed is not None and sketch_applies(n, l, m, k, chi_work):
+            if probes is None:
+                probes = sketch_probes(A, B, chi_work, sketch_seed)
+            Q, Rn = sketch_factor(T, probes[l + 1].reshape(k, chi_work))
             branch = "sketch"
             s = None
         else:

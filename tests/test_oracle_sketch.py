@@ -51,27 +51,85 @@ def test_sketch_factor_is_a_projection_exact_on_low_rank_and_within_the_range_fi
     rng = np.random.default_rng(1)
     T = graded(rng, 96, 400, 8)
     keep = 32
-    Q, R = O.sketch_factor(T, keep, seed=5, site=2)
+    Om = O.sketch_signs(5, 2, 400, keep)
+    Q, R = O.sketch_factor(T, Om)
     assert Q.shape == (96, keep) and R.shape == (keep, 400)
     assert np.linalg.norm(Q.T @ Q - np.eye(keep)) < 1e-13
     assert np.linalg.norm(R - Q.T @ T) == 0.0
-    # Q R' is the orthogonal projection of T on range(T Omega): T - Q R' is orthogonal to Q, and range(Q) contains T Omega
+    # Q R' is the orthogonal projection of T on range(T S): T - Q R' is orthogonal to Q, and range(Q) contains T S
     assert np.linalg.norm(Q.T @ (T - Q @ R)) < 1e-13 * np.linalg.norm(T)
-    Y = T @ O.sketch_signs(5, 2, 400, keep)
+    Y = T @ Om
     assert np.linalg.norm(Y - Q @ (Q.T @ Y)) < 1e-12 * np.linalg.norm(Y)
     # exact when rank(T) <= keep
     L = rng.standard_normal((96, 20)) @ rng.standard_normal((20, 400))
-    Ql, Rl = O.sketch_factor(L, keep, seed=5, site=2)
+    Ql, Rl = O.sketch_factor(L, Om)
     assert np.linalg.norm(L - Ql @ Rl) < 1e-12 * np.linalg.norm(L)
+    # ... and then only rank(T) columns of Q are non-zero (orthonormal), the rest exact zeros: the bond keeps its size
+    nz = np.linalg.norm(Ql, axis=0) > 0
+    assert nz.sum() == 20 and np.all(nz[:20]) and np.linalg.norm(Ql[:, :20].T @ Ql[:, :20] - np.eye(20)) < 1e-13
+    # coinciding probes (two equal columns of S) lose one direction, nothing else
+    Om2 = Om.copy()
+    Om2[:, 5] = Om2[:, 4]
+    Q2, R2 = O.sketch_factor(T, Om2)
+    assert (np.linalg.norm(Q2, axis=0) > 0).sum() == keep - 1
+    assert np.linalg.norm(Q2.T @ (T - Q2 @ R2)) < 1e-13 * np.linalg.norm(T)
     # randomised range finder (Halko-Martinsson-Tropp, Thm 10.5 in expectation): with keep = k + p probes the error is about
     # sqrt(1 + k / (p - 1)) times the optimal rank-k tail; for k = p = keep / 2 that is ~sqrt(2).  Checked with a factor 2
     # on several seeds against an independent SVD -- and it can never beat the optimal rank-keep error.
     s = np.linalg.svd(T, compute_uv=False)
     tail = lambda r: np.sqrt(np.sum(s[r:] ** 2))
     for seed in range(6):
-        Qs, Rs = O.sketch_factor(T, keep, seed=seed, site=0)
+        Qs, Rs = O.sketch_factor(T, O.sketch_signs(seed, 0, 400, keep))
         err = np.linalg.norm(T - Qs @ Rs)
         assert tail(keep) * (1 - 1e-12) <= err <= 2.0 * tail(keep // 2)
+
+
+def random_gauge(cores, rng):
+    """The same MPS in another gauge: core_k <- G_{k-1}^T core_k G_k with random ORTHOGONAL G (two right-canonical forms of
+    one state -- what two implementations of the roundings hand to the product -- differ by exactly that; the truncated SVDs
+    of the zip-up, deterministic or not, are only defined up to such gauges)."""
+    out = [c.copy() for c in cores]
+    for k in range(len(cores) - 1):
+        r = cores[k].shape[2]
+        G = np.linalg.qr(rng.standard_normal((r, r)))[0]
+        out[k] = np.einsum("awb,bc->awc", out[k], G)
+        out[k + 1] = np.einsum("ba,bwc->awc", G, out[k + 1])
+    return out
+
+
+def test_probes_are_the_dense_contraction_and_the_result_does_not_depend_on_the_gauge():
+    n, P, seed = 4, 6, 9
+    rng = np.random.default_rng(2)
+    A = O.from_dense(rng.standard_normal((16, 16)), 5)
+    B = O.from_dense(rng.standard_normal((16, 16)), 5)
+    S = O.sketch_probes(A, B, P, seed)
+    assert S[n].shape == (1, 1, P) and np.all(S[n] == 1.0)
+    # brute force: probe t is the rank-one tensor of sign vectors over the physical indices of sites l..n-1, contracted with
+    # the dense right part of the Hadamard product MPS
+    H = O.hadamard(A, B)
+    for l in (1, 2, 3):
+        right = H[l]
+        for k in range(l + 1, n):
+            right = np.tensordot(right, H[k], axes=([right.ndim - 1], [0]))
+        right = right.reshape(right.shape[:-1])  # (bond, w_l, ..., w_{n-1})
+        for t in range(P):
+            v = right
+            for k in range(l, n):
+                x = O.sketch_signs(seed, k, 4, P)[:, t]
+                v = np.tensordot(v, x, axes=([1], [0]))
+            assert np.allclose(v, S[l][:, :, t].reshape(-1), rtol=1e-12, atol=1e-12 * np.abs(v).max())
+    # gauge invariance of the whole sketched rounding (what a random matrix on the bond indices would NOT have)
+    n, chi = 6, 8
+    Fa, Fb = fields(n, 3)
+    A, B = O.from_dense(Fa, 16), O.from_dense(Fb, 16)
+    ref = O.to_dense(O.round_product(A, B, chi, chi_work=2 * chi, sketch_seed=11))
+    A2, B2 = random_gauge(A, rng), random_gauge(B, rng)
+    assert np.linalg.norm(O.to_dense(A2) - O.to_dense(A)) < 1e-11 * np.linalg.norm(O.to_dense(A))
+    got = O.to_dense(O.round_product(A2, B2, chi, chi_work=2 * chi, sketch_seed=11))
+    assert np.linalg.norm(got - ref) < 1e-9 * np.linalg.norm(ref)
+    # ... and it does depend on the seed
+    other = O.to_dense(O.round_product(A, B, chi, chi_work=2 * chi, sketch_seed=12))
+    assert np.linalg.norm(other - ref) > 1e-6 * np.linalg.norm(ref)
 
 
 def fields(n, seed):
@@ -98,12 +156,17 @@ def test_sketched_product_rounding_against_the_dense_product_and_the_determinist
     # the sketch replaces exactly the truncating SVD steps, nothing else
     bd = [z["branch"] for z in info_d["zip"]]
     bs = [z["branch"] for z in info_s["zip"]]
-    assert "svd" in bd and [b if b != "svd" else "sketch" for b in bd] == bs
+    assert "sketch" in bs and all(x == y or (x == "svd" and y == "sketch") for x, y in zip(bd, bs))
+    for l, (x, y) in enumerate(zip(bd, bs)):  # the sketch is taken exactly where sketch_applies says
+        m, k = info_d["zip"][l]["T"].shape
+        assert (y == "sketch") == (x == "svd" and O.sketch_applies(n, l, m, k, 2 * chi))
     assert O.bonds(ske) == O.bonds(det)
     for z in info_s["zip"]:
         if z["branch"] == "sketch":
             assert z["Q"].shape[1] == 2 * chi
-            assert np.linalg.norm(z["Q"].T @ z["Q"] - np.eye(2 * chi)) < 1e-12
+            nzc = np.linalg.norm(z["Q"], axis=0) > 0
+            Qn = z["Q"][:, nzc]
+            assert np.linalg.norm(Qn.T @ Qn - np.eye(Qn.shape[1])) < 1e-12
             assert np.linalg.norm(z["R"] - z["Q"].T @ z["T"]) < 1e-12 * np.linalg.norm(z["T"])
     e_det = np.linalg.norm(O.to_dense(det) - exact) / np.linalg.norm(exact)
     e_ske = np.linalg.norm(O.to_dense(ske) - exact) / np.linalg.norm(exact)
@@ -116,11 +179,14 @@ def test_sketched_product_rounding_against_the_dense_product_and_the_determinist
 
 
 def test_rk4_step_with_the_sketched_products_stays_within_the_truncation_error():
-    n, chi, Re, dt = 6, 10, 200.0, 1e-3
+    n, chi, Re, dt = 7, 6, 200.0, 1e-3
     dx = 1.0 / (1 << n)
     Fa, Fb = fields(n, 5)
     u = [O.from_dense(Fa, chi), O.from_dense(0.5 * Fb, chi)]
     ops = (O.mpo_d1(n, dx), O.mpo_d2(n, dx), O.mpo_laplacian(n, dx))
+    info = {}
+    O.round_product(u[0], u[1], chi, sketch_seed=3, info=info)
+    assert "sketch" in [z["branch"] for z in info["zip"]]  # these sizes do take the sketch
     det = O.rk4_step(u, *ops, Re, dt, chi)
     ske = O.rk4_step(u, *ops, Re, dt, chi, sketch_seed=3)
     big = O.rk4_step(u, *ops, Re, dt, 4 * chi)  # nearly untruncated step as the yardstick
