@@ -260,8 +260,7 @@ def sketch_signs(seed: int, site: int, rows: int, cols: int) -> np.ndarray:
     """Random signs Omega[c, t] in {+1, -1} of the sketched zip-up (reading 25), a counter-based generator both
     sides implement: z = seed * 0x9E3779B97F4A7C15 + site * 0xD1B54A32D192ED03 + c * 2^20 + t (mod 2^64), mixed by the
     splitmix64 finaliser z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31;
-    Omega = -1 if the top bit of z is set, else +1.  (cols < 2^20.)  The zip-up uses it with rows = 4: row c = the physical
-    index w of site `site`, column t = the probe."""
+    Omega = -1 if the top bit of z is set, else +1.  (cols < 2^20.)  The zip-up uses it with rows = 4 P (sketch_mixers)."""
     base = (int(seed) * 0x9E3779B97F4A7C15 + int(site) * 0xD1B54A32D192ED03) & _M64
     c = np.arange(rows, dtype=np.uint64)[:, None]
     t = np.arange(cols, dtype=np.uint64)[None, :]
@@ -275,20 +274,32 @@ def sketch_signs(seed: int, site: int, rows: int, cols: int) -> np.ndarray:
     return np.where((z >> np.uint64(63)) == 1, -1.0, 1.0)
 
 
+def sketch_mixers(seed: int, site: int, n_probes: int) -> np.ndarray:
+    """G[w][u][t] = sketch_signs(seed, site, 4 P, P)[w P + u, t] / sqrt(P), P = n_probes: site `site`'s core of the random
+    tensor train the probes are (physical index w, bonds u -> t)."""
+    P = int(n_probes)
+    return sketch_signs(seed, site, D_PHYS * P, P).reshape(D_PHYS, P, P) * (1.0 / math.sqrt(P))
+
+
 def sketch_probes(A, B, n_probes: int, seed: int):
-    """Structured probes of the sketched zip-up (reading 25).  Probe t is the rank-one tensor x^{(1)}_t (x) ... (x) x^{(n)}_t
-    of random sign vectors over the PHYSICAL indices, x^{(k)}_t[w] = sketch_signs(seed, k, 4, n_probes)[w, t] (sites k
-    counted from 0).  Contracted through the product's own site tensors from the right they give, for every bond l,
-        S_l[a, b, t] = sum_w x^{(l)}_t[w] sum_{a', b'} A_l[a, w, a'] B_l[b, w, b'] S_{l+1}[a', b', t],     S_n = 1,
+    """Structured probes of the sketched zip-up (reading 25): a random tensor train over the PHYSICAL indices with bond P =
+    n_probes and sign cores G_k (sketch_mixers; sites k counted from 0; the open bond t at the left end numbers the probes),
+        Omega[w_l .. w_{n-1}; t] = sum_{u's} G_l[w_l][u_{l+1}, t] G_{l+1}[w_{l+1}][u_{l+2}, u_{l+1}] ... G_{n-1}[w_{n-1}][u_n, u_{n-1}],
+    closed by the all-ones vector at u_n.  Contracted through the product's own site tensors from the right they give, for
+    every bond l,
+        S_l[a, b, t] = sum_{w, u} G_l[w][u, t] sum_{a', b'} A_l[a, w, a'] B_l[b, w, b'] S_{l+1}[a', b', u],     S_n = 1,
     i.e. the probes as seen from the bond (a, b) left of site l.  Because they live on the physical indices, T S is the
     same whatever gauge the bonds of A and B are in -- a random matrix on the bond indices themselves would not be
-    (measured: two gauges of the same operand gave results 10 % apart).  Returns [S_0, ..., S_n]."""
+    (measured: two gauges of the same operand gave results 10 % apart).  Probes with bond 1 (one rank-one tensor of sign
+    vectors per probe) are cheaper still but fail too often: over 12 seeds their worst range-finder error was 12 .. 1000 x the
+    optimal rank-P/2 tail of the unfolding, against 0.08 .. 1.07 x for the bond-P train (randomised TT rounding in the
+    literature uses such trains for the same reason).  Returns [S_0, ..., S_n]."""
     n = len(A)
     S = [None] * (n + 1)
     S[n] = np.ones((1, 1, n_probes))
     for l in range(n - 1, -1, -1):
-        x = sketch_signs(seed, l, D_PHYS, n_probes)
-        S[l] = np.einsum("wt,awc,bwd,cdt->abt", x, A[l], B[l], S[l + 1], optimize=True)
+        G = sketch_mixers(seed, l, n_probes)
+        S[l] = np.einsum("wut,awc,bwd,cdu->abt", G, A[l], B[l], S[l + 1], optimize=True)
     return S
 
 
@@ -309,9 +320,10 @@ def sketch_factor(T: np.ndarray, Sl: np.ndarray):
 
 def sketch_applies(n: int, l: int, m: int, k: int, chi_work: int) -> bool:
     """The sketch replaces the truncated SVD at zip-up site l (0-based) where that SVD really truncates (chi_work < min(m, k))
-    and the sites to the right still carry at least 4 chi_work physical configurations (4^(n-1-l) >= 4 chi_work): sign probes
-    over fewer configurations coincide or are linearly dependent too often to span a chi_work-dimensional range."""
-    return chi_work < min(m, k) and 4 ** (n - 1 - l) >= 4 * chi_work
+    and the sites to the right still carry at least 2 chi_work physical configurations (4^(n-1-l) >= 2 chi_work, DESIGN.md
+    reading 25): the probes seen from bond l+1 span at most 4^(n-1-l) dimensions, and sign probes over fewer configurations
+    coincide or are linearly dependent too often to span a chi_work-dimensional range."""
+    return chi_work < min(m, k) and 4 ** (n - 1 - l) >= 2 * chi_work
 
 
 def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None, sketch_seed=None):
@@ -329,7 +341,7 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
     round_mps(hadamard(A, B)).
     sketch_seed (an int): the cheaper compression of reading 25 -- wherever the line above takes a truncated SVD that
     really truncates (chi_work < min(4r, a'b')) and enough sites remain to the right (sketch_applies), take instead
-    Q = orth(T S), R' = Q^T T with chi_work structured random sign probes contracted through the remaining sites
+    Q = orth(T S), R' = Q^T T with chi_work structured random probes (a sign tensor train) contracted through the remaining sites
     (sketch_probes, sketch_factor)."""
     if chi_work is None:
         chi_work = 2 * int(chi_max)

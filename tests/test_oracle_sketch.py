@@ -104,20 +104,53 @@ def test_probes_are_the_dense_contraction_and_the_result_does_not_depend_on_the_
     B = O.from_dense(rng.standard_normal((16, 16)), 5)
     S = O.sketch_probes(A, B, P, seed)
     assert S[n].shape == (1, 1, P) and np.all(S[n] == 1.0)
-    # brute force: probe t is the rank-one tensor of sign vectors over the physical indices of sites l..n-1, contracted with
-    # the dense right part of the Hadamard product MPS
+    # the cores of the probe train are the generator's signs, row w P + u, column t, over sqrt(P)
+    for k in (0, 3):
+        G = O.sketch_mixers(seed, k, P)
+        assert G.shape == (4, P, P)
+        for w, uu, t in ((0, 0, 0), (3, 5, 5), (2, 1, 4), (1, 4, 0)):
+            assert G[w, uu, t] == sign_bigint(seed, k, w * P + uu, t) / np.sqrt(P)
+    # brute force: the probes are the dense tensor Omega[w_l .. w_{n-1}; t] of that train (closed by ones at the right end),
+    # contracted with the dense right part of the Hadamard product MPS
     H = O.hadamard(A, B)
     for l in (1, 2, 3):
         right = H[l]
         for k in range(l + 1, n):
             right = np.tensordot(right, H[k], axes=([right.ndim - 1], [0]))
-        right = right.reshape(right.shape[:-1])  # (bond, w_l, ..., w_{n-1})
-        for t in range(P):
-            v = right
-            for k in range(l, n):
-                x = O.sketch_signs(seed, k, 4, P)[:, t]
-                v = np.tensordot(v, x, axes=([1], [0]))
-            assert np.allclose(v, S[l][:, :, t].reshape(-1), rtol=1e-12, atol=1e-12 * np.abs(v).max())
+        right = right.reshape(right.shape[0], -1)  # (bond, (w_l, ..., w_{n-1}))
+        Om = None
+        for k in range(n - 1, l - 1, -1):
+            G = np.array([[[sign_bigint(seed, k, w * P + uu, t) for t in range(P)] for uu in range(P)] for w in range(4)]) / np.sqrt(P)
+            if Om is None:
+                Om = G.sum(axis=1)  # (w_{n-1}, t)
+            else:
+                Om = np.tensordot(G, Om, axes=([1], [Om.ndim - 1]))  # (w_k, t, w_{k+1}, ...) -> move t last
+                Om = np.moveaxis(Om, 1, -1)
+        v = right @ Om.reshape(-1, P)
+        assert np.allclose(v, S[l].reshape(-1, P), rtol=1e-12, atol=1e-12 * np.abs(v).max())
+    # a bond-1 train (one rank-one sign tensor per probe) would also be gauge invariant, but its range finder fails too often;
+    # this one stays within the optimal rank-P/2 tail of the TRUE unfolding (T times the dense right part) on every seed tried
+    n6, cw = 7, 8
+    Fa, Fb = fields(n6, 3)
+    A6, B6 = O.from_dense(Fa, 16), O.from_dense(Fb, 16)
+    H6 = O.hadamard(A6, B6)
+    for sd in range(1, 7):
+        info = {}
+        O.round_product(A6, B6, cw // 2, chi_work=cw, sketch_seed=sd, info=info)
+        took = 0
+        for l, z in enumerate(info["zip"]):
+            if z["branch"] != "sketch":
+                continue
+            took += 1
+            E = np.ones((1, 1))
+            for k in range(n6 - 1, l, -1):
+                r0, d, r1 = H6[k].shape
+                E = (H6[k].reshape(r0 * d, r1) @ E).reshape(r0, -1)
+            M = z["T"] @ E
+            s = np.linalg.svd(M, compute_uv=False)
+            err = np.linalg.norm(M - z["Q"] @ (z["Q"].T @ M))
+            assert err <= 2.0 * np.sqrt(np.sum(s[cw // 2:] ** 2))
+        assert took >= 3
     # gauge invariance of the whole sketched rounding (what a random matrix on the bond indices would NOT have)
     n, chi = 6, 8
     Fa, Fb = fields(n, 3)
