@@ -320,10 +320,12 @@ def sketch_factor(T: np.ndarray, Sl: np.ndarray):
 
 def sketch_applies(n: int, l: int, m: int, k: int, chi_work: int) -> bool:
     """The sketch replaces the truncated SVD at zip-up site l (0-based) where that SVD really truncates (chi_work < min(m, k))
-    and the sites to the right still carry at least 2 chi_work physical configurations (4^(n-1-l) >= 2 chi_work, DESIGN.md
-    reading 25): the probes seen from bond l+1 span at most 4^(n-1-l) dimensions, and sign probes over fewer configurations
-    coincide or are linearly dependent too often to span a chi_work-dimensional range."""
-    return chi_work < min(m, k) and 4 ** (n - 1 - l) >= 2 * chi_work
+    and the c = 4^(n-1-l) physical configurations to the right of the site are either many, c >= 2 chi_work (the probes seen
+    from bond l+1 span at most c dimensions: a random range finder wants them oversampled), or few, c <= chi_work: then the
+    true unfolding has rank <= c <= chi_work, the probes span its whole range and the step loses nothing (DESIGN.md reading
+    25).  In between (chi_work < c < 2 chi_work) the truncated SVD stays."""
+    c = 4 ** (n - 1 - l)
+    return chi_work < min(m, k) and (c >= 2 * chi_work or c <= chi_work)
 
 
 def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = None, info=None, sketch_seed=None):

@@ -137,7 +137,7 @@ def test_probes_are_the_dense_contraction_and_the_result_does_not_depend_on_the_
     for sd in range(1, 7):
         info = {}
         O.round_product(A6, B6, cw // 2, chi_work=cw, sketch_seed=sd, info=info)
-        took = 0
+        took = exact = 0
         for l, z in enumerate(info["zip"]):
             if z["branch"] != "sketch":
                 continue
@@ -149,8 +149,11 @@ def test_probes_are_the_dense_contraction_and_the_result_does_not_depend_on_the_
             M = z["T"] @ E
             s = np.linalg.svd(M, compute_uv=False)
             err = np.linalg.norm(M - z["Q"] @ (z["Q"].T @ M))
-            assert err <= 2.0 * np.sqrt(np.sum(s[cw // 2:] ** 2))
-        assert took >= 3
+            assert err <= 2.0 * np.sqrt(np.sum(s[cw // 2:] ** 2)) + 1e-11 * s[0]
+            if 4 ** (n6 - 1 - l) <= cw:  # few configurations left: the probes span the whole range, nothing is lost
+                exact += 1
+                assert err <= 1e-11 * s[0] and (np.linalg.norm(z["Q"], axis=0) > 0).sum() <= 4 ** (n6 - 1 - l)
+        assert took >= 4 and exact >= 1
     # gauge invariance of the whole sketched rounding (what a random matrix on the bond indices would NOT have)
     n, chi = 6, 8
     Fa, Fb = fields(n, 3)
