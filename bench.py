@@ -35,6 +35,7 @@ UNIT = "steps/s"
 
 
 EPS = 0.0     # --eps: truncation tolerance of every rounding (Eq. 16); 0 = pure chi_max cap, the BASELINE configs
+SKETCH = None  # --product-compression sketch: seed of the sketched zip-up (reading 25); None = deterministic zip-up
 SKEW = False  # --convection skew: the paper's skew-symmetric convection (PAPER.md Eq. B2) instead of the convective form
 
 
@@ -43,7 +44,9 @@ def workload(cfg: int):
     name = {2: "config2 double shear layer", 3: "config3 decaying jet", 4: "config4 decaying turbulence"}[cfg]
     desc = (f"{name}: 2^{c['n']}x2^{c['n']} grid ({c['n']} sites, d=4), chi_max={c['chi']}, chi_work={2 * c['chi']}, "
             f"Re={c['Re']:g}, dt={c['dt']:g}, eps={EPS:g}, "
-            f"{'skew-symmetric convection (PAPER.md Eq. B2)' if SKEW else 'convective form'}, one qtt_rk4_step per step")
+            f"{'skew-symmetric convection (PAPER.md Eq. B2)' if SKEW else 'convective form'}, "
+            f"{'SKETCHED zip-up (seed %d; NOT the BASELINE method: DESIGN.md reading 25), ' % SKETCH if SKETCH is not None else ''}"
+            f"one qtt_rk4_step per step")
     return c, desc
 
 
@@ -112,7 +115,8 @@ def oracle_step_seconds(cfg: int, state=None):
         state = dict(U=[O.from_dense(ux, chi), O.from_dense(uy, chi)], Dx=O.mpo_d1(n, dx), Dy=O.mpo_d2(n, dx),
                      Lap=O.mpo_laplacian(n, dx))
     t0 = time.perf_counter()
-    state["U"] = O.rk4_step(state["U"], state["Dx"], state["Dy"], state["Lap"], c["Re"], c["dt"], chi, eps=EPS, skew=SKEW)
+    state["U"] = O.rk4_step(state["U"], state["Dx"], state["Dy"], state["Lap"], c["Re"], c["dt"], chi, eps=EPS, skew=SKEW,
+                             sketch_seed=SKETCH)
     t = time.perf_counter() - t0
     return t, "one whole oracle RK4 step per timed step (no extrapolation)", state
 
@@ -303,6 +307,25 @@ def run_ours(args):
     ux, uy = I.config_fields(args.config, seed=replica_seed(rank))
     u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
     ctx.synchronize()
+    sketch_record = None
+    if SKETCH is not None:
+        # what the cheaper compression costs in accuracy: one step from the same state in both modes, and the
+        # deterministic step's own distance to a step at twice the bond (its truncation error), for scale
+        def one_step(mode, bond):
+            Q.qtt_ctx_set_product_compression(ctx, mode, SKETCH or 0)
+            w = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in (ux, uy)]
+            Q.qtt_rk4_step(ctx, w, Dx, Dy, Lap, c["Re"], c["dt"], bond, EPS)
+            d = [Q.qtt_to_dense(ctx, x) for x in w]
+            ctx.synchronize()
+            return d
+        det, ske, fine = one_step(False, chi), one_step(True, chi), one_step(False, 2 * chi)
+        nrm = lambda a, b: float(sum(torch.linalg.norm(x - y) ** 2 for x, y in zip(a, b)) ** 0.5
+                                 / sum(torch.linalg.norm(y) ** 2 for y in b) ** 0.5)
+        sketch_record = {"seed": SKETCH, "rel_diff_sketch_vs_svd_one_step": nrm(ske, det),
+                         "rel_diff_svd_chi_vs_2chi_one_step": nrm(det, fine),
+                         "rel_diff_sketch_chi_vs_svd_2chi_one_step": nrm(ske, fine)}
+        del det, ske, fine
+        Q.qtt_ctx_set_product_compression(ctx, True, SKETCH)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
     def step():
@@ -373,6 +396,8 @@ def run_ours(args):
                    "parallelism": "replicas only"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "validation": validation,
     }
+    if sketch_record:
+        line["product_compression"] = sketch_record
     if rank == 0:
         line.update(roofline_and_baseline(Q, ctx, u, (Dx, Dy, Lap), c, chi, args, ms_per_step))
         print(json.dumps(line), flush=True)
@@ -734,14 +759,20 @@ def main():
     ap.add_argument("--eps", type=float, default=0.0,
                     help="truncation tolerance of every rounding (PAPER.md Eq. 16-17) on top of the chi_max cap; 0 (default) = the "
                          "BASELINE configs.  eps > 0 runs eagerly (data-dependent ranks: one stream synchronisation per bond)")
+    ap.add_argument("--product-compression", default="svd", choices=("svd", "sketch"),
+                    help="svd (default): the deterministic zip-up of the BASELINE configs; sketch: the randomised range finder of "
+                         "SURVEY.md section 8f next-4 (DESIGN.md reading 25) at the sites its rule admits -- another method, "
+                         "reported with its one-step distance to the deterministic result")
+    ap.add_argument("--sketch-seed", type=int, default=1)
     ap.add_argument("--variational", action="store_true",
                     help="time one stage of the paper's variational solver (SURVEY.md section 8f next-1) at the workload's shape")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
                     help="only run the row-a2 site-contraction GEMM passes at the bulk-site shapes of bond CHI and "
                          "print their TFLOP/s (the command the ncu capture in profiles/ is taken on)")
     args = ap.parse_args()
-    global SKEW, EPS
+    global SKEW, EPS, SKETCH
     SKEW = args.convection == "skew"
+    SKETCH = args.sketch_seed if args.product_compression == "sketch" else None
     EPS = args.eps
     if args.impl == "reference":
         return run_reference(args)

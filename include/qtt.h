@@ -78,6 +78,22 @@ qtt_status qtt_ctx_set_graphs(qtt_ctx* ctx, int enabled);
  * 1: the paper's skew-symmetric form, PAPER.md:432-435 Eq. B2, 1/2 (u_j (.) D_j u_i + D_j (u_j (.) u_i)): per
  * right-hand side three more products (u_1 u_1, u_1 u_2, u_2 u_2), four more applies and 5-term sums. */
 qtt_status qtt_ctx_set_convection(qtt_ctx* ctx, int skew_symmetric);
+/* SURVEY.md section 8f next-4, "a cheaper product compression" (the repeated SVDs are what the paper wants
+ * replaced; reading 25).  mode 0 (default): every truncating step of the zip-up (qtt_round of a product handle,
+ * the products inside qtt_rk4_step) keeps the chi_work largest left singular vectors of T_l (4 r_l x a_{l+1} b_{l+1}).
+ * mode 1: at the sites where chi_work < min(4 r_l, a_{l+1} b_{l+1}) and c = 4^(n-1-l) satisfies c >= 2 chi_work or
+ * c <= chi_work, it keeps an orthonormal basis Q of range(T_l S_{l+1}) instead.  The probes are a random tensor train over
+ * the PHYSICAL indices with bond P = chi_work and sign cores G_k[w][u][t] = +-1/sqrt(P), (seed, site k, row w P + u,
+ * column t) -> sign by the counter-based generator the oracle implements too (oracle sketch_signs, sketch_mixers);
+ * S_{l+1} (a_{l+1} b_{l+1} x P) is that train contracted through the product's own cores from the last site down to l+1
+ * (oracle sketch_probes): a function of the state, not of the gauge of its bonds.  Q spans the numerical range only
+ * (singular values of the sketch above 8 eps ||.||_F; the other columns are zero).  Cost per site: three DMMA GEMMs for
+ * S_l, one for the sketch, and the SVD step of a chi_work x 4 r_l matrix -- instead of the LQ of T_l and the SVD of its
+ * 4 r_l x 4 r_l factor.  The result is the projection of T_l on a random chi_work-dimensional subspace of the range of
+ * the true unfolding, not the truncated SVD of T_l: error <= ~sqrt(2) x the optimal rank-chi_work/2 tail in expectation
+ * (Halko-Martinsson-Tropp), nothing lost where c <= chi_work or rank(T_l) <= chi_work.  seed is any 64-bit value.  Takes
+ * effect at the next call; graphs are re-captured.  Errors: QTT_INVALID_ARG for a NULL ctx or mode outside {0, 1}. */
+qtt_status qtt_ctx_set_product_compression(qtt_ctx* ctx, int mode, unsigned long long seed);
 /* Synchronises the stream and reports the Jacobi convergence record since the last call:
  * the largest number of sweeps any SVD used, and how many SVDs hit the sweep limit (then QTT_NUMERIC). */
 qtt_status qtt_ctx_jacobi_stats(qtt_ctx* ctx, int* max_sweeps, int* limit_hits);

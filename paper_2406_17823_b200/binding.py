@@ -335,6 +335,11 @@ def qtt_ctx_set_convection(ctx: Context, skew_symmetric: bool) -> None:
     ctx.check(ctx.lib.qtt_ctx_set_convection(ctx.h, 1 if skew_symmetric else 0))
 
 
+def qtt_ctx_set_product_compression(ctx: Context, sketch: bool, seed: int = 0) -> None:
+    """False: truncated SVD in the zip-up (default); True: randomised range finder with sign probes (reading 25)."""
+    ctx.check(ctx.lib.qtt_ctx_set_product_compression(ctx.h, 1 if sketch else 0, int(seed)))
+
+
 def qtt_ctx_set_graphs(ctx: Context, enabled: bool) -> None:
     ctx.check(ctx.lib.qtt_ctx_set_graphs(ctx.h, 1 if enabled else 0))
 

@@ -166,7 +166,8 @@ struct Rk4Plan {
   std::vector<int> rin[2], rout[2];
   const MpoData *Dx, *Dy, *Lap;
   double Re, dt;
-  int chi, chi_work, skew;
+  int chi, chi_work, skew, sketch;
+  unsigned long long sketch_seed;
   double* in_buf[2] = {nullptr, nullptr};
   double* out_buf[2] = {nullptr, nullptr};
   cudaGraph_t graph = nullptr;
@@ -347,6 +348,12 @@ qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes) {
 qtt_status qtt_ctx_set_convection(qtt_ctx* ctx, int skew_symmetric) {
   if (!ctx || (skew_symmetric != 0 && skew_symmetric != 1)) return QTT_INVALID_ARG;
   ctx->skew = skew_symmetric;
+  return QTT_OK;
+}
+qtt_status qtt_ctx_set_product_compression(qtt_ctx* ctx, int mode, unsigned long long seed) {
+  if (!ctx || (mode != 0 && mode != 1)) return QTT_INVALID_ARG;
+  ctx->sketch = mode;
+  ctx->sketch_seed = seed;
   return QTT_OK;
 }
 qtt_status qtt_ctx_set_graphs(qtt_ctx* ctx, int enabled) {
@@ -713,7 +720,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
   Rk4Plan* plan = nullptr;
   for (Rk4Plan* p : ctx->plans)
     if (p->rin[0] == uv[0].r && p->rin[1] == uv[1].r && p->Dx == Dx->data && p->Dy == Dy->data &&
-        p->Lap == Lap->data && p->Re == Re && p->dt == dt && p->chi == chi_max && p->chi_work == cw && p->skew == ctx->skew &&
+        p->Lap == Lap->data && p->Re == Re && p->dt == dt && p->chi == chi_max && p->chi_work == cw && p->skew == ctx->skew && p->sketch == ctx->sketch && p->sketch_seed == ctx->sketch_seed &&
         p->lo0 == ctx->arena.lo && p->hi0 == ctx->arena.hi)
       plan = p;
   if (!plan) {
@@ -726,6 +733,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
     plan->Dx = Dx->data; plan->Dy = Dy->data; plan->Lap = Lap->data;
     ++Dx->data->refs; ++Dy->data->refs; ++Lap->data->refs;
     plan->Re = Re; plan->dt = dt; plan->chi = chi_max; plan->chi_work = cw; plan->skew = ctx->skew;
+    plan->sketch = ctx->sketch; plan->sketch_seed = ctx->sketch_seed;
     plan->lo0 = ctx->arena.lo; plan->hi0 = ctx->arena.hi;
     for (int i = 0; i < 2; ++i) plan->rin[i] = uv[i].r;
     rk4_out_bonds(plan->rin, Dx->data, Dy->data, Lap->data, chi_max, cw, ctx->skew, plan->rout);

@@ -178,6 +178,8 @@ cudaError_t qtt_launch_transpose(const double* src, int rows, int cols, int lds,
 cudaError_t qtt_launch_copy2d(const double* src, int rows, int cols, int lds, double* dst, int ldd,
                               cudaStream_t stream);
 cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t stream);
+// X[a][w][b][t] *= x_t[w], the sign vector of probe t at site `site` of the sketched zip-up (movement.cu; a < na, b < nbp, t < P)
+cudaError_t qtt_launch_sketch_mixers(unsigned long long seed, int site, double* G, int P, cudaStream_t stream);
 // Diagnostics (spectrum.cu): unnormalised 2-D DFT of a real N x N field (complex output, interleaved re/im, transposed
 // wave-number order; tmp_c: 2 N^2 doubles) and the shell sums of the TKE spectrum (Eq. 13-15).
 cudaError_t qtt_launch_fft2_real(const double* F, double* out_c, double* tmp_c, int nbits, cudaStream_t stream);

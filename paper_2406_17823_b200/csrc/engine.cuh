@@ -93,6 +93,8 @@ struct qtt_ctx {
   size_t mat_limit = (size_t)2 << 30;
   int graphs = 1;
   int skew = 0;  // 1: skew-symmetric convection (PAPER.md Eq. B2) in qtt_rk4_step
+  int sketch = 0;  // 1: the truncating steps of the zip-up use a randomised range finder (reading 25)
+  unsigned long long sketch_seed = 0;
   int profiling = 0;
   QttStats stats;           // this context's launch counter and profiler records (bound on entry of every qtt_* call)
   double* ones = nullptr;   // device: 1.0

@@ -249,3 +249,34 @@ cudaError_t qtt_launch_fill(double* dst, i64 n, double value, cudaStream_t strea
   }
   return cudaGetLastError();
 }
+
+// Sign vectors of the sketched zip-up (reading 25): probe t carries at site `site` the sign vector
+// Core of the random sign tensor train the sketched zip-up probes with (reading 25; oracle sketch_mixers):
+// G[c][t] = +-scale, c = w * P + u < 4 P, t < P, minus where the top bit of the splitmix64 finaliser of
+// seed * 0x9E3779B97F4A7C15 + site * 0xD1B54A32D192ED03 + c * 2^20 + t (mod 2^64) is set -- the counter-based generator the
+// oracle implements too (oracle sketch_signs); scale = 1 / sqrt(P) is one correctly rounded double on both sides, so the
+// two sides use bit-identical cores.
+__global__ void qtt_sketch_mixers_kernel(unsigned long long base, double* G, i64 n, int P, double scale) {
+  for (i64 idx = (i64)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (i64)gridDim.x * blockDim.x) {
+    const unsigned long long t = (unsigned long long)(idx % P);
+    const unsigned long long c = (unsigned long long)(idx / P);
+    unsigned long long z = base + (c << 20) + t;
+    z ^= z >> 30;
+    z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27;
+    z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    G[idx] = (z >> 63) ? -scale : scale;
+  }
+}
+cudaError_t qtt_launch_sketch_mixers(unsigned long long seed, int site, double* G, int P, cudaStream_t stream) {
+  const i64 n = 4ll * P * P;
+  if (n <= 0) return cudaSuccess;
+  if (P >= (1 << 20)) return cudaErrorInvalidValue;
+  const unsigned long long base = seed * 0x9E3779B97F4A7C15ull + (unsigned long long)site * 0xD1B54A32D192ED03ull;
+  int blocks = (int)((n + 255) / 256);
+  blocks = blocks > 148 * 8 ? 148 * 8 : blocks;
+  QttProf prof(QK_MOVE, stream, 8.0 * (double)n);
+  qtt_sketch_mixers_kernel<<<blocks, 256, 0, stream>>>(base, G, n, P, 1.0 / sqrt((double)P));
+  return cudaGetLastError();
+}

@@ -489,6 +489,73 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
     Rbuf[1][i] = ctx->arena.tmp(mx);
   }
   std::vector<GemmProb> g;
+  // ---- sketched zip-up (reading 25): where does each operand take the sketch, and the probes (a random sign tensor train of
+  //      bond P = chi_work over the physical indices) seen from every bond, right to left:
+  //      S_l[(a,b),t] = sum_{w,u} G_l[w][u,t] sum_{a',b'} A_l[a,w,a'] B_l[b,w,b'] S_{l+1}[(a',b'),u],   S_n = 1
+  std::vector<std::vector<char>> sk(nb, std::vector<char>(n, 0));
+  std::vector<std::vector<double*>> S(nb, std::vector<double*>(n + 1, nullptr));
+  if (ctx->sketch) {
+    const int P = chi_work;
+    int lmin_all = n;
+    for (int i = 0; i < nb; ++i) {
+      std::vector<int> rw, ro;
+      qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro);
+      int lmin = n;
+      for (int l = 0; l + 1 < n; ++l) {
+        const i64 m = 4ll * rw[l], kk = (i64)A[i].r[l + 1] * B[i].r[l + 1];
+        const int rem = n - 1 - l;
+        // configurations to the right: many (oversampled random range finder) or few (the probes span the whole range)
+        const bool enough = rem >= 16 || (1ll << (2 * rem)) >= 2ll * chi_work || (1ll << (2 * rem)) <= (i64)chi_work;
+        if (chi_work < std::min(m, kk) && enough) {
+          sk[i][l] = 1;
+          lmin = std::min(lmin, l);
+        }
+      }
+      if (lmin == n) continue;
+      lmin_all = std::min(lmin_all, lmin);
+      S[i][n] = ctx->arena.tmp((size_t)P);
+      QTT_CU(qtt_launch_fill(S[i][n], P, 1.0, ctx->stream));
+      for (int l = n - 1; l > lmin; --l) S[i][l] = ctx->arena.tmp((size_t)A[i].r[l] * B[i].r[l] * P);
+    }
+    for (int l = n - 1; l > lmin_all; --l) {
+      const size_t mark = ctx->arena.hi;
+      double* G = ctx->arena.tmp((size_t)4 * P * P);
+      QTT_CU(qtt_launch_sketch_mixers(ctx->sketch_seed, l, G, P, ctx->stream));
+      std::vector<double*> X(nb, nullptr), Z(nb, nullptr);
+      for (int i = 0; i < nb; ++i) {
+        if (!S[i][l]) continue;
+        const int a = A[i].r[l], a2 = A[i].r[l + 1], b2 = B[i].r[l + 1];
+        X[i] = ctx->arena.tmp((size_t)4 * a * b2 * P);
+        Z[i] = ctx->arena.tmp((size_t)4 * a * b2 * P);
+        // X[a][w][(b',u)] = sum_a' A[a,w,a'] S_{l+1}[a'][(b',u)]
+        g.push_back(gemm_nn(A[i].core[l], a2, S[i][l + 1], (i64)b2 * P, X[i], (i64)b2 * P, 4 * a, b2 * P, a2));
+      }
+      run_gemms(ctx, g);
+      for (int i = 0; i < nb; ++i) {
+        if (!S[i][l]) continue;
+        const int a = A[i].r[l], b2 = B[i].r[l + 1];
+        // Z[a][w][b'][t] = sum_u X[a][w][b'][u] G[w][u][t]      (rows (a,b') of the w-th slab; batched over w)
+        GemmProb p = gemm_base(X[i], G, Z[i], a * b2, P, P);
+        p.nbatch = 4;
+        p.a_div = b2; p.a_hi = 4 * (i64)b2 * P; p.a_lo = P; p.a_k = 1; p.a_bs = (i64)b2 * P;
+        p.b_k = P; p.b_n = 1; p.b_bs = (i64)P * P;
+        p.c_div = b2; p.c_hi = 4 * (i64)b2 * P; p.c_lo = P; p.c_n = 1; p.c_bs = (i64)b2 * P;
+        g.push_back(p);
+      }
+      run_gemms(ctx, g);
+      for (int i = 0; i < nb; ++i) {
+        if (!S[i][l]) continue;
+        const int a = A[i].r[l], b = B[i].r[l], b2 = B[i].r[l + 1];
+        // S_l[(a,b)][t] = sum_{(w,b')} B[b,(w,b')] Z[a][(w,b')][t]      (batched over a)
+        GemmProb p = gemm_nn(B[i].core[l], 4 * (i64)b2, Z[i], P, S[i][l], P, b, P, 4 * b2);
+        p.nbatch = a;
+        p.a_bs = 0; p.b_bs = 4 * (i64)b2 * P; p.c_bs = (i64)b * P;
+        g.push_back(p);
+      }
+      run_gemms(ctx, g);
+      ctx->arena.hi = mark;
+    }
+  }
   for (int l = 0; l < n; ++l) {
     const size_t site_mark = ctx->arena.hi;
     std::vector<double*> T(nb);
@@ -539,6 +606,25 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
       keep[i] = (int)std::min<i64>(std::min<i64>(m, kk), chi_work);
       Qt[i] = ctx->arena.keep((size_t)keep[i] * m);
       SvdJob j;
+      if (sk[i][l]) {
+        // cheaper compression (reading 25): Q = a basis of range(T S_{l+1}) with chi_work structured sign probes instead of the
+        // top-chi_work left singular vectors: one GEMM and the SVD step of a chi_work x m matrix instead of the LQ of T and the
+        // SVD of its m x m factor.   Yt[t][i] = sum_c S[c][t] T[i][c]
+        double* Yt = ctx->arena.tmp((size_t)keep[i] * m);
+        GemmProb p = gemm_base(S[i][l + 1], T[i], Yt, keep[i], m, (int)kk);
+        p.a_lo = 1; p.a_k = keep[i];
+        p.b_k = 1; p.b_n = kk;
+        p.c_lo = m; p.c_n = 1;
+        g.push_back(p);
+        j.X = Yt; j.p = keep[i]; j.q = m;
+        j.out = Qt[i]; j.r_cap = keep[i]; j.chi_max = keep[i];
+        j.sigma = nullptr;
+        j.rank = reinterpret_cast<int*>(ctx->arena.tmp(1));
+        j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
+        j.rank_deficient = true;
+        svd.push_back(j);
+        continue;
+      }
       if (m <= kk) {
         double* Tc = ctx->arena.tmp((size_t)m * kk);
         QTT_CU(cudaMemcpyAsync(Tc, T[i], sizeof(double) * (size_t)m * kk, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -556,6 +642,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
       j.delta_ptr = nullptr; j.delta_out = nullptr; j.delta_scale = 0.0;
       svd.push_back(j);
     }
+    run_gemms(ctx, g);  // (the sketches Y^T = Omega^T T^T, if any)
     run_lq(ctx, lq);
     run_svd(ctx, svd);
     // R' = Q^T T  (keep x kk), into the other carry buffer
