@@ -326,6 +326,7 @@ def run_ours(args):
                          "rel_diff_sketch_chi_vs_svd_2chi_one_step": nrm(ske, fine)}
         del det, ske, fine
         Q.qtt_ctx_set_product_compression(ctx, True, SKETCH)
+        Q.qtt_ctx_jacobi_stats(ctx)  # the validation record below is about the timed steps, not the 2 chi yardstick step
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
     def step():

@@ -37,6 +37,8 @@ where the paper is silent/garbled and the reading taken):
   O11 fidelity, chi_eps         PAPER.md:160 Eq. 12; Eq. 16-17 (diagnostics)
       tke_spectrum              PAPER.md:173-184 Eq. 13-15
   O12 variational_cost / variational_stage   PAPER.md:107-132 Sec. II.C; 437-452 Eq. B3-B6; 522-544 Eq. B20-B24
+  O13 sketch_signs / sketch_mixers / sketch_probes / sketch_factor / sketch_applies, round_product(sketch_seed=)
+                                PAPER.md:318 ("cheaper product compression"; reading 25: randomised range finder)
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
 grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
@@ -52,6 +54,9 @@ with a gap at chi_work, and the projected dense product as the state handed to t
 rule by hand-computed tails, brute-force minimality and a case where the 1/sqrt(n-1) split decides the rank.
 O12 (variational stage) is pinned in tests/test_oracle_variational.py by the dense normal equations of Theta,
 finite-difference stationarity at truncating bonds and the dense operator product.
+O13 (sketched zip-up) is pinned in tests/test_oracle_sketch.py by a big-integer restatement of the generator, the dense
+probe train, projector algebra, the range-finder bound against independent SVDs of the matrix and of the true unfolding,
+gauge invariance and the dense elementwise product.
 """
 from __future__ import annotations
 
