@@ -304,7 +304,12 @@ def sketch_probes(A, B, n_probes: int, seed: int):
     S[n] = np.ones((1, 1, n_probes))
     for l in range(n - 1, -1, -1):
         G = sketch_mixers(seed, l, n_probes)
-        S[l] = np.einsum("wut,awc,bwd,cdu->abt", G, A[l], B[l], S[l + 1], optimize=True)
+        a, b = A[l].shape[0], B[l].shape[0]
+        S[l] = np.zeros((a, b, n_probes))
+        for w in range(D_PHYS):  # the formula above, one physical index at a time (plain matrix products)
+            X = np.tensordot(A[l][:, w, :], S[l + 1], axes=([1], [0]))  # [a, b', u]
+            Z = X @ G[w]  # [a, b', t]
+            S[l] += np.tensordot(Z, B[l][:, w, :], axes=([1], [1])).transpose(0, 2, 1)  # [a, t, b] -> [a, b, t]
     return S
 
 
