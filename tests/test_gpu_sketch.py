@@ -134,3 +134,34 @@ def test_sketch_does_not_depend_on_the_gauge_of_the_operands(Q, ctx):
             h = Q.qtt_hadamard(ctx, g[j], gg)
             Q.qtt_round(ctx, h, chi)
             assert rel(gpu_dense(Q, ctx, h), O.to_dense(want)) <= TOL
+
+
+def test_config3_full_size_sketched_steps_match_oracle(Q):
+    """The launch configuration `bench.py --product-compression sketch` times (BASELINE config 3 shapes: 2^10 x 2^10, chi 64,
+    chi_work = P = 128, graph replay): two free-running steps against the oracle's sketched steps with the same seed, dense
+    1024 x 1024 fields; every kind of site occurs (many configurations to the right, few, and the deterministic ones between)."""
+    cfg = I.CONFIGS[3]
+    n, chi, seed = cfg["n"], cfg["chi"], 1
+    dx = 1.0 / (1 << n)
+    ux, uy = I.config_fields(3)
+    U = [O.from_dense(ux, chi), O.from_dense(uy, chi)]
+    ops_o = (O.mpo_d1(n, dx), O.mpo_d2(n, dx), O.mpo_laplacian(n, dx))
+    info = {}
+    O.round_product(U[0], U[1], chi, sketch_seed=seed, info=info)
+    kinds = {(z["branch"], 4 ** (n - 1 - l) >= 4 * chi) for l, z in enumerate(info["zip"])}
+    assert ("sketch", True) in kinds and ("sketch", False) in kinds
+    c = Q.Context(device=0, workspace_bytes=8 << 30)
+    try:
+        ops_g = (Q.qtt_mpo_central_difference(c, n, 1, dx), Q.qtt_mpo_central_difference(c, n, 2, dx), Q.qtt_mpo_laplacian(c, n, dx))
+        Q.qtt_ctx_set_graphs(c, True)
+        Q.qtt_ctx_set_product_compression(c, True, seed)
+        g = [Q.qtt_mps_from_cores(c, U[0]), Q.qtt_mps_from_cores(c, U[1])]
+        for step in range(2):
+            U = O.rk4_step(U, *ops_o, cfg["Re"], cfg["dt"], chi, sketch_seed=seed)
+            Q.qtt_rk4_step(c, g, *ops_g, cfg["Re"], cfg["dt"], chi)
+            for i in range(2):
+                assert Q.qtt_mps_bonds(g[i]) == O.bonds(U[i])
+                assert rel(gpu_dense(Q, c, g[i]), O.to_dense(U[i])) <= TOL, (step, i)
+        assert Q.qtt_ctx_jacobi_stats(c)[1] == 0
+    finally:
+        c.close()
