@@ -723,6 +723,9 @@ def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     a2 = [r for r in per_launch if r["family"] == "gemm" and r["shape"][1] == chi and r["shape"][2] == chi
           and r["shape"][0] in (4 * chi, 2 * chi * chi)]
     a2_ms, a2_work = sum(r["ms"] for r in a2), sum(r["work"] for r in a2)
+    if SKETCH is not None:
+        roofline_step["note"] = ("flop model of the DETERMINISTIC step (SURVEY.md section 8d) over the sketched step's time: the sketched "
+                                 "zip-up does less work than that, so this fraction overstates what the kernels achieve")
     out = {"roofline": roof, "roofline_step": roofline_step, "families": fams,
            "contraction_a2": {"tflops": a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12, "peak_tflops": peaks["dmma"],
                               "frac": (a2_work / max(a2_ms * 1e-3, 1e-12) * 1e-12) / peaks["dmma"] if peaks["dmma"] else None,

@@ -165,3 +165,25 @@ def test_config3_full_size_sketched_steps_match_oracle(Q):
         assert Q.qtt_ctx_jacobi_stats(c)[1] == 0
     finally:
         c.close()
+
+
+@pytest.mark.parametrize("skew,eps", [(True, 0.0), (False, 1e-6)])
+def test_sketch_composes_with_skew_convection_and_the_eps_rule(Q, ctx, skew, eps):
+    """The mode switch is orthogonal to the other two: the paper's skew-symmetric convection (7 products per right-hand side
+    through the sketched zip-up) and the eps rank rule (data-dependent ranks, eager launches)."""
+    n, chi, Re, dt, seed = 7, 6, 200.0, 1e-3, 17
+    dx = 1.0 / (1 << n)
+    Fa, Fb = fields(n, 8)
+    U = [O.from_dense(Fa, chi), O.from_dense(0.5 * Fb, chi)]
+    ops_o = (O.mpo_d1(n, dx), O.mpo_d2(n, dx), O.mpo_laplacian(n, dx))
+    ops_g = (Q.qtt_mpo_central_difference(ctx, n, 1, dx), Q.qtt_mpo_central_difference(ctx, n, 2, dx),
+             Q.qtt_mpo_laplacian(ctx, n, dx))
+    Q.qtt_ctx_set_convection(ctx, skew)
+    Q.qtt_ctx_set_product_compression(ctx, True, seed)
+    g = [Q.qtt_mps_from_cores(ctx, U[0]), Q.qtt_mps_from_cores(ctx, U[1])]
+    Q.qtt_rk4_step(ctx, g, *ops_g, Re, dt, chi, eps)
+    want = O.rk4_step(U, *ops_o, Re, dt, chi, eps=eps, skew=skew, sketch_seed=seed)
+    for i in range(2):
+        same = Q.qtt_mps_bonds(g[i]) == O.bonds(want[i])
+        assert same or eps > 0.0  # eps > 0: a tail within rounding distance of the threshold may fall on either side (reading 17)
+        assert rel(gpu_dense(Q, ctx, g[i]), O.to_dense(want[i])) <= (TOL if same else 10 * eps)
