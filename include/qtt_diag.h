@@ -21,6 +21,22 @@ int qtt_diag_gemm(void* stream, const double* A_dev, const double* B_dev, double
  * scratch_dev: batch * 3 * 64 * m doubles.  SURVEY.md section 8 row a4. */
 int qtt_diag_lq(void* stream, double* Y_dev, int batch, int k, int m, int ld, double* R_dev, double* scratch_dev);
 
+/* qtt_diag_lq for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same kernels and launch sequence, with the scratch of the blocked path in a device array
+ * that is part of the library image (QTT_LQ_NOALLOC_MAX_DOUBLES doubles = 6 MiB, held by every GPU that loads the library
+ * until the process exits).  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ * Arguments as qtt_diag_lq (device pointers, caller-owned: Y_dev destroyed unless small, R_dev <- batch k x k factors),
+ * 1 <= batch <= 16, k <= m <= ld.  Limit: matrices too large for the cluster-resident kernel need batch * 3 * 64 * m doubles
+ * of scratch, so batch * m <= 4096; beyond that the call launches nothing, prints the reason to stderr and returns
+ * QTT_NOALLOC_TOO_LARGE (use qtt_diag_lq with your own buffer).  QTT_NOALLOC_BAD_ARG for NULL pointers or sizes out of
+ * range; otherwise 0 or a cudaError_t value.  All calls share the one array (per device) and it keeps the previous call's
+ * contents: the part a call uses is cleared on `stream` first, and calls that OVERLAP on the GPU (different streams without
+ * a dependency between them) race on it -- keep them on one stream or order them with events.  SURVEY.md section 8 row a4. */
+#define QTT_LQ_NOALLOC_MAX_DOUBLES 786432 /* 3 * 64 * 4096 */
+#define QTT_NOALLOC_BAD_ARG (-1)
+#define QTT_NOALLOC_TOO_LARGE (-2)
+int qtt_lq_noalloc(void* stream, double* Y_dev, int batch, int k, int m, int ld, double* R_dev);
+
 /* One-sided Jacobi on the rows of `batch` matrices X_i (p x q, ld, stride p*ld), in place: rows of the result
  * are mutually orthogonal (X = J^T Sigma V^T).  status_dev: 2 ints (zero them first): [0] <- max sweeps,
  * [1] += matrices that hit the sweep limit.  SURVEY.md section 8 row a5. */

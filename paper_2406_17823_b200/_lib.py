@@ -76,6 +76,7 @@ PROTOTYPES = {
                                 C.c_longlong, C.c_longlong, C.c_double, C.c_double, C.c_int, C.c_longlong,
                                 C.c_longlong, C.c_longlong]),
     "qtt_diag_lq": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
+    "qtt_lq_noalloc": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P]),
     "qtt_diag_rowjacobi": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P]),
     "qtt_diag_rowjacobi_streamed": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
     "qtt_diag_svd_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),

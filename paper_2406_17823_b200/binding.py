@@ -371,3 +371,27 @@ def qtt_ctx_profile_report(ctx: Context) -> dict:
     ms, work, cnt = (C.c_double * n)(), (C.c_double * n)(), (C.c_longlong * n)()
     ctx.check(ctx.lib.qtt_ctx_profile_report(ctx.h, ms, work, cnt))
     return {f: {"ms": ms[i], "work": work[i], "launches": int(cnt[i])} for i, f in enumerate(PROF_FAMILIES)}
+
+
+LQ_NOALLOC_MAX_DOUBLES = 3 * 64 * 4096  # include/qtt_diag.h QTT_LQ_NOALLOC_MAX_DOUBLES
+
+
+def qtt_lq_noalloc(Y: torch.Tensor, R: torch.Tensor, stream: "torch.cuda.Stream | None" = None) -> None:
+    """include/qtt_diag.h qtt_lq_noalloc: Q-less LQ of the batch Y (batch x k x m, fp64, CUDA, contiguous; destroyed) into R
+    (batch x k x k) without any device allocation by the library: its scratch is a 6 MiB device array built into the library
+    (matrices too large for the cluster-resident kernel: batch * m <= 4096).  Calls that overlap on the GPU race on it."""
+    if Y.dim() != 3 or R.dim() != 3 or not (Y.is_cuda and R.is_cuda and Y.is_contiguous() and R.is_contiguous()) \
+            or Y.dtype != torch.float64 or R.dtype != torch.float64:
+        raise ValueError("qtt_lq_noalloc wants contiguous fp64 CUDA tensors Y (batch, k, m) and R (batch, k, k)")
+    batch, k, m = Y.shape
+    if tuple(R.shape) != (batch, k, k):
+        raise ValueError(f"R must be {(batch, k, k)}, got {tuple(R.shape)}")
+    st = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = _lib.load().qtt_lq_noalloc(C.c_void_p(st), C.c_void_p(Y.data_ptr()), batch, k, m, m, C.c_void_p(R.data_ptr()))
+    if rc == -2:
+        raise ValueError(f"qtt_lq_noalloc: batch {batch} x m {m} exceeds the built-in scratch ({LQ_NOALLOC_MAX_DOUBLES} doubles: "
+                         f"batch * m <= 4096); use qtt_diag_lq with a caller-allocated buffer")
+    if rc == -1:
+        raise ValueError(f"qtt_lq_noalloc: invalid sizes (1 <= batch {batch} <= 16, 1 <= k {k} <= m {m} <= 16384)")
+    if rc != 0:
+        raise RuntimeError(f"qtt_lq_noalloc: CUDA error {rc}")

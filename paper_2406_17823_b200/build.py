@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqtt_b200.so")
-SOURCES = ["gemm.cu", "movement.cu", "lq.cu", "jacobi.cu", "bj2.cu", "sbj.cu", "qrcp.cu", "sweeps.cu", "api.cu", "operators.cu", "spectrum.cu", "variational.cu", "probe.cu"]
+SOURCES = ["gemm.cu", "movement.cu", "lq.cu", "jacobi.cu", "bj2.cu", "sbj.cu", "qrcp.cu", "sweeps.cu", "api.cu", "operators.cu", "spectrum.cu", "variational.cu", "probe.cu", "noalloc.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC",
