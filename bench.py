@@ -592,7 +592,7 @@ def variational_bench(args):
     peaks = fp64_peaks(Q, ctx)
     times, infos = [], []
     th0 = Q.qtt_variational_cost(ctx, a, a, B, Dx, Dy, h, mu)
-    for rep in range(2 + max(args.steps, 1)):  # 0: warm-up, 1: profiled (event pair per launch, not timed), 2..: timed
+    for rep in range(3 + max(args.steps, 1)):  # 0: warm-up, 1: profiled (event pair per launch), 2: warm-up again, 3..: timed
         v = [Q.qtt_mps_clone(ctx, x) for x in a]
         if rep == 1:
             Q.qtt_ctx_profile(ctx, True)
@@ -601,7 +601,7 @@ def variational_bench(args):
         t0 = time.perf_counter()
         info = Q.qtt_variational_stage(ctx, v, a, B, Dx, Dy, h, mu)
         ctx.synchronize()
-        if rep >= 2:
+        if rep >= 3:
             times.append(time.perf_counter() - t0)
             infos.append(info)
         if rep == 1:
