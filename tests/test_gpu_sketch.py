@@ -187,3 +187,28 @@ def test_sketch_composes_with_skew_convection_and_the_eps_rule(Q, ctx, skew, eps
         same = Q.qtt_mps_bonds(g[i]) == O.bonds(want[i])
         assert same or eps > 0.0  # eps > 0: a tail within rounding distance of the threshold may fall on either side (reading 17)
         assert rel(gpu_dense(Q, ctx, g[i]), O.to_dense(want[i])) <= (TOL if same else 10 * eps)
+
+
+def test_sketch_edge_cases_short_chains_and_a_zero_operand(Q, ctx):
+    """Chains too short for any site to satisfy the rule fall back to the deterministic zip-up; a zero operand gives a zero
+    product (the sketch of a zero matrix has rank 0: every basis column is zero)."""
+    Q.qtt_ctx_set_product_compression(ctx, True, 5)
+    for n in (1, 2, 3):
+        Fa, Fb = fields(n, n)
+        A, B = O.from_dense(Fa, 4), O.from_dense(Fb, 4)
+        info = {}
+        want = O.round_product(A, B, 2, chi_work=2, sketch_seed=5, info=info)
+        h = Q.qtt_hadamard(ctx, Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, B))
+        Q.qtt_round_ex(ctx, h, 2, 0.0, 2)
+        assert rel(gpu_dense(Q, ctx, h), O.to_dense(want)) <= TOL
+    n, chi = 7, 6
+    Fa, _ = fields(n, 4)
+    A = O.from_dense(Fa, chi)
+    Z = [np.zeros_like(c) for c in A]
+    info = {}
+    want = O.round_product(A, Z, chi, sketch_seed=5, info=info)
+    assert "sketch" in [z["branch"] for z in info["zip"]] and np.all(O.to_dense(want) == 0.0)
+    h = Q.qtt_hadamard(ctx, Q.qtt_mps_from_cores(ctx, A), Q.qtt_mps_from_cores(ctx, Z))
+    Q.qtt_round(ctx, h, chi)
+    got = gpu_dense(Q, ctx, h)
+    assert np.all(np.isfinite(got)) and np.all(got == 0.0)
