@@ -136,11 +136,11 @@ def from_dense(F: np.ndarray, chi_max: int = 1 << 30, eps: float = 0.0):
 
 def to_tensor(cores) -> np.ndarray:
     """Contract an MPS to the full tensor U[w_1..w_n] (Eq. 4)."""
-    T = cores[0].reshape(D_PHYS, -1)
+    T = cores[0].reshape(cores[0].shape[1], -1)
     for c in cores[1:]:
         r0, d, r1 = c.shape
         T = (T @ c.reshape(r0, d * r1)).reshape(-1, r1)
-    return T.reshape((D_PHYS,) * len(cores))
+    return T.reshape((cores[0].shape[1],) * len(cores))
 
 
 def to_dense(cores) -> np.ndarray:
@@ -195,7 +195,7 @@ def lincomb(terms):
         else:
             rl = sum(c.shape[0] for c in cs)
             rr = sum(c.shape[2] for c in cs)
-            blk = np.zeros((rl, D_PHYS, rr))
+            blk = np.zeros((rl, cs[0].shape[1], rr))
             i = j = 0
             for c in cs:
                 blk[i : i + c.shape[0], :, j : j + c.shape[2]] = c
@@ -393,7 +393,7 @@ def round_product(A, B, chi_max: int, eps: float = 0.0, chi_work: int | None = N
         cores.append(Q.reshape(r, d, rn))
         R = Rn.reshape(rn, a2, b2)
     T4 = np.einsum("rab,awc,bwd->rwcd", R, A[n - 1], B[n - 1], optimize=True)
-    cores.append(T4.reshape(T4.shape[0], D_PHYS, 1))
+    cores.append(T4.reshape(T4.shape[0], T4.shape[1], 1))
     if info is not None:
         info["zip"] = zip_log
         info["zip_cores"] = [c.copy() for c in cores]  # Q_1..Q_{n-1}, T_n: the state the R->L sweep starts from

@@ -95,6 +95,20 @@ def decaying_turbulence(n: int = 11, seed: int = 0, k0: float = 16.0):
     return ux * scale, uy * scale
 
 
+def taylor_green_3d(n: int = 4, seed: int = 0, noise: float = 1e-3):
+    """3D stand-in workload (PAPER.md:320-322 names the 3D Taylor-Green vortex of ref. [13]): arrays F[x][y][z] on
+    [0, 1)^3, u = (sin X cos Y cos Z, -cos X sin Y cos Z, 0) with X = 2 pi x etc., plus ``noise`` * N(0,1) (seeded) on
+    every component so that the bonds are not the closed-form ones."""
+    N = 1 << n
+    t = 2.0 * np.pi * np.arange(N, dtype=np.float64) / N
+    X, Y, Z = np.meshgrid(t, t, t, indexing="ij")
+    rng = np.random.default_rng(seed)
+    u1 = np.sin(X) * np.cos(Y) * np.cos(Z) + noise * rng.standard_normal((N, N, N))
+    u2 = -np.cos(X) * np.sin(Y) * np.cos(Z) + noise * rng.standard_normal((N, N, N))
+    u3 = noise * rng.standard_normal((N, N, N))
+    return u1, u2, u3
+
+
 def bond_profile(n: int, chi: int, d: int = 4):
     """Bonds r_0..r_n with r_0 = r_n = 1 and r_l = min(d^l, d^(n-l), chi)."""
     return [1] + [int(min(d**l, d ** (n - l), chi)) for l in range(1, n)] + [1]
