@@ -40,6 +40,10 @@ where the paper is silent/garbled and the reading taken):
   O13 sketch_signs / sketch_mixers / sketch_probes / sketch_factor / sketch_applies, round_product(sketch_seed=)
                                 PAPER.md:318 ("cheaper product compression"; reading 25: randomised range finder)
 
+  P1-P4 (oracle/qtt_oracle_3d.py) the 3D encoding with physical dimension 8: encode3, from_dense3, mpo_stencil3 / mpo_d3 /
+                                mpo_laplacian3, rhs3 / rk4_step3 (reading 26); O3-O7 here read the
+                                physical dimension off the core shapes and serve both encodings
+
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense brute force on 2^4..2^6
 grids, Table II golden entries (tests/golden/), circulant stencil of Eq. 6,
 analytic finite-difference of sin/cos, bond-2 closed forms, the root-sum-square

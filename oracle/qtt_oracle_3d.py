@@ -108,32 +108,45 @@ def mpo_stencil3(n: int, direction: int, coeffs):
     return cores
 
 
+def _channel_core3(channels):
+    """Bulk core of Table II for a list of channels (coordinate j, shift s = +-1); channel 0 = identity.
+    A channel c > 0 at a site flips the bit of its coordinate (input bit = output bit + s mod 2) and stays in c when the
+    addition carries on to the more significant site (s = +1: output bit 1; s = -1: output bit 0), else falls to channel 0
+    -- the entries alpha_{m+1} = 1, 2 of Table II, with the bit of coordinate j in place of the x bit."""
+    D = 1 + len(channels)
+    C = np.zeros((D, D3, D3, D))
+    for w in range(D3):
+        C[0, w, w, 0] = 1.0
+    for c, (j, shift) in enumerate(channels, start=1):
+        pos = 3 - j
+        for w in range(D3):
+            b = (w >> pos) & 1
+            wp = w ^ (1 << pos)
+            onward = (b == 1) if shift > 0 else (b == 0)
+            C[c if onward else 0, w, wp, c] = 1.0
+    return C
+
+
+def _fold3(C, n, R):
+    cores = [C.copy() for _ in range(n)]
+    cores[0] = np.einsum("a,awvb->wvb", np.ones(C.shape[0]), C)[None]   # L = ones on the most-significant end
+    cores[-1] = np.einsum("awvb,b->awv", C, np.asarray(R, dtype=np.float64))[..., None]  # R on the least-significant end
+    return cores
+
+
 def mpo_d3(n: int, direction: int, dx: float):
-    """Central difference along one direction (PAPER.md:395-404 Eq. A1-A3): (F[x+1] - F[x-1]) / (2 dx), bond 3."""
-    return mpo_stencil3(n, direction, np.array([-1.0, 0.0, 1.0]) / (2.0 * dx))
+    """Central difference along one direction (PAPER.md:395-404 Eq. A1-A3): (F[x+1] - F[x-1]) / (2 dx), bond 3, channels
+    identity / +1 / -1 as in Table II, L = (1,1,1), R = (0, 1, -1) / (2 dx)."""
+    assert direction in (1, 2, 3) and n >= 2
+    return _fold3(_channel_core3([(direction, +1), (direction, -1)]), n, np.array([0.0, 1.0, -1.0]) / (2.0 * dx))
 
 
 def mpo_laplacian3(n: int, dx: float):
     """7-point Laplacian, bond 7 (reading 3 with three coordinates): channel 0 = identity, channels 2j-1 / 2j = shift
-    by +1 / -1 along direction j; a channel c > 0 at a site flips the bit of its coordinate and stays in c when the
-    addition carries on, else falls to channel 0; L = ones, R = (-6, 1, 1, 1, 1, 1, 1) / dx^2."""
-    D = 7
-    C = np.zeros((D, D3, D3, D))
-    for w in range(D3):
-        C[0, w, w, 0] = 1.0
-    for j in (1, 2, 3):
-        pos = 3 - j
-        for c, shift in ((2 * j - 1, +1), (2 * j, -1)):
-            for w in range(D3):
-                b = (w >> pos) & 1          # output bit; input = output + shift
-                wp = w ^ (1 << pos)
-                onward = (b == 1) if shift > 0 else (b == 0)
-                C[c if onward else 0, w, wp, c] = 1.0
-    cores = [C.copy() for _ in range(n)]
-    cores[0] = np.einsum("a,awvb->wvb", np.ones(D), C)[None]
-    R = np.array([-6.0, 1, 1, 1, 1, 1, 1]) / dx**2
-    cores[-1] = np.einsum("awvb,b->awv", C, R)[..., None]
-    return cores
+    by +1 / -1 along direction j; L = ones, R = (-6, 1, 1, 1, 1, 1, 1) / dx^2."""
+    assert n >= 2
+    ch = [(j, s) for j in (1, 2, 3) for s in (+1, -1)]
+    return _fold3(_channel_core3(ch), n, np.array([-6.0, 1, 1, 1, 1, 1, 1]) / dx**2)
 
 
 # --------------------------------------------------------------------------- P4

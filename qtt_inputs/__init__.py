@@ -22,4 +22,5 @@ from .fields import (  # noqa: F401
     random_cores,
     bond_profile,
     config_fields,
+    taylor_green_3d,
 )

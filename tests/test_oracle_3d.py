@@ -79,7 +79,18 @@ def test_mpo_d3_is_the_rolled_central_difference(direction):
     ax = direction - 1
     ref = (np.roll(F, -1, axis=ax) - np.roll(F, 1, axis=ax)) / (2 * dx)
     assert _rel(G, ref) < 1e-13
-    # a wrong sign of the shift, a transposed operator or a wrong coordinate all fail: check one entry by hand
+    # the same operator built as a stencil MPO (another bond basis: carries -1, 0, +1)
+    S = o3.to_dense3(o2.apply_mpo(o3.mpo_stencil3(n, direction, np.array([-1.0, 0.0, 1.0]) / (2 * dx)), A))
+    assert _rel(G, S) < 1e-13
+    # the bulk core restricted to a field that does not depend on the other two coordinates is Table II verbatim
+    if direction == 1:
+        C = o3._channel_core3([(1, +1), (1, -1)])
+        T2 = np.zeros((3, 4, 4, 3))
+        for am, am1, w, wp in o2._TABLE_II:
+            T2[am, w, wp, am1] = 1.0
+        # omega_3d = 2 * omega_2d + z_bit: take z_bit = 0 on both sides
+        assert np.array_equal(C[:, 0::2, 0::2, :], T2)
+
     idx = [2, 5, 7]
     ip, im = list(idx), list(idx)
     ip[ax] = (idx[ax] + 1) % N
