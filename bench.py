@@ -624,6 +624,71 @@ def variational_bench(args):
     return 0
 
 
+def three_d_bench(args):
+    """SURVEY.md section 8f next-4 (reading 26): one right-hand side of the 3D Burgers equations in the d = 8
+    encoding, composed from the batched C-ABI primitives as a caller would -- f_i = -sum_j u_j (.) D_j u_i + (1/Re) Lap u_i,
+    i = 1..3: one batch of 12 apply + round, one of 9 zip-ups, one of 3 four-term sums -- on the Taylor-Green vortex plus seeded
+    noise (qtt_inputs.taylor_green_3d) at 2^n points per direction.  Device-timed with CUDA events on the context's stream
+    (eager launches: no graph for the composed path).  Prints ONE JSON line."""
+    import torch
+    import paper_2406_17823_b200 as Q
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    n, chi, Re = args.three_d, args.three_d_chi, 1600.0
+    ctx = Q.Context(device=0, workspace_bytes=int(args.workspace_gib * (1 << 30)))
+    Q.qtt_ctx_set_phys_dim(ctx, 8)
+    dx = 1.0 / (1 << n)
+    Dj = [Q.qtt_mpo_central_difference(ctx, n, j, dx) for j in (1, 2, 3)]
+    Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
+    u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in I.taylor_green_3d(n, seed=0, noise=1e-3)]
+
+    def rhs():
+        g = [[Q.qtt_apply_mpo(ctx, Dj[j], u[i]) for j in range(3)] for i in range(3)]
+        lap = [Q.qtt_apply_mpo(ctx, Lap, u[i]) for i in range(3)]
+        Q.qtt_round_batch(ctx, [x for row in g for x in row] + lap, chi)
+        c = [[Q.qtt_hadamard(ctx, u[j], g[i][j]) for j in range(3)] for i in range(3)]
+        Q.qtt_round_batch(ctx, [x for row in c for x in row], chi)
+        for i in range(3):  # Re * f_i = lap - Re (c_i1 + c_i2 + c_i3): qtt_axpy weights the term it adds
+            for j in (2, 1, 0):
+                Q.qtt_axpy(ctx, -Re, c[i][j], lap[i])
+        Q.qtt_round_batch(ctx, lap, chi)
+        return lap
+
+    peaks = fp64_peaks(Q, ctx)
+    times = []
+    for rep in range(args.warmup + max(args.steps, 1)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctx.synchronize()
+        l0 = Q.qtt_ctx_launch_count(ctx)
+        e0.record(ctx.stream)
+        f = rhs()
+        e1.record(ctx.stream)
+        ctx.synchronize()
+        if rep >= args.warmup:
+            times.append(e0.elapsed_time(e1))
+        launches = Q.qtt_ctx_launch_count(ctx) - l0
+    Q.qtt_ctx_profile(ctx, True)
+    Q.qtt_ctx_profile_report(ctx)
+    f = rhs()
+    fam = Q.qtt_ctx_profile_report(ctx)
+    Q.qtt_ctx_profile(ctx, False)
+    sweeps, hits = Q.qtt_ctx_jacobi_stats(ctx)
+    ms = float(np.median(times))
+    g = fam["gemm"]
+    line = {"metric": "3D Burgers right-hand sides/s at 2^%d^3, d=8, chi=%d fp64" % (n, chi), "value": 1e3 / ms, "unit": "rhs/s",
+            "ms_per_rhs": ms, "n_gpus": 1, "steps": len(times), "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "Taylor-Green vortex + 1e-3 N(0,1) on a 2^%d cube (%d sites, d=8), chi_max=%d, chi_work=%d, "
+                                   "Re=%g: 12 apply+round, 9 zip-ups, 3 four-term sums, batched per level" % (n, n, chi, 2 * chi, Re),
+                       "timing": "CUDA events on the context's stream around the eagerly launched composition, median"},
+            "bonds": Q.qtt_mps_bonds(f[0]), "norms": [Q.qtt_mps_norm(ctx, x) for x in f],
+            "gpu_launches": int(launches), "jacobi_max_sweeps": sweeps, "jacobi_limit_hits": hits,
+            "family_ms": {k: round(v["ms"], 3) for k, v in fam.items()},
+            "gemm_tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12,
+            "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"], "fp64_peaks_tflops": peaks}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def roofline_and_baseline(Q, ctx, u, ops, c, chi, args, ms_per_step):
     """Per-kernel-family device times of one more (eagerly launched, event-bracketed) step -> roofline of the
     dominant family; the site-contraction TFLOP/s; and the CPU oracle timed on a bounded sample."""
@@ -768,6 +833,9 @@ def main():
                          "SURVEY.md section 8f next-4 (DESIGN.md reading 25) at the sites its rule admits -- another method, "
                          "reported with its one-step distance to the deterministic result")
     ap.add_argument("--sketch-seed", type=int, default=1)
+    ap.add_argument("--three-d", type=int, default=0, metavar="NBITS",
+                    help="time one 3D Burgers right-hand side in the d = 8 encoding on a 2^NBITS cube (SURVEY.md section 8f next-4)")
+    ap.add_argument("--three-d-chi", type=int, default=32)
     ap.add_argument("--variational", action="store_true",
                     help="time one stage of the paper's variational solver (SURVEY.md section 8f next-1) at the workload's shape")
     ap.add_argument("--probe-contraction", type=int, default=0, metavar="CHI",
@@ -782,6 +850,8 @@ def main():
         return run_reference(args)
     if args.primitive_sweep:
         return primitive_sweep(args)
+    if args.three_d:
+        return three_d_bench(args)
     if args.variational:
         return variational_bench(args)
     if args.probe_contraction:

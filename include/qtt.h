@@ -69,6 +69,19 @@ void qtt_ctx_destroy(qtt_ctx* ctx);
 const char* qtt_last_error(const qtt_ctx* ctx);
 /* Working bond chi_work of the fused Hadamard+round ("zip-up", reading 8); 0 = 2*chi_max. */
 qtt_status qtt_ctx_set_chi_work(qtt_ctx* ctx, int chi_work);
+/* SURVEY.md section 8f next-4, "3D (d = 8) encoding" ("the methods outlined here can be generalized to 3D",
+ * PAPER.md:320-322; reading 26).  Physical dimension of every site of this context's MPS / MPO handles: 4
+ * (default) = the 2D quantics encoding of PAPER.md Eq. 3, w_k = 2 x_k + y_k; 8 = a 2^n x 2^n x 2^n grid with
+ * w_k = 4 x_k + 2 y_k + z_k (the bits of one length scale share a site, bit 1 most significant).  With d = 8:
+ * qtt_mps_from_dense / qtt_to_dense take dense_dev[(x*N + y)*N + z] (n_bits <= 9), cores are r x 8 x r', MPO cores
+ * D x 8 x 8 x D', the MPO builders accept direction 1, 2, 3 (x, y, z) and qtt_mpo_laplacian is the 7-point stencil of
+ * bond 7; qtt_apply_mpo, qtt_hadamard, qtt_axpy, qtt_round / qtt_round_batch / qtt_round_ex (zip-up included), qtt_mps_dot /
+ * norm / schmidt / fidelity / chi_eps / clone / get_core run the same kernels on d r-row unfoldings.  qtt_rk4_step,
+ * qtt_variational_*, qtt_tke_spectrum and the sketched product compression are built for two velocity components on a 2D
+ * grid and return QTT_INVALID_ARG when d = 8 (a 3D right-hand side is composed from the calls above).
+ * Errors: QTT_INVALID_ARG for d outside {4, 8}, or for a switch while MPS / MPO handles of the context are alive. */
+qtt_status qtt_ctx_set_phys_dim(qtt_ctx* ctx, int d);
+int qtt_ctx_phys_dim(const qtt_ctx* ctx); /* 4 or 8; 0 for a NULL context */
 /* Largest lazy result (bytes of all cores) that qtt_to_dense / qtt_mps_get_core may materialise. */
 qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes);
 /* 1: qtt_rk4_step with eps == 0 is captured once into a CUDA graph per shape signature and replayed
@@ -111,29 +124,31 @@ qtt_status qtt_ctx_profile_report(qtt_ctx* ctx, double* ms_host, double* work_ho
 long long qtt_ctx_launch_count(const qtt_ctx* ctx);
 
 /* PAPER.md:67-72 Eq. 4 (reading 9): right-to-left TT-SVD of the dense field dense_dev[x*N + y], N = 2^n_bits,
- * keeping per bond r = rank rule(chi_max, eps) (see qtt_round). */
+ * keeping per bond r = rank rule(chi_max, eps) (see qtt_round).  (Physical dimension 8: dense_dev[(x*N + y)*N + z].) */
 qtt_status qtt_mps_from_dense(qtt_ctx* ctx, const double* dense_dev, int n_bits, int chi_max, double eps,
                               qtt_mps** out);
-/* Upload explicit cores (host arrays, core k is bonds[k] x 4 x bonds[k+1] row-major, bonds has n+1 entries). */
+/* Upload explicit cores (host arrays, core k is bonds[k] x d x bonds[k+1] row-major, d = qtt_ctx_phys_dim, bonds has
+ * n+1 entries). */
 qtt_status qtt_mps_from_cores(qtt_ctx* ctx, int n_sites, const int* bonds, const double* const* cores_host,
                               qtt_mps** out);
-/* PAPER.md:69 Eq. 4: contract the MPS and undo the bit interleave; dense_dev_out holds N*N doubles. */
+/* PAPER.md:69 Eq. 4: contract the MPS and undo the bit interleave; dense_dev_out holds N*N doubles (N*N*N for d = 8). */
 qtt_status qtt_to_dense(qtt_ctx* ctx, const qtt_mps* x, double* dense_dev_out);
 
-/* MPO from host cores W_k[D_{k-1}][4 out][4 in][D_k] (Eq. 7, App. A Table II); bonds has n+1
- * entries with both ends 1. */
+/* MPO from host cores W_k[D_{k-1}][d out][d in][D_k], d = qtt_ctx_phys_dim (Eq. 7, App. A Table II); bonds
+ * has n+1 entries with both ends 1. */
 qtt_status qtt_mpo_create(qtt_ctx* ctx, int n_sites, const int* bonds, const double* const* cores_host,
                           qtt_mpo** out);
 /* PAPER.md:391-424 App. A (Eq. A1-A3, Table II): the periodic central-difference MPO
- * (F[i+1] - F[i-1]) / (2 dx) along direction 1 (x) or 2 (y), bond 3, boundary vectors L = (1,1,1) on the
+ * (F[i+1] - F[i-1]) / (2 dx) along direction 1 (x) or 2 (y) (or 3 (z) when d = 8), bond 3, boundary vectors L = (1,1,1) on the
  * most-significant site and R = (0, 1, -1)/(2 dx) on the least-significant site folded into the end cores.
  * Index convention: w = output, w' = contracted with the MPS (reading 1).  n_sites >= 2. */
 qtt_status qtt_mpo_central_difference(qtt_ctx* ctx, int n_sites, int direction, double dx, qtt_mpo** out);
 /* Compact periodic 5-point Laplacian MPO, bond 5 (reading 3): channels identity, x+1, x-1, y+1, y-1;
- * L = (1,1,1,1,1), R = (-4,1,1,1,1)/dx^2.  n_sites >= 2. */
+ * L = (1,1,1,1,1), R = (-4,1,1,1,1)/dx^2.  With d = 8: the 7-point Laplacian, bond 7, channels identity, x+-1, y+-1, z+-1,
+ * R = (-6,1,1,1,1,1,1)/dx^2.  n_sites >= 2. */
 qtt_status qtt_mpo_laplacian(qtt_ctx* ctx, int n_sites, double dx, qtt_mpo** out);
 /* PAPER.md:98 ("MPOs for finite-difference stencils of any order"), construction of App. A generalised: the periodic
- * stencil (O F)[x] = sum_{k=-K..K} coeffs_host[k + K] * F[x + k] along direction 1 (x) or 2 (y), K = half_width in
+ * stencil (O F)[x] = sum_{k=-K..K} coeffs_host[k + K] * F[x + k] along direction 1 (x) or 2 (y) (or 3 (z) when d = 8), K = half_width in
  * 1..16, as an MPO of bond 2K + 1 (bond index = carry of the addition x + k + K).  n_sites >= 2. */
 qtt_status qtt_mpo_stencil(qtt_ctx* ctx, int n_sites, int direction, int half_width, const double* coeffs_host,
                            qtt_mpo** out);

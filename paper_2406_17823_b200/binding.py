@@ -120,9 +120,10 @@ def _cores_args(cores: Sequence[np.ndarray], ndim: int):
 
 # ------------------------------------------------------------------ the calls of include/qtt.h
 def qtt_mps_from_dense(ctx: Context, dense: torch.Tensor, chi_max: int, eps: float = 0.0) -> Mps:
-    """dense: N x N fp64 CUDA tensor F[x][y]."""
-    if dense.dtype != torch.float64 or not dense.is_cuda or dense.dim() != 2 or dense.shape[0] != dense.shape[1]:
-        raise ValueError("dense must be a square fp64 CUDA tensor")
+    """dense: N x N fp64 CUDA tensor F[x][y] (N x N x N, F[x][y][z], in a context of physical dimension 8)."""
+    ndim = 3 if qtt_ctx_phys_dim(ctx) == 8 else 2
+    if dense.dtype != torch.float64 or not dense.is_cuda or dense.dim() != ndim or len(set(dense.shape)) != 1:
+        raise ValueError(f"dense must be a fp64 CUDA tensor with {ndim} equal dimensions")
     dense = dense.contiguous()
     n = int(dense.shape[0]).bit_length() - 1
     if (1 << n) != dense.shape[0]:
@@ -134,8 +135,16 @@ def qtt_mps_from_dense(ctx: Context, dense: torch.Tensor, chi_max: int, eps: flo
     return Mps(ctx, h)
 
 
+def _check_phys(ctx: Context, arrs, axes) -> None:
+    d = qtt_ctx_phys_dim(ctx)
+    for a in arrs:
+        if any(a.shape[ax] != d for ax in axes):
+            raise ValueError(f"site tensors of this context have physical dimension {d}")
+
+
 def qtt_mps_from_cores(ctx: Context, cores: Sequence[np.ndarray]) -> Mps:
     arrs, n, bonds, ptrs = _cores_args(cores, 3)
+    _check_phys(ctx, arrs, (1,))
     h = C.c_void_p()
     ctx.check(ctx.lib.qtt_mps_from_cores(ctx.h, n, bonds, ptrs, C.byref(h)))
     return Mps(ctx, h)
@@ -144,7 +153,7 @@ def qtt_mps_from_cores(ctx: Context, cores: Sequence[np.ndarray]) -> Mps:
 def qtt_to_dense(ctx: Context, x: Mps) -> torch.Tensor:
     n = ctx.lib.qtt_mps_num_sites(x.h)
     N = 1 << n
-    out = torch.empty((N, N), dtype=torch.float64, device=ctx.device)
+    out = torch.empty((N,) * (3 if qtt_ctx_phys_dim(ctx) == 8 else 2), dtype=torch.float64, device=ctx.device)
     ctx.stream.wait_stream(torch.cuda.current_stream(ctx.device))
     ctx.check(ctx.lib.qtt_to_dense(ctx.h, x.h, C.c_void_p(out.data_ptr())))
     out.record_stream(ctx.stream)
@@ -154,6 +163,7 @@ def qtt_to_dense(ctx: Context, x: Mps) -> torch.Tensor:
 
 def qtt_mpo_create(ctx: Context, cores: Sequence[np.ndarray]) -> Mpo:
     arrs, n, bonds, ptrs = _cores_args(cores, 4)
+    _check_phys(ctx, arrs, (1, 2))
     h = C.c_void_p()
     ctx.check(ctx.lib.qtt_mpo_create(ctx.h, n, bonds, ptrs, C.byref(h)))
     return Mpo(ctx, h)
@@ -263,7 +273,7 @@ def _host_array(shape, pinned: bool) -> np.ndarray:
 
 def qtt_mps_get_core(ctx: Context, x: Mps, k: int, pinned: bool = False) -> np.ndarray:
     r = qtt_mps_bonds(x)
-    out = _host_array((r[k], 4, r[k + 1]), pinned)
+    out = _host_array((r[k], qtt_ctx_phys_dim(ctx), r[k + 1]), pinned)
     ctx.check(ctx.lib.qtt_mps_get_core(ctx.h, x.h, k, out.ctypes.data_as(C.POINTER(C.c_double))))
     return out
 
@@ -288,7 +298,7 @@ def qtt_mps_schmidt(ctx: Context, x: Mps) -> list:
     """Schmidt values per bond (index 1..n-1; entries 0 and n are None)."""
     r = qtt_mps_bonds(x)
     n = len(r) - 1
-    cap = max(max(r), 1) * 4
+    cap = max(max(r), 1) * qtt_ctx_phys_dim(ctx)
     buf = np.zeros((n + 1, cap), dtype=np.float64)
     counts = (C.c_int * (n + 1))()
     ctx.check(ctx.lib.qtt_mps_schmidt(ctx.h, x.h, buf.ctypes.data_as(C.POINTER(C.c_double)), cap, counts))
@@ -329,6 +339,15 @@ def qtt_mps_clone(ctx: Context, x: Mps) -> Mps:
 
 def qtt_ctx_set_chi_work(ctx: Context, chi_work: int) -> None:
     ctx.check(ctx.lib.qtt_ctx_set_chi_work(ctx.h, int(chi_work)))
+
+
+def qtt_ctx_set_phys_dim(ctx: Context, d: int) -> None:
+    """4: 2D quantics encoding (default); 8: 3D (include/qtt.h).  Only while no MPS / MPO handle of the context is alive."""
+    ctx.check(ctx.lib.qtt_ctx_set_phys_dim(ctx.h, int(d)))
+
+
+def qtt_ctx_phys_dim(ctx: Context) -> int:
+    return int(ctx.lib.qtt_ctx_phys_dim(ctx.h))
 
 
 def qtt_ctx_set_convection(ctx: Context, skew_symmetric: bool) -> None:

@@ -18,6 +18,7 @@ void mpo_release(MpoData* w) {
   if (!w) return;
   if (--w->refs > 0) return;
   if (w->storage && w->ctx) w->ctx->release(w->storage, w->ctx->user);
+  if (w->storage && w->ctx) --w->ctx->live;
   delete w;
 }
 
@@ -25,6 +26,7 @@ void body_release(Body* b) {
   if (!b) return;
   if (--b->refs > 0) return;
   if (b->storage && b->ctx) b->ctx->release(b->storage, b->ctx->user);
+  if (b->storage && b->ctx) --b->ctx->live;
   mpo_release(b->mpo);
   body_release(b->x);
   body_release(b->a);
@@ -38,9 +40,9 @@ Body* body_retain(Body* b) {
   return b;
 }
 
-size_t cores_doubles(const std::vector<int>& r) {
+size_t cores_doubles(const std::vector<int>& r, int d) {
   size_t s = 0;
-  for (size_t k = 0; k + 1 < r.size(); ++k) s += (size_t)r[k] * 4 * r[k + 1];
+  for (size_t k = 0; k + 1 < r.size(); ++k) s += (size_t)r[k] * d * r[k + 1];
   return s;
 }
 
@@ -51,17 +53,18 @@ Body* body_new_dense(qtt_ctx* ctx, const std::vector<int>& rcap) {
   b->kind = BODY_DENSE;
   b->n = (int)rcap.size() - 1;
   b->r = rcap;
-  b->storage_doubles = cores_doubles(rcap);
+  b->storage_doubles = cores_doubles(rcap, ctx->d);
   b->storage = static_cast<double*>(ctx->alloc(std::max<size_t>(b->storage_doubles, 1) * sizeof(double), ctx->user));
   if (!b->storage) {
     delete b;
     QTT_THROW(QTT_CAPACITY, "alloc callback returned NULL");
   }
+  ++ctx->live;
   b->core.resize(b->n);
   size_t off = 0;
   for (int k = 0; k < b->n; ++k) {
     b->core[k] = b->storage + off;
-    off += (size_t)rcap[k] * 4 * rcap[k + 1];
+    off += (size_t)rcap[k] * ctx->d * rcap[k + 1];
   }
   b->tight = true;
   return b;
@@ -91,7 +94,7 @@ View view_of_body(const Body* b) {
 // Dense view of any body; lazy kinds are materialised in the tmp stack (bounded by the limit).
 View materialize(qtt_ctx* ctx, const Body* b) {
   if (b->kind == BODY_DENSE) return view_of_body(b);
-  if (cores_doubles(b->r) * sizeof(double) > ctx->mat_limit)
+  if (cores_doubles(b->r, ctx->d) * sizeof(double) > ctx->mat_limit)
     QTT_THROW(QTT_CAPACITY, "lazy result exceeds the materialisation limit; round it instead");
   if (b->kind == BODY_APPLIED) {
     View x = materialize(ctx, b->x);
@@ -340,6 +343,16 @@ qtt_status qtt_ctx_set_chi_work(qtt_ctx* ctx, int chi_work) {
   ctx->chi_work = chi_work;
   return QTT_OK;
 }
+qtt_status qtt_ctx_set_phys_dim(qtt_ctx* ctx, int d) {
+  if (!ctx || (d != 4 && d != 8)) return QTT_INVALID_ARG;
+  if (d != ctx->d && ctx->live != 0) {
+    ctx->err = "qtt_ctx_set_phys_dim: free every MPS / MPO handle of the context before switching the encoding";
+    return QTT_INVALID_ARG;
+  }
+  ctx->d = d;
+  return QTT_OK;
+}
+int qtt_ctx_phys_dim(const qtt_ctx* ctx) { return ctx ? ctx->d : 0; }
 qtt_status qtt_ctx_set_materialize_limit(qtt_ctx* ctx, size_t bytes) {
   if (!ctx) return QTT_INVALID_ARG;
   ctx->mat_limit = bytes;
@@ -402,7 +415,7 @@ qtt_status qtt_mps_from_cores(qtt_ctx* ctx, int n, const int* bonds, const doubl
     if (v < 1) QTT_THROW(QTT_SHAPE_MISMATCH, "bond dimensions must be >= 1");
   Body* b = body_new_dense(ctx, r);
   for (int k = 0; k < n; ++k)
-    QTT_CU(cudaMemcpyAsync(b->core[k], cores_host[k], sizeof(double) * (size_t)r[k] * 4 * r[k + 1],
+    QTT_CU(cudaMemcpyAsync(b->core[k], cores_host[k], sizeof(double) * (size_t)r[k] * ctx->d * r[k + 1],
                            cudaMemcpyHostToDevice, ctx->stream));
   QTT_CU(cudaStreamSynchronize(ctx->stream));  // host arrays may go away
   *out = new qtt_mps{ctx, b};
@@ -419,16 +432,18 @@ qtt_status qtt_mpo_create(qtt_ctx* ctx, int n, const int* bonds, const double* c
   w->n = n;
   w->D.assign(bonds, bonds + n + 1);
   size_t tot = 0;
-  for (int k = 0; k < n; ++k) tot += (((size_t)w->D[k] * 16 * w->D[k + 1]) + 31) & ~(size_t)31;
+  const size_t dd = (size_t)ctx->d * ctx->d;
+  for (int k = 0; k < n; ++k) tot += (((size_t)w->D[k] * dd * w->D[k + 1]) + 31) & ~(size_t)31;
   w->storage = static_cast<double*>(ctx->alloc(tot * sizeof(double), ctx->user));
   if (!w->storage) {
     delete w;
     QTT_THROW(QTT_CAPACITY, "alloc callback returned NULL");
   }
+  ++ctx->live;
   size_t off = 0;
   w->core.resize(n);
   for (int k = 0; k < n; ++k) {
-    size_t sz = (size_t)w->D[k] * 16 * w->D[k + 1];
+    size_t sz = (size_t)w->D[k] * dd * w->D[k + 1];
     w->core[k] = w->storage + off;
     QTT_CU(cudaMemcpyAsync(w->storage + off, cores_host[k], sz * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     off += (sz + 31) & ~(size_t)31;
@@ -466,7 +481,7 @@ qtt_status qtt_mps_clone(qtt_ctx* ctx, const qtt_mps* x, qtt_mps** out) {
   View v = materialize(ctx, x->body);
   Body* b = body_new_dense(ctx, v.r);
   for (int k = 0; k < v.n; ++k)
-    QTT_CU(cudaMemcpyAsync(b->core[k], v.core[k], sizeof(double) * (size_t)v.r[k] * 4 * v.r[k + 1],
+    QTT_CU(cudaMemcpyAsync(b->core[k], v.core[k], sizeof(double) * (size_t)v.r[k] * ctx->d * v.r[k + 1],
                            cudaMemcpyDeviceToDevice, ctx->stream));
   *out = new qtt_mps{ctx, b};
   QTT_API_END(ctx)
@@ -478,7 +493,7 @@ qtt_status qtt_mps_get_core(qtt_ctx* ctx, const qtt_mps* x, int k, double* host_
   set_device(ctx);
   ArenaScope scope(ctx);
   View v = materialize(ctx, x->body);
-  QTT_CU(cudaMemcpyAsync(host_out, v.core[k], sizeof(double) * (size_t)v.r[k] * 4 * v.r[k + 1], cudaMemcpyDeviceToHost,
+  QTT_CU(cudaMemcpyAsync(host_out, v.core[k], sizeof(double) * (size_t)v.r[k] * ctx->d * v.r[k + 1], cudaMemcpyDeviceToHost,
                          ctx->stream));
   check_numeric(ctx);
   QTT_API_END(ctx)
@@ -496,7 +511,8 @@ qtt_status qtt_mps_core_ptr(qtt_ctx* ctx, const qtt_mps* x, int k, const double*
 
 qtt_status qtt_mps_from_dense(qtt_ctx* ctx, const double* dense_dev, int n_bits, int chi_max, double eps,
                               qtt_mps** out) {
-  if (!ctx || !dense_dev || !out || n_bits < 1 || n_bits > 13 || chi_max < 1 || eps < 0.0) return QTT_INVALID_ARG;
+  if (!ctx || !dense_dev || !out || n_bits < 1 || n_bits > (ctx->d == 8 ? 9 : 13) || chi_max < 1 || eps < 0.0)
+    return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
   ArenaScope scope(ctx);
@@ -504,11 +520,11 @@ qtt_status qtt_mps_from_dense(qtt_ctx* ctx, const double* dense_dev, int n_bits,
   std::vector<int> full(n + 1, 1);
   for (int k = 1; k < n; ++k) {
     int l = std::min(k, n - k);
-    full[k] = l >= 15 ? (1 << 30) : (1 << (2 * l));
+    full[k] = l >= (ctx->d == 8 ? 10 : 15) ? (1 << 30) : (1 << ((ctx->d == 8 ? 3 : 2) * l));
   }
   std::vector<int> caps(n + 1, 1);
   for (int k = n - 1; k >= 1; --k)
-    caps[k] = (int)std::min<long long>(std::min<long long>(chi_max, full[k]), 4ll * caps[k + 1]);
+    caps[k] = (int)std::min<long long>(std::min<long long>(chi_max, full[k]), (long long)ctx->d * caps[k + 1]);
   Body* b = body_new_dense(ctx, caps);
   try {
     OutMps o = out_of_body(b);
@@ -630,7 +646,7 @@ static qtt_status round_batch_impl(qtt_ctx* ctx, int batch, qtt_mps* const* xs, 
       std::vector<OutMps> out;
       for (int i : dense_idx) {
         in.push_back(materialize(ctx, xs[i]->body));
-        fresh[i] = body_new_dense(ctx, qtt_round_caps(in.back().r, chi_max));
+        fresh[i] = body_new_dense(ctx, qtt_round_caps(in.back().r, chi_max, ctx->d));
         out.push_back(out_of_body(fresh[i]));
       }
       qtt_round_dense_batch(ctx, in, chi_max, eps, out);
@@ -644,7 +660,7 @@ static qtt_status round_batch_impl(qtt_ctx* ctx, int batch, qtt_mps* const* xs, 
         A.push_back(materialize(ctx, xs[i]->body->a));
         B.push_back(materialize(ctx, xs[i]->body->b));
         std::vector<int> rw, ro;
-        qtt_zip_caps(A.back().r, B.back().r, chi_max, cw, rw, ro);
+        qtt_zip_caps(A.back().r, B.back().r, chi_max, cw, rw, ro, ctx->d);
         fresh[i] = body_new_dense(ctx, ro);
         out.push_back(out_of_body(fresh[i]));
       }
@@ -684,6 +700,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
     return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
+  if (ctx->d != 4) QTT_THROW(QTT_INVALID_ARG, "qtt_rk4_step is built for the 2D encoding (physical dimension 4)");
   const int n = u[0]->body->n;
   if (u[1]->body->n != n || Dx->data->n != n || Dy->data->n != n || Lap->data->n != n || n < 2)
     QTT_THROW(QTT_SHAPE_MISMATCH, "rk4_step operands differ in length (or fewer than two sites)");
@@ -739,8 +756,8 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
     rk4_out_bonds(plan->rin, Dx->data, Dy->data, Lap->data, chi_max, cw, ctx->skew, plan->rout);
     try {
       for (int i = 0; i < 2; ++i) {
-        plan->in_buf[i] = static_cast<double*>(ctx->alloc(cores_doubles(plan->rin[i]) * sizeof(double), ctx->user));
-        plan->out_buf[i] = static_cast<double*>(ctx->alloc(cores_doubles(plan->rout[i]) * sizeof(double), ctx->user));
+        plan->in_buf[i] = static_cast<double*>(ctx->alloc(cores_doubles(plan->rin[i], 4) * sizeof(double), ctx->user));
+        plan->out_buf[i] = static_cast<double*>(ctx->alloc(cores_doubles(plan->rout[i], 4) * sizeof(double), ctx->user));
         if (!plan->in_buf[i] || !plan->out_buf[i]) QTT_THROW(QTT_CAPACITY, "alloc callback returned NULL");
       }
       View pin[2] = {packed_view(plan->rin[0], plan->in_buf[0]), packed_view(plan->rin[1], plan->in_buf[1])};
@@ -770,7 +787,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
   for (int i = 0; i < 2; ++i) {
     size_t off = 0;
     if (u[i]->body->kind == BODY_DENSE && u[i]->body->tight) {
-      QTT_CU(cudaMemcpyAsync(plan->in_buf[i], u[i]->body->storage, cores_doubles(uv[i].r) * sizeof(double),
+      QTT_CU(cudaMemcpyAsync(plan->in_buf[i], u[i]->body->storage, cores_doubles(uv[i].r, 4) * sizeof(double),
                              cudaMemcpyDeviceToDevice, ctx->stream));
     } else {
       for (int k = 0; k < n; ++k) {
@@ -790,7 +807,7 @@ qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, co
       body_release(b);
       u[i]->body = b = nb;
     }
-    QTT_CU(cudaMemcpyAsync(b->storage, plan->out_buf[i], cores_doubles(plan->rout[i]) * sizeof(double),
+    QTT_CU(cudaMemcpyAsync(b->storage, plan->out_buf[i], cores_doubles(plan->rout[i], 4) * sizeof(double),
                            cudaMemcpyDeviceToDevice, ctx->stream));
   }
   QTT_API_END(ctx)
@@ -819,12 +836,12 @@ qtt_status qtt_mps_schmidt(qtt_ctx* ctx, const qtt_mps* x, double* sigma_host, i
   for (int k = 0; k <= n; ++k) counts[k] = 0;
   if (n < 2) return QTT_OK;
   const int big = 1 << 30;
-  std::vector<int> caps = qtt_round_caps(v.r, big);
+  std::vector<int> caps = qtt_round_caps(v.r, big, ctx->d);
   OutMps o;
   o.n = n;
   o.rcap = caps;
   o.core.resize(n);
-  for (int k = 0; k < n; ++k) o.core[k] = ctx->arena.keep((size_t)caps[k] * 4 * caps[k + 1]);
+  for (int k = 0; k < n; ++k) o.core[k] = ctx->arena.keep((size_t)caps[k] * ctx->d * caps[k + 1]);
   std::vector<OutMps> outs{o};
   SigmaCapture sc;
   qtt_round_dense_batch(ctx, {v}, big, 0.0, outs, &sc);
@@ -846,20 +863,21 @@ qtt_status qtt_mps_norm(qtt_ctx* ctx, const qtt_mps* x, double* out_host) {
   View v = materialize(ctx, x->body);
   const int n = v.n;
   if (n < 2) {
-    double h[4];
-    QTT_CU(cudaMemcpyAsync(h, v.core[0], sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    double h[8] = {0, 0, 0, 0, 0, 0, 0, 0}, s2 = 0.0;
+    QTT_CU(cudaMemcpyAsync(h, v.core[0], sizeof(double) * ctx->d, cudaMemcpyDeviceToHost, ctx->stream));
     QTT_CU(cudaStreamSynchronize(ctx->stream));
-    *out_host = std::sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2] + h[3] * h[3]);
+    for (int i = 0; i < ctx->d; ++i) s2 += h[i] * h[i];
+    *out_host = std::sqrt(s2);
     return QTT_OK;
   }
   // the Schmidt values of the last bond carry the whole norm
   const int big = 1 << 30;
-  std::vector<int> caps = qtt_round_caps(v.r, big);
+  std::vector<int> caps = qtt_round_caps(v.r, big, ctx->d);
   OutMps o;
   o.n = n;
   o.rcap = caps;
   o.core.resize(n);
-  for (int k = 0; k < n; ++k) o.core[k] = ctx->arena.keep((size_t)caps[k] * 4 * caps[k + 1]);
+  for (int k = 0; k < n; ++k) o.core[k] = ctx->arena.keep((size_t)caps[k] * ctx->d * caps[k + 1]);
   std::vector<OutMps> outs{o};
   SigmaCapture sc;
   qtt_round_dense_batch(ctx, {v}, big, 0.0, outs, &sc);
@@ -891,6 +909,7 @@ qtt_status qtt_tke_spectrum(qtt_ctx* ctx, const qtt_mps* u1, const qtt_mps* u2, 
   if (!ctx || !u1 || !u2 || !E_host || nbins < 1) return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
+  if (ctx->d != 4) QTT_THROW(QTT_INVALID_ARG, "qtt_tke_spectrum is built for the 2D encoding (physical dimension 4)");
   ArenaScope scope(ctx);
   const int n = u1->body->n;
   if (u2->body->n != n || (mean1 && mean1->body->n != n) || (mean2 && mean2->body->n != n))
@@ -935,7 +954,7 @@ qtt_status qtt_mps_chi_eps(qtt_ctx* ctx, const qtt_mps* x, double eps, int* chi_
   if (st != QTT_OK) return st;
   int cap = 1;
   for (int k = 0; k <= n; ++k) cap = std::max(cap, r[k]);
-  cap *= 4;
+  cap *= ctx->d;
   std::vector<double> sig((size_t)(n + 1) * cap, 0.0);
   st = qtt_mps_schmidt(ctx, x, sig.data(), cap, counts.data());
   if (st != QTT_OK) return st;
@@ -967,6 +986,7 @@ qtt_status qtt_variational_cost(qtt_ctx* ctx, const qtt_mps* const v[2], const q
     if (!v[i] || !a[i] || !B[i]) return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
+  if (ctx->d != 4) QTT_THROW(QTT_INVALID_ARG, "qtt_variational_cost is built for the 2D encoding (physical dimension 4)");
   ArenaScope scope(ctx);
   View vv[2], va[2], vb[2];
   for (int i = 0; i < 2; ++i) {
@@ -991,6 +1011,7 @@ qtt_status qtt_variational_stage(qtt_ctx* ctx, qtt_mps* const v[2], const qtt_mp
     if (!v[i] || !a[i] || !B[i]) return QTT_INVALID_ARG;
   QTT_API_BEGIN
   set_device(ctx);
+  if (ctx->d != 4) QTT_THROW(QTT_INVALID_ARG, "qtt_variational_stage is built for the 2D encoding (physical dimension 4)");
   ArenaScope scope(ctx);
   View vv[2], va[2], vb[2];
   for (int i = 0; i < 2; ++i) {

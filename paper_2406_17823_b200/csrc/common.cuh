@@ -151,7 +151,7 @@ int qtt_select_max_rows();  // largest p the sort handles (shared-memory keys)
 // ----------------------------------------------------------------------------------------------
 // Data movement (bandwidth-bound).
 // MPO x MPS site expand (paper Sec. II.B): out[(al,a), w, (be,b)] = sum_w' W[al,w,w',be] * A[a,w',b].
-struct ExpandProb { const double* W; const double* A; double* out; int Dl, Dr, a, b; };
+struct ExpandProb { const double* W; const double* A; double* out; int Dl, Dr, a, b; int d; };  // d: physical dimension (4 or 8)
 #define QTT_MOVE_MAX_BATCH 16
 struct ExpandGroup { int nprob; ExpandProb p[QTT_MOVE_MAX_BATCH]; };
 cudaError_t qtt_launch_expand(const ExpandProb* probs, int n, cudaStream_t stream);
@@ -160,17 +160,19 @@ cudaError_t qtt_launch_expand(const ExpandProb* probs, int n, cudaStream_t strea
 struct ConcatProb {
   const double* src[5]; double alpha[5]; int rl[5], rr[5]; int nterm;
   double* out; int mode;  // 0 first (row concat of columns), 1 middle (block diagonal), 2 last (stack rows)
+  int d;                  // physical dimension (4 or 8)
 };
 struct ConcatGroup { int nprob; ConcatProb p[QTT_MOVE_MAX_BATCH]; };
 cudaError_t qtt_launch_concat(const ConcatProb* probs, int n, cudaStream_t stream);
 
 // Hadamard site tensor (paper Eq. 8): out[(a,b), w, (a2,b2)] = A[a,w,a2] * B[b,w,b2].
-struct KronProb { const double* A; const double* B; double* out; int a, a2, b, b2; };
+struct KronProb { const double* A; const double* B; double* out; int a, a2, b, b2; int d; };
 struct KronGroup { int nprob; KronProb p[QTT_MOVE_MAX_BATCH]; };
 cudaError_t qtt_launch_kron(const KronProb* probs, int n, cudaStream_t stream);
 
-// Quantics bit interleave (paper Eq. 3): dense F[x][y] (N x N) <-> tensor U[w_1..w_n], w_k = 2 x_k + y_k.
-cudaError_t qtt_launch_interleave(const double* F, double* U, int nbits, int inverse, cudaStream_t stream);
+// Quantics bit interleave (paper Eq. 3): dense F[x][y] (N x N) <-> tensor U[w_1..w_n], w_k = 2 x_k + y_k (ndim = 2), or
+// dense F[x][y][z] (N^3) <-> U with w_k = 4 x_k + 2 y_k + z_k (ndim = 3; reading 26).
+cudaError_t qtt_launch_interleave(const double* F, double* U, int nbits, int ndim, int inverse, cudaStream_t stream);
 // Generic 2-D transpose / strided copy: dst[j * ldd + i] = src[i * lds + j], i < rows, j < cols.
 cudaError_t qtt_launch_transpose(const double* src, int rows, int cols, int lds, double* dst, int ldd,
                                  cudaStream_t stream);

@@ -31,7 +31,7 @@ struct Arena {
   double* tmp(size_t doubles);
 };
 
-// An MPS with explicit dense cores in device memory: core[k] is r[k] x 4 x r[k+1], row-major.
+// An MPS with explicit dense cores in device memory: core[k] is r[k] x d x r[k+1], row-major, d = ctx->d (4 or 8).
 struct View {
   int n = 0;
   std::vector<int> r;
@@ -89,6 +89,8 @@ struct qtt_ctx {
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   Arena side_arena;
   std::string err;
+  int d = 4;  // physical dimension: 4 = 2D grid (Eq. 3), 8 = 3D grid (reading 26); fixed while handles live
+  int live = 0;  // MPS / MPO handles alive (qtt_ctx_set_phys_dim refuses to switch under them)
   int chi_work = 0;
   size_t mat_limit = (size_t)2 << 30;
   int graphs = 1;
@@ -113,10 +115,11 @@ struct OutMps {
 };
 
 // static (eps == 0) bonds of round(dense MPS with bonds r, chi)
-std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi);
+// (d = physical dimension; the default serves the callers that are built for the 2D encoding only)
+std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi, int d = 4);
 // working bonds of the zip-up and static bonds of its result
 void qtt_zip_caps(const std::vector<int>& ra, const std::vector<int>& rb, int chi, int chi_work,
-                  std::vector<int>& rwork, std::vector<int>& rout);
+                  std::vector<int>& rwork, std::vector<int>& rout, int d = 4);
 
 struct SigmaCapture {
   // per item, per bond k (1..n-1): device pointer to the singular values (count[k] of them)

@@ -14,29 +14,33 @@ inline int grid_for(i64 n) {
 }
 
 // out[(al,a), w, (be,b)] = sum_w' W[al,w,w',be] * A[a,w',b]      (MPO bond index major)
+// (DP = physical dimension, a compile-time constant so that the index arithmetic stays shifts and the w' loop unrolls)
+template <int DP>
 __global__ void qtt_expand_kernel(const __grid_constant__ ExpandGroup g) {
   const ExpandProb& P = g.p[blockIdx.y];
   const int Dl = P.Dl, Dr = P.Dr, a = P.a, b = P.b;
-  const i64 n = (i64)Dl * a * 4 * Dr * b;
+  constexpr int d = DP;
+  const i64 n = (i64)Dl * a * d * Dr * b;
   const i64 rowlen = (i64)Dr * b;
   for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
     i64 t = idx;
     int bb = (int)(t % b); t /= b;
     int be = (int)(t % Dr); t /= Dr;
-    int w = (int)(t % 4); t /= 4;
+    int w = (int)(t % d); t /= d;
     int aa = (int)(t % a);
     int al = (int)(t / a);
     double s = 0.0;
 #pragma unroll
-    for (int wp = 0; wp < 4; ++wp) {
-      double wv = P.W[((al * 4 + w) * 4 + wp) * Dr + be];
-      if (wv != 0.0) s += wv * P.A[((i64)aa * 4 + wp) * b + bb];
+    for (int wp = 0; wp < d; ++wp) {
+      double wv = P.W[((al * d + w) * d + wp) * Dr + be];
+      if (wv != 0.0) s += wv * P.A[((i64)aa * d + wp) * b + bb];
     }
     P.out[idx] = s;
     (void)rowlen;
   }
 }
 
+template <int DP>
 __global__ void qtt_concat_kernel(const __grid_constant__ ConcatGroup g) {
   const ConcatProb& P = g.p[blockIdx.y];
   int RL = 0, RR = 0;
@@ -52,12 +56,13 @@ __global__ void qtt_concat_kernel(const __grid_constant__ ConcatGroup g) {
       RR += P.rr[t];
     }
   }
-  const i64 n = (i64)RL * 4 * RR;
+  constexpr int d = DP;
+  const i64 n = (i64)RL * d * RR;
   for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
     int c = (int)(idx % RR);
     i64 t2 = idx / RR;
-    int w = (int)(t2 % 4);
-    int r = (int)(t2 / 4);
+    int w = (int)(t2 % d);
+    int r = (int)(t2 / d);
     // locate the term of the row and of the column
     int tr = 0, tc = 0, r_in = r, c_in = c;
     if (P.mode != 0) {
@@ -68,28 +73,30 @@ __global__ void qtt_concat_kernel(const __grid_constant__ ConcatGroup g) {
     }
     double v = 0.0;
     if (P.mode == 0) {
-      v = P.alpha[tc] * P.src[tc][((i64)r * 4 + w) * P.rr[tc] + c_in];
+      v = P.alpha[tc] * P.src[tc][((i64)r * d + w) * P.rr[tc] + c_in];
     } else if (P.mode == 2) {
-      v = P.src[tr][((i64)r_in * 4 + w) * P.rr[tr] + c];
+      v = P.src[tr][((i64)r_in * d + w) * P.rr[tr] + c];
     } else if (tr == tc) {
-      v = P.src[tr][((i64)r_in * 4 + w) * P.rr[tr] + c_in];
+      v = P.src[tr][((i64)r_in * d + w) * P.rr[tr] + c_in];
     }
     P.out[idx] = v;
   }
 }
 
 // out[(a,b), w, (a2,b2)] = A[a,w,a2] * B[b,w,b2]                  (Eq. 8)
+template <int DP>
 __global__ void qtt_kron_kernel(const __grid_constant__ KronGroup g) {
   const KronProb& P = g.p[blockIdx.y];
-  const i64 n = (i64)P.a * P.b * 4 * P.a2 * P.b2;
+  constexpr int d = DP;
+  const i64 n = (i64)P.a * P.b * d * P.a2 * P.b2;
   for (i64 idx = (i64)blockIdx.x * NT + threadIdx.x; idx < n; idx += (i64)gridDim.x * NT) {
     i64 t = idx;
     int bb2 = (int)(t % P.b2); t /= P.b2;
     int aa2 = (int)(t % P.a2); t /= P.a2;
-    int w = (int)(t % 4); t /= 4;
+    int w = (int)(t % d); t /= d;
     int bb = (int)(t % P.b);
     int aa = (int)(t / P.b);
-    P.out[idx] = P.A[((i64)aa * 4 + w) * P.a2 + aa2] * P.B[((i64)bb * 4 + w) * P.b2 + bb2];
+    P.out[idx] = P.A[((i64)aa * d + w) * P.a2 + aa2] * P.B[((i64)bb * d + w) * P.b2 + bb2];
   }
 }
 
@@ -116,6 +123,25 @@ __global__ void qtt_interleave_kernel(const double* __restrict__ src, double* __
       dst[d] = src[t];  // tensor -> dense
     else
       dst[t] = src[d];  // dense -> tensor
+  }
+}
+// Three coordinates (reading 26): t = (w_1 ... w_n)_8, w_k = 4 x_k + 2 y_k + z_k; dense index = (x * N + y) * N + z.
+__global__ void qtt_interleave3_kernel(const double* __restrict__ src, double* __restrict__ dst, int nbits,
+                                       int inverse) {
+  const i64 n = 1ll << (3 * nbits);
+  for (i64 t = (i64)blockIdx.x * NT + threadIdx.x; t < n; t += (i64)gridDim.x * NT) {
+    i64 x = 0, y = 0, z = 0;
+    for (int k = 0; k < nbits; ++k) {
+      const i64 w = (t >> (3 * k)) & 7;  // site n - k: bit k of every coordinate
+      x |= ((w >> 2) & 1) << k;
+      y |= ((w >> 1) & 1) << k;
+      z |= (w & 1) << k;
+    }
+    const i64 d = (((x << nbits) | y) << nbits) | z;
+    if (inverse)
+      dst[d] = src[t];
+    else
+      dst[t] = src[d];
   }
 }
 
@@ -156,12 +182,16 @@ cudaError_t qtt_launch_expand(const ExpandProb* probs, int n, cudaStream_t strea
     i64 mx = 1;
     for (int i = 0; i < g.nprob; ++i) {
       g.p[i] = probs[b0 + i];
-      i64 sz = (i64)g.p[i].Dl * g.p[i].a * 4 * g.p[i].Dr * g.p[i].b;
+      if ((g.p[i].d != 4 && g.p[i].d != 8) || g.p[i].d != probs[b0].d) return cudaErrorInvalidValue;
+      i64 sz = (i64)g.p[i].Dl * g.p[i].a * g.p[i].d * g.p[i].Dr * g.p[i].b;
       mx = sz > mx ? sz : mx;
     }
     {
       QttProf prof(QK_MOVE, stream, 16.0 * (double)mx * g.nprob);
-      qtt_expand_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      if (g.p[0].d == 8)
+        qtt_expand_kernel<8><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      else
+        qtt_expand_kernel<4><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
     }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
@@ -175,17 +205,21 @@ cudaError_t qtt_launch_concat(const ConcatProb* probs, int n, cudaStream_t strea
     i64 mx = 1;
     for (int i = 0; i < g.nprob; ++i) {
       g.p[i] = probs[b0 + i];
+      if ((g.p[i].d != 4 && g.p[i].d != 8) || g.p[i].d != probs[b0].d) return cudaErrorInvalidValue;
       i64 RL = 0, RR = 0;
       for (int t = 0; t < g.p[i].nterm; ++t) {
         RL += g.p[i].rl[t];
         RR += g.p[i].rr[t];
       }
-      i64 sz = RL * 4 * RR;
+      i64 sz = RL * g.p[i].d * RR;
       mx = sz > mx ? sz : mx;
     }
     {
       QttProf prof(QK_MOVE, stream, 16.0 * (double)mx * g.nprob);
-      qtt_concat_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      if (g.p[0].d == 8)
+        qtt_concat_kernel<8><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      else
+        qtt_concat_kernel<4><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
     }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
@@ -199,22 +233,32 @@ cudaError_t qtt_launch_kron(const KronProb* probs, int n, cudaStream_t stream) {
     i64 mx = 1;
     for (int i = 0; i < g.nprob; ++i) {
       g.p[i] = probs[b0 + i];
-      i64 sz = (i64)g.p[i].a * g.p[i].b * 4 * g.p[i].a2 * g.p[i].b2;
+      if ((g.p[i].d != 4 && g.p[i].d != 8) || g.p[i].d != probs[b0].d) return cudaErrorInvalidValue;
+      i64 sz = (i64)g.p[i].a * g.p[i].b * g.p[i].d * g.p[i].a2 * g.p[i].b2;
       mx = sz > mx ? sz : mx;
     }
     {
       QttProf prof(QK_MOVE, stream, 8.0 * (double)mx * g.nprob);
-      qtt_kron_kernel<<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      if (g.p[0].d == 8)
+        qtt_kron_kernel<8><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
+      else
+        qtt_kron_kernel<4><<<dim3(grid_for(mx), g.nprob), NT, 0, stream>>>(g);
     }
     QTT_CHECK_CUDA(cudaGetLastError());
   }
   return cudaSuccess;
 }
 
-cudaError_t qtt_launch_interleave(const double* src, double* dst, int nbits, int inverse, cudaStream_t stream) {
+cudaError_t qtt_launch_interleave(const double* src, double* dst, int nbits, int ndim, int inverse,
+                                  cudaStream_t stream) {
+  if ((ndim != 2 && ndim != 3) || nbits < 1 || ndim * nbits > 40) return cudaErrorInvalidValue;
+  const i64 n = 1ll << (ndim * nbits);
   {
-    QttProf prof(QK_MOVE, stream, 16.0 * (double)(1ll << (2 * nbits)));
-    qtt_interleave_kernel<<<grid_for(1ll << (2 * nbits)), NT, 0, stream>>>(src, dst, nbits, inverse);
+    QttProf prof(QK_MOVE, stream, 16.0 * (double)n);
+    if (ndim == 3)
+      qtt_interleave3_kernel<<<grid_for(n), NT, 0, stream>>>(src, dst, nbits, inverse);
+    else
+      qtt_interleave_kernel<<<grid_for(n), NT, 0, stream>>>(src, dst, nbits, inverse);
   }
   return cudaGetLastError();
 }

@@ -27,28 +27,28 @@ double* Arena::tmp(size_t doubles) {
 }
 
 // ------------------------------------------------------------------------------------------ shapes
-std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi) {
+std::vector<int> qtt_round_caps(const std::vector<int>& r, int chi, int d) {
   const int n = (int)r.size() - 1;
   std::vector<int> p(n + 1), out(n + 1);
   p[0] = 1;
-  for (int k = 1; k <= n; ++k) p[k] = std::min(4 * p[k - 1], r[k]);
+  for (int k = 1; k <= n; ++k) p[k] = (int)std::min<long long>((long long)d * p[k - 1], r[k]);
   out[n] = 1;
-  for (int k = n - 1; k >= 1; --k) out[k] = std::max(1, std::min(chi, std::min(p[k], 4 * out[k + 1])));
+  for (int k = n - 1; k >= 1; --k) out[k] = std::max(1, (int)std::min<long long>(std::min(chi, p[k]), (long long)d * out[k + 1]));
   out[0] = 1;
   return out;
 }
 
 void qtt_zip_caps(const std::vector<int>& ra, const std::vector<int>& rb, int chi, int chi_work,
-                  std::vector<int>& rwork, std::vector<int>& rout) {
+                  std::vector<int>& rwork, std::vector<int>& rout, int d) {
   const int n = (int)ra.size() - 1;
   rwork.assign(n + 1, 1);
   for (int k = 1; k < n; ++k) {
     long long kk = (long long)ra[k] * rb[k];
-    long long m = 4ll * rwork[k - 1];
+    long long m = (long long)d * rwork[k - 1];
     rwork[k] = (int)std::min<long long>(std::min(m, kk), chi_work);
   }
   rout.assign(n + 1, 1);
-  for (int k = n - 1; k >= 1; --k) rout[k] = std::max(1, std::min(chi, std::min(rwork[k], 4 * rout[k + 1])));
+  for (int k = n - 1; k >= 1; --k) rout[k] = std::max(1, (int)std::min<long long>(std::min(chi, rwork[k]), (long long)d * rout[k + 1]));
 }
 
 // ------------------------------------------------------------------------------------------ helpers
@@ -245,6 +245,7 @@ struct SweepItem {
 // R->L truncated-SVD sweep (oracle O6 step ii) for a batch.
 void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, std::vector<OutMps>& out,
               SigmaCapture* cap) {
+  const int d = ctx->d;
   const int nb = (int)items.size();
   const int n = items[0].n;
   std::vector<const double*> C(nb, ctx->ones);
@@ -273,7 +274,7 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
     // B = core_k * C   (r_k x 4 rc)
     for (int i = 0; i < nb; ++i) {
       const LeftCore& c = items[i].core[k];
-      const int q = 4 * rc[i];
+      const int q = d * rc[i];
       if (c.form == 2) {
         B[i] = C[i];
       } else if (c.rr == 1 && rc[i] == 1 && C[i] == ctx->ones) {
@@ -281,9 +282,9 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
       } else {
         double* Bb = ctx->arena.tmp((size_t)c.rl * q);
         if (c.form == 0)
-          g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], Bb, rc[i], 4 * c.rl, rc[i], c.rr));
+          g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], Bb, rc[i], d * c.rl, rc[i], c.rr));
         else
-          g.push_back(gemm_tn(c.ptr, 4 * c.rl, C[i], rc[i], Bb, rc[i], 4 * c.rl, rc[i], c.rr));
+          g.push_back(gemm_tn(c.ptr, d * c.rl, C[i], rc[i], Bb, rc[i], d * c.rl, rc[i], c.rr));
         B[i] = Bb;
       }
     }
@@ -291,7 +292,7 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
     // M = R_{k} * B  (pk x 4 rc), or a copy of B when the left block is an isometry
     for (int i = 0; i < nb; ++i) {
       const LeftCore& c = items[i].core[k];
-      const int q = 4 * rc[i];
+      const int q = d * rc[i];
       const int p = items[i].Rf[k] ? items[i].pk[k] : c.rl;
       double* Mb = ctx->arena.tmp((size_t)p * q);
       if (items[i].Rf[k])
@@ -328,7 +329,7 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
     for (int i = 0; i < nb; ++i) {
       const LeftCore& c = items[i].core[k];
       const int p = items[i].Rf[k] ? items[i].pk[k] : c.rl;
-      rank_host[i] = std::max(1, std::min(std::min(chi, out[i].rcap[k]), std::min(p, 4 * rc[i])));
+      rank_host[i] = std::max(1, std::min(std::min(chi, out[i].rcap[k]), std::min(p, d * rc[i])));
     }
     if (eps > 0.0) {
       for (int i = 0; i < nb; ++i)
@@ -338,7 +339,7 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
     // C_{k} <- B * core'^T   (r_k x r')
     for (int i = 0; i < nb; ++i) {
       const LeftCore& c = items[i].core[k];
-      const int q = 4 * rc[i];
+      const int q = d * rc[i];
       const int rn = rank_host[i];
       double* Cn = Cbuf[k & 1][i];
       g2.push_back(gemm_nt(B[i], q, out[i].core[k], q, Cn, rn, c.rl, rn, q));
@@ -353,11 +354,11 @@ void sweep_rl(qtt_ctx* ctx, std::vector<SweepItem>& items, int chi, double eps, 
   for (int i = 0; i < nb; ++i) {
     const LeftCore& c = items[i].core[0];
     if (c.form == 2)
-      QTT_CU(qtt_launch_copy2d(C[i], 4, rc[i], rc[i], out[i].core[0], rc[i], ctx->stream));
+      QTT_CU(qtt_launch_copy2d(C[i], d, rc[i], rc[i], out[i].core[0], rc[i], ctx->stream));
     else if (c.form == 0)
-      g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], out[i].core[0], rc[i], 4 * c.rl, rc[i], c.rr));
+      g.push_back(gemm_nn(c.ptr, c.rr, C[i], rc[i], out[i].core[0], rc[i], d * c.rl, rc[i], c.rr));
     else
-      g.push_back(gemm_tn(c.ptr, 4 * c.rl, C[i], rc[i], out[i].core[0], rc[i], 4 * c.rl, rc[i], c.rr));
+      g.push_back(gemm_tn(c.ptr, d * c.rl, C[i], rc[i], out[i].core[0], rc[i], d * c.rl, rc[i], c.rr));
   }
   run_gemms(ctx, g);
 }
@@ -384,6 +385,7 @@ void qtt_row_space_basis(qtt_ctx* ctx, double* X, int p, int q, double* out) {
 // ------------------------------------------------------------------------------------------ O6
 void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, double eps, std::vector<OutMps>& out,
                            SigmaCapture* cap) {
+  const int d = ctx->d;
   const int nb = (int)in.size();
   if (nb == 0) return;
   const int n = in[0].n;
@@ -395,7 +397,7 @@ void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, d
   }
   if (n == 1) {
     for (int i = 0; i < nb; ++i) {
-      QTT_CU(qtt_launch_copy2d(in[i].core[0], 1, 4, 4, out[i].core[0], 4, ctx->stream));
+      QTT_CU(qtt_launch_copy2d(in[i].core[0], 1, d, d, out[i].core[0], d, ctx->stream));
       out[i].r.assign(2, 1);
     }
     return;
@@ -419,7 +421,7 @@ void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, d
     for (int i = 0; i < nb; ++i) {
       SweepItem& it = items[i];
       const int r1 = in[i].r[k + 1];
-      const int rows = 4 * it.pk[k], cols = r1;
+      const int rows = d * it.pk[k], cols = r1;
       if (rows <= cols) {
         if (k > 0) Rnew[i] = ctx->arena.tmp((size_t)rows * cols);
       } else {
@@ -431,12 +433,12 @@ void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, d
       SweepItem& it = items[i];
       const int rk = in[i].r[k], r1 = in[i].r[k + 1];
       const int pk = it.pk[k];
-      const int rows = 4 * pk, cols = r1;
+      const int rows = d * pk, cols = r1;
       if (rows <= cols) {
         if (k == 0) {
           it.Rf[1] = in[i].core[0];
         } else {
-          g.push_back(gemm_nn(it.Rf[k], rk, in[i].core[k], 4 * (i64)r1, Rnew[i], 4 * (i64)r1, pk, 4 * r1, rk));
+          g.push_back(gemm_nn(it.Rf[k], rk, in[i].core[k], d * (i64)r1, Rnew[i], d * (i64)r1, pk, d * r1, rk));
           it.Rf[k + 1] = Rnew[i];
         }
         it.pk[k + 1] = rows;
@@ -444,10 +446,10 @@ void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, d
         // Y = X^T (cols x rows), written transposed by the GEMM:  Y[b][(i,w)] = sum_a core[a,w,b] R[i,a]
         double* Y = ctx->arena.tmp((size_t)cols * rows);
         GemmProb p = gemm_base(in[i].core[k], it.Rf[k], Y, r1, pk, rk);
-        p.nbatch = 4;
-        p.a_lo = 1; p.a_k = 4 * (i64)r1; p.a_bs = r1;
+        p.nbatch = d;
+        p.a_lo = 1; p.a_k = d * (i64)r1; p.a_bs = r1;
         p.b_k = 1; p.b_n = rk; p.b_bs = 0;
-        p.c_lo = 4 * (i64)pk; p.c_n = 4; p.c_bs = 1;
+        p.c_lo = d * (i64)pk; p.c_n = d; p.c_bs = 1;
         g.push_back(p);
         lq.push_back(LqJob{Y, cols, rows, rows, Rnew[i]});
         it.Rf[k + 1] = Rnew[i];
@@ -464,6 +466,7 @@ void qtt_round_dense_batch(qtt_ctx* ctx, const std::vector<View>& in, int chi, d
 // ------------------------------------------------------------------------------------------ O7
 void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std::vector<View>& B, int chi, double eps,
                              int chi_work, std::vector<OutMps>& out) {
+  const int d = ctx->d;
   const int nb = (int)A.size();
   if (nb == 0) return;
   const int n = A[0].n;
@@ -482,7 +485,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
     items[i].pk.assign(n + 1, 1);
     // carry R_l (rwork[l] x a_l b_l) ping-pongs between two buffers of the largest size
     std::vector<int> rw, ro;
-    qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro);
+    qtt_zip_caps(A[i].r, B[i].r, chi, chi_work, rw, ro, d);
     size_t mx = 1;
     for (int l = 1; l < n; ++l) mx = std::max(mx, (size_t)rw[l] * A[i].r[l] * B[i].r[l]);
     Rbuf[0][i] = ctx->arena.tmp(mx);
@@ -494,6 +497,8 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
   //      S_l[(a,b),t] = sum_{w,u} G_l[w][u,t] sum_{a',b'} A_l[a,w,a'] B_l[b,w,b'] S_{l+1}[(a',b'),u],   S_n = 1
   std::vector<std::vector<char>> sk(nb, std::vector<char>(n, 0));
   std::vector<std::vector<double*>> S(nb, std::vector<double*>(n + 1, nullptr));
+  if (ctx->sketch && d != 4)
+    QTT_THROW(QTT_INVALID_ARG, "the sketched product compression is built for physical dimension 4 only");
   if (ctx->sketch) {
     const int P = chi_work;
     int lmin_all = n;
@@ -563,25 +568,25 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
     std::vector<double*> X(nb);
     for (int i = 0; i < nb; ++i) {
       const int a = A[i].r[l], a2 = A[i].r[l + 1], b = B[i].r[l];
-      X[i] = ctx->arena.tmp((size_t)r[i] * 4 * a2 * b);
-      GemmProb p = gemm_base(A[i].core[l], R[i], X[i], 4 * a2, b, a);
+      X[i] = ctx->arena.tmp((size_t)r[i] * d * a2 * b);
+      GemmProb p = gemm_base(A[i].core[l], R[i], X[i], d * a2, b, a);
       p.nbatch = r[i];
-      p.a_lo = 1; p.a_k = 4 * (i64)a2; p.a_bs = 0;
+      p.a_lo = 1; p.a_k = d * (i64)a2; p.a_bs = 0;
       p.b_k = b; p.b_n = 1; p.b_bs = (i64)a * b;
-      p.c_lo = b; p.c_n = 1; p.c_bs = 4 * (i64)a2 * b;
+      p.c_lo = b; p.c_n = 1; p.c_bs = d * (i64)a2 * b;
       g.push_back(p);
     }
     run_gemms(ctx, g);
     // T[(i,w),(a',b')] = sum_b X[i,w,a',b] B[b,w,b']   (second half)
     for (int i = 0; i < nb; ++i) {
       const int a2 = A[i].r[l + 1], b = B[i].r[l], b2 = B[i].r[l + 1];
-      const size_t tsz = (size_t)4 * r[i] * a2 * b2;
+      const size_t tsz = (size_t)d * r[i] * a2 * b2;
       T[i] = (l == n - 1) ? ctx->arena.keep(tsz) : ctx->arena.tmp(tsz);
       GemmProb p = gemm_base(X[i], B[i].core[l], T[i], r[i] * a2, b2, b);
-      p.nbatch = 4;
-      p.a_div = a2; p.a_hi = 4 * (i64)a2 * b; p.a_lo = b; p.a_k = 1; p.a_bs = (i64)a2 * b;
-      p.b_k = 4 * (i64)b2; p.b_n = 1; p.b_bs = b2;
-      p.c_div = a2; p.c_hi = 4 * (i64)a2 * b2; p.c_lo = b2; p.c_n = 1; p.c_bs = (i64)a2 * b2;
+      p.nbatch = d;
+      p.a_div = a2; p.a_hi = d * (i64)a2 * b; p.a_lo = b; p.a_k = 1; p.a_bs = (i64)a2 * b;
+      p.b_k = d * (i64)b2; p.b_n = 1; p.b_bs = b2;
+      p.c_div = a2; p.c_hi = d * (i64)a2 * b2; p.c_lo = b2; p.c_n = 1; p.c_bs = (i64)a2 * b2;
       g.push_back(p);
     }
     run_gemms(ctx, g);
@@ -596,7 +601,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
     std::vector<int> keep(nb, 0);
     std::vector<double*> Qt(nb, nullptr);
     for (int i = 0; i < nb; ++i) {
-      const int m = 4 * r[i];
+      const int m = d * r[i];
       const i64 kk = (i64)A[i].r[l + 1] * B[i].r[l + 1];
       if (m <= std::min<i64>(kk, chi_work)) {
         items[i].core[l] = LeftCore{nullptr, r[i], m, 2};
@@ -647,7 +652,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
     run_svd(ctx, svd);
     // R' = Q^T T  (keep x kk), into the other carry buffer
     for (int i = 0; i < nb; ++i) {
-      const int m = 4 * r[i];
+      const int m = d * r[i];
       const i64 kk = (i64)A[i].r[l + 1] * B[i].r[l + 1];
       double* Rn = Rbuf[l & 1][i];
       if (keep[i] == 0) {
@@ -665,7 +670,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
   }
   if (n == 1) {
     for (int i = 0; i < nb; ++i) {
-      QTT_CU(qtt_launch_copy2d(items[i].core[0].ptr, 1, 4, 4, out[i].core[0], 4, ctx->stream));
+      QTT_CU(qtt_launch_copy2d(items[i].core[0].ptr, 1, d, d, out[i].core[0], d, ctx->stream));
       out[i].r.assign(2, 1);
     }
     return;
@@ -676,6 +681,7 @@ void qtt_round_product_batch(qtt_ctx* ctx, const std::vector<View>& A, const std
 // ------------------------------------------------------------------------------------------ lazy kinds
 void qtt_expand_apply_batch(qtt_ctx* ctx, const std::vector<const MpoData*>& W, const std::vector<View>& x,
                             std::vector<View>& out) {
+  const int d = ctx->d;
   const int nb = (int)x.size();
   out.assign(nb, View());
   if (nb == 0) return;
@@ -690,9 +696,9 @@ void qtt_expand_apply_batch(qtt_ctx* ctx, const std::vector<const MpoData*>& W, 
   for (int k = 0; k < n; ++k) {
     std::vector<ExpandProb> e;
     for (int i = 0; i < nb; ++i) {
-      double* o = ctx->arena.tmp((size_t)out[i].r[k] * 4 * out[i].r[k + 1]);
+      double* o = ctx->arena.tmp((size_t)out[i].r[k] * d * out[i].r[k + 1]);
       out[i].core[k] = o;
-      e.push_back(ExpandProb{W[i]->core[k], x[i].core[k], o, W[i]->D[k], W[i]->D[k + 1], x[i].r[k], x[i].r[k + 1]});
+      e.push_back(ExpandProb{W[i]->core[k], x[i].core[k], o, W[i]->D[k], W[i]->D[k + 1], x[i].r[k], x[i].r[k + 1], d});
     }
     QTT_CU(qtt_launch_expand(e.data(), (int)e.size(), ctx->stream));
   }
@@ -706,6 +712,7 @@ View qtt_expand_apply(qtt_ctx* ctx, const MpoData* W, const View& x) {
 
 void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double, View>>>& terms,
                       std::vector<View>& out) {
+  const int d = ctx->d;
   const int nb = (int)terms.size();
   out.assign(nb, View());
   if (nb == 0) return;
@@ -727,6 +734,7 @@ void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<doub
       ConcatProb p;
       std::memset(&p, 0, sizeof(p));
       p.nterm = (int)terms[i].size();
+      p.d = d;
       for (int t = 0; t < p.nterm; ++t) {
         p.src[t] = terms[i][t].second.core[k];
         p.alpha[t] = terms[i][t].first;
@@ -734,7 +742,7 @@ void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<doub
         p.rr[t] = terms[i][t].second.r[k + 1];
       }
       p.mode = (n == 1) ? 3 : (k == 0 ? 0 : (k == n - 1 ? 2 : 1));
-      double* o = ctx->arena.tmp((size_t)out[i].r[k] * 4 * out[i].r[k + 1]);
+      double* o = ctx->arena.tmp((size_t)out[i].r[k] * d * out[i].r[k + 1]);
       out[i].core[k] = o;
       p.out = o;
       c.push_back(p);
@@ -746,14 +754,15 @@ void qtt_concat_batch(qtt_ctx* ctx, const std::vector<std::vector<std::pair<doub
 
 View qtt_kron(qtt_ctx* ctx, const View& a, const View& b) {
   if (a.n != b.n) QTT_THROW(QTT_SHAPE_MISMATCH, "product operands differ in length");
+  const int d = ctx->d;
   View o;
   o.n = a.n;
   o.r.resize(a.n + 1);
   o.core.resize(a.n);
   for (int k = 0; k <= a.n; ++k) o.r[k] = a.r[k] * b.r[k];
   for (int k = 0; k < a.n; ++k) {
-    double* out = ctx->arena.tmp((size_t)o.r[k] * 4 * o.r[k + 1]);
-    KronProb p{a.core[k], b.core[k], out, a.r[k], a.r[k + 1], b.r[k], b.r[k + 1]};
+    double* out = ctx->arena.tmp((size_t)o.r[k] * d * o.r[k + 1]);
+    KronProb p{a.core[k], b.core[k], out, a.r[k], a.r[k + 1], b.r[k], b.r[k + 1], d};
     QTT_CU(qtt_launch_kron(&p, 1, ctx->stream));
     o.core[k] = out;
   }
@@ -762,29 +771,33 @@ View qtt_kron(qtt_ctx* ctx, const View& a, const View& b) {
 
 // ------------------------------------------------------------------------------------------ boundary
 void qtt_to_dense_view(qtt_ctx* ctx, const View& v, double* dense_dev_out) {
+  const int d = ctx->d, ndim = d == 8 ? 3 : 2;
   const int n = v.n;
+  if (ndim * n > 30) QTT_THROW(QTT_CAPACITY, "grid too large for a dense array");
   const double* T = v.core[0];  // 4 x r_1
-  i64 rows = 4;
+  i64 rows = d;
   std::vector<GemmProb> g;
   for (int k = 1; k < n; ++k) {
-    double* Tn = ctx->arena.tmp((size_t)rows * 4 * v.r[k + 1]);
-    g.push_back(gemm_nn(T, v.r[k], v.core[k], 4 * (i64)v.r[k + 1], Tn, 4 * (i64)v.r[k + 1], (int)rows, 4 * v.r[k + 1],
+    double* Tn = ctx->arena.tmp((size_t)rows * d * v.r[k + 1]);
+    g.push_back(gemm_nn(T, v.r[k], v.core[k], d * (i64)v.r[k + 1], Tn, d * (i64)v.r[k + 1], (int)rows, d * v.r[k + 1],
                         v.r[k]));
     run_gemms(ctx, g);
     T = Tn;
-    rows *= 4;
+    rows *= d;
   }
-  QTT_CU(qtt_launch_interleave(T, dense_dev_out, n, 1, ctx->stream));
+  QTT_CU(qtt_launch_interleave(T, dense_dev_out, n, ndim, 1, ctx->stream));
 }
 
 void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, double eps, OutMps& out) {
+  const int d = ctx->d, ndim = d == 8 ? 3 : 2;
   const int n = nbits;
-  const i64 total = 1ll << (2 * n);
+  if (ndim * n > 30) QTT_THROW(QTT_CAPACITY, "grid too large for a dense array");
+  const i64 total = 1ll << (ndim * n);
   double* carry = ctx->arena.tmp((size_t)total);
-  QTT_CU(qtt_launch_interleave(dense_dev, carry, n, 0, ctx->stream));
+  QTT_CU(qtt_launch_interleave(dense_dev, carry, n, ndim, 0, ctx->stream));
   out.r.assign(n + 1, 1);
   if (n == 1) {
-    QTT_CU(qtt_launch_copy2d(carry, 1, 4, 4, out.core[0], 4, ctx->stream));
+    QTT_CU(qtt_launch_copy2d(carry, 1, d, d, out.core[0], d, ctx->stream));
     return;
   }
   int rc = 1;
@@ -792,9 +805,9 @@ void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, d
   int* rank_dev = reinterpret_cast<int*>(ctx->arena.tmp(1));
   std::vector<GemmProb> g;
   for (int k = n - 1; k >= 1; --k) {
-    // unfolding M: 4^k x (4 rc)
-    const i64 rows = 1ll << (2 * k);
-    const int q = 4 * rc;
+    // unfolding M: d^k x (d rc)
+    const i64 rows = 1ll << (ndim * k);
+    const int q = d * rc;
     if (rows > 2147483647ll / std::max(q, 1)) QTT_THROW(QTT_CAPACITY, "grid too large");
     std::vector<SvdJob> svd;
     SvdJob j;
@@ -840,22 +853,23 @@ void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, d
     rc = rn;
     out.r[k] = rn;
   }
-  QTT_CU(qtt_launch_copy2d(carry, 4, rc, rc, out.core[0], rc, ctx->stream));
+  QTT_CU(qtt_launch_copy2d(carry, d, rc, rc, out.core[0], rc, ctx->stream));
 }
 
 double* qtt_dot_view(qtt_ctx* ctx, const View& a, const View& b) {
+  const int d = ctx->d;
   if (a.n != b.n) QTT_THROW(QTT_SHAPE_MISMATCH, "operands differ in length");
   const double* E = ctx->ones;  // ra x rb
   std::vector<GemmProb> g;
   for (int k = 0; k < a.n; ++k) {
     const int ra = a.r[k], rb = b.r[k], a2 = a.r[k + 1], b2 = b.r[k + 1];
     // G[b,(w,a')] = sum_a E[a,b] A[a,(w,a')]
-    double* G = ctx->arena.tmp((size_t)rb * 4 * a2);
-    g.push_back(gemm_tn(E, rb, a.core[k], 4 * (i64)a2, G, 4 * (i64)a2, rb, 4 * a2, ra));
+    double* G = ctx->arena.tmp((size_t)rb * d * a2);
+    g.push_back(gemm_tn(E, rb, a.core[k], d * (i64)a2, G, d * (i64)a2, rb, d * a2, ra));
     run_gemms(ctx, g);
     // E'[a',b'] = sum_{(b,w)} G[(b,w),a'] B[(b,w),b']
     double* En = ctx->arena.tmp((size_t)a2 * b2);
-    g.push_back(gemm_tn(G, a2, b.core[k], b2, En, b2, a2, b2, 4 * rb));
+    g.push_back(gemm_tn(G, a2, b.core[k], b2, En, b2, a2, b2, d * rb));
     run_gemms(ctx, g);
     E = En;
   }
