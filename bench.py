@@ -672,11 +672,28 @@ def three_d_bench(args):
     f = rhs()
     fam = Q.qtt_ctx_profile_report(ctx)
     Q.qtt_ctx_profile(ctx, False)
+    # whole RK4 steps through the library's own 3D step (qtt_rk4_step3: four right-hand sides, stage and final sums)
+    dt = 0.1 * dx
+    v = [Q.qtt_mps_clone(ctx, x) for x in u]
+    step_ms = []
+    for rep in range(args.warmup + max(args.steps, 1)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctx.synchronize()
+        l0 = Q.qtt_ctx_launch_count(ctx)
+        e0.record(ctx.stream)
+        Q.qtt_rk4_step3(ctx, v, Dj, Lap, Re, dt, chi)
+        e1.record(ctx.stream)
+        ctx.synchronize()
+        if rep >= args.warmup:
+            step_ms.append(e0.elapsed_time(e1))
+        step_launches = Q.qtt_ctx_launch_count(ctx) - l0
     sweeps, hits = Q.qtt_ctx_jacobi_stats(ctx)
     ms = float(np.median(times))
     g = fam["gemm"]
     line = {"metric": "3D Burgers right-hand sides/s at 2^%d^3, d=8, chi=%d fp64" % (n, chi), "value": 1e3 / ms, "unit": "rhs/s",
-            "ms_per_rhs": ms, "n_gpus": 1, "steps": len(times), "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+            "ms_per_rhs": ms, "rk4_step3": {"ms_per_step": float(np.median(step_ms)), "steps_per_s": 1e3 / float(np.median(step_ms)),
+                                            "dt": dt, "gpu_launches_per_step": int(step_launches),
+                                            "norms_after": [Q.qtt_mps_norm(ctx, x) for x in v]}, "n_gpus": 1, "steps": len(times), "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "Taylor-Green vortex + 1e-3 N(0,1) on a 2^%d cube (%d sites, d=8), chi_max=%d, chi_work=%d, "
                                    "Re=%g: 12 apply+round, 9 zip-ups, 3 four-term sums, batched per level" % (n, n, chi, 2 * chi, Re),
                        "timing": "CUDA events on the context's stream around the eagerly launched composition, median"},

@@ -78,7 +78,7 @@ qtt_status qtt_ctx_set_chi_work(qtt_ctx* ctx, int chi_work);
  * bond 7; qtt_apply_mpo, qtt_hadamard, qtt_axpy, qtt_round / qtt_round_batch / qtt_round_ex (zip-up included), qtt_mps_dot /
  * norm / schmidt / fidelity / chi_eps / clone / get_core run the same kernels on d r-row unfoldings.  qtt_rk4_step,
  * qtt_variational_*, qtt_tke_spectrum and the sketched product compression are built for two velocity components on a 2D
- * grid and return QTT_INVALID_ARG when d = 8 (a 3D right-hand side is composed from the calls above).
+ * grid and return QTT_INVALID_ARG when d = 8 (the 3D time step is qtt_rk4_step3).
  * Errors: QTT_INVALID_ARG for d outside {4, 8}, or for a switch while MPS / MPO handles of the context are alive. */
 qtt_status qtt_ctx_set_phys_dim(qtt_ctx* ctx, int d);
 int qtt_ctx_phys_dim(const qtt_ctx* ctx); /* 4 or 8; 0 for a NULL context */
@@ -176,6 +176,14 @@ qtt_status qtt_round_batch(qtt_ctx* ctx, int batch, qtt_mps* const* xs, int chi_
  * one rounding after every apply, product and sum (readings 4, 5, 7, 10). */
 qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, const qtt_mpo* Dy, const qtt_mpo* Lap,
                         double Re, double dt, int chi_max, double eps);
+/* The same step for three velocity components on a 3D grid (reading 26; needs
+ * qtt_ctx_set_phys_dim(ctx, 8)): u = (u_1, u_2, u_3) in place, D = (D_x, D_y, D_z),
+ * f_i = -sum_{j=1..3} u_j (.) D_j u_i + (1/Re) Lap u_i, roundings as above: per right-hand side one batch of 12 apply + round,
+ * one of 9 zip-ups, one of 3 four-term sums; stage and final combinations as in qtt_rk4_step.  Launches are issued eagerly
+ * (no CUDA graph); eps > 0 synchronises once per bond.  Errors: QTT_INVALID_ARG for NULL arguments, a context of physical
+ * dimension 4, or the sketched product compression; QTT_SHAPE_MISMATCH for operands of different length or n < 2. */
+qtt_status qtt_rk4_step3(qtt_ctx* ctx, qtt_mps* const u[3], const qtt_mpo* const D[3], const qtt_mpo* Lap, double Re, double dt,
+                         int chi_max, double eps);
 
 /* Inspection. */
 int qtt_mps_num_sites(const qtt_mps* x);

@@ -38,6 +38,7 @@ PROTOTYPES = {
     "qtt_ctx_set_convection": (C.c_int, [_P, C.c_int]),
     "qtt_ctx_set_phys_dim": (C.c_int, [_P, C.c_int]),
     "qtt_ctx_phys_dim": (C.c_int, [_P]),
+    "qtt_rk4_step3": (C.c_int, [_P, _PP, _PP, _P, C.c_double, C.c_double, C.c_int, C.c_double]),
     "qtt_ctx_set_product_compression": (C.c_int, [_P, C.c_int, C.c_ulonglong]),
     "qtt_ctx_jacobi_stats": (C.c_int, [_P, _IP, _IP]),
     "qtt_ctx_launch_count": (C.c_longlong, [_P]),

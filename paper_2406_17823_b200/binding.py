@@ -234,6 +234,16 @@ def qtt_rk4_step(ctx: Context, u: Sequence[Mps], Dx: Mpo, Dy: Mpo, Lap: Mpo, Re:
     ctx.check(ctx.lib.qtt_rk4_step(ctx.h, arr, Dx.h, Dy.h, Lap.h, float(Re), float(dt), int(chi_max), float(eps)))
 
 
+def qtt_rk4_step3(ctx: Context, u: Sequence[Mps], D: Sequence[Mpo], Lap: Mpo, Re: float, dt: float, chi_max: int,
+                  eps: float = 0.0) -> None:
+    """One RK4 step of the three-component Burgers equations in a context of physical dimension 8 (in place)."""
+    if len(u) != 3 or len(D) != 3:
+        raise ValueError("three components and three derivative MPOs")
+    ua = (C.c_void_p * 3)(u[0].h, u[1].h, u[2].h)
+    da = (C.c_void_p * 3)(D[0].h, D[1].h, D[2].h)
+    ctx.check(ctx.lib.qtt_rk4_step3(ctx.h, ua, da, Lap.h, float(Re), float(dt), int(chi_max), float(eps)))
+
+
 def qtt_variational_cost(ctx: Context, v: Sequence[Mps], a: Sequence[Mps], B: Sequence[Mps], D1: Mpo, D2: Mpo, h: float,
                          mu: float) -> float:
     """Theta of PAPER.md Eq. B6."""

@@ -694,6 +694,47 @@ qtt_status qtt_round_ex(qtt_ctx* ctx, qtt_mps* x, int chi_max, double eps, int c
 }
 
 // ------------------------------------------------------------------------------------------ RK4
+qtt_status qtt_rk4_step3(qtt_ctx* ctx, qtt_mps* const u[3], const qtt_mpo* const D[3], const qtt_mpo* Lap, double Re, double dt,
+                         int chi_max, double eps) {
+  if (!ctx || !u || !D || !Lap || chi_max < 1 || eps < 0.0 || !(Re > 0.0)) return QTT_INVALID_ARG;
+  for (int i = 0; i < 3; ++i)
+    if (!u[i] || !D[i]) return QTT_INVALID_ARG;
+  QTT_API_BEGIN
+  set_device(ctx);
+  if (ctx->d != 8) QTT_THROW(QTT_INVALID_ARG, "qtt_rk4_step3 needs the 3D encoding (qtt_ctx_set_phys_dim(ctx, 8))");
+  if (ctx->sketch) QTT_THROW(QTT_INVALID_ARG, "the sketched product compression is built for physical dimension 4 only");
+  const int n = u[0]->body->n;
+  for (int i = 0; i < 3; ++i)
+    if (u[i]->body->n != n || D[i]->data->n != n) QTT_THROW(QTT_SHAPE_MISMATCH, "rk4_step3 operands differ in length");
+  if (Lap->data->n != n || n < 2) QTT_THROW(QTT_SHAPE_MISMATCH, "rk4_step3 operands differ in length (or fewer than two sites)");
+  const int cw = ctx->chi_work > 0 ? ctx->chi_work : 2 * chi_max;
+  ArenaScope scope(ctx);
+  View uv[3] = {materialize(ctx, u[0]->body), materialize(ctx, u[1]->body), materialize(ctx, u[2]->body)};
+  const MpoData* Dj[3] = {D[0]->data, D[1]->data, D[2]->data};
+  // capacity bonds of the result: min(chi, 8^k, 8^(n-k)) (the sweep fills in the actual ones)
+  std::vector<int> caps(n + 1, 1);
+  for (int k = 1; k < n; ++k) {
+    const int l = std::min(k, n - k);
+    caps[k] = (int)std::min<long long>(chi_max, l >= 10 ? (1ll << 30) : (1ll << (3 * l)));
+  }
+  Body* fresh[3] = {nullptr, nullptr, nullptr};
+  try {
+    for (int i = 0; i < 3; ++i) fresh[i] = body_new_dense(ctx, caps);
+    OutMps out[3] = {out_of_body(fresh[0]), out_of_body(fresh[1]), out_of_body(fresh[2])};
+    qtt_rk4_eager3(ctx, uv, Dj, Lap->data, Re, dt, chi_max, eps, cw, out);
+    for (int i = 0; i < 3; ++i) body_set_bonds(fresh[i], out[i].r);
+  } catch (...) {
+    for (int i = 0; i < 3; ++i) body_release(fresh[i]);
+    throw;
+  }
+  for (int i = 0; i < 3; ++i) {
+    body_release(u[i]->body);
+    u[i]->body = fresh[i];
+  }
+  if (eps > 0.0) check_numeric(ctx);
+  QTT_API_END(ctx)
+}
+
 qtt_status qtt_rk4_step(qtt_ctx* ctx, qtt_mps* const u[2], const qtt_mpo* Dx, const qtt_mpo* Dy, const qtt_mpo* Lap,
                         double Re, double dt, int chi_max, double eps) {
   if (!ctx || !u || !u[0] || !u[1] || !Dx || !Dy || !Lap || chi_max < 1 || eps < 0.0 || !(Re > 0.0))

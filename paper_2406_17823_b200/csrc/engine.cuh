@@ -145,6 +145,9 @@ View qtt_kron(qtt_ctx* ctx, const View& a, const View& b);
 void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
                    double dt, int chi, double eps, int chi_work, int skew, OutMps out[2]);
 
+void qtt_rk4_eager3(qtt_ctx* ctx, const View u[3], const MpoData* const Dj[3], const MpoData* Lap, double Re, double dt,
+                    int chi, double eps, int chi_work, OutMps out[3]);
+
 void qtt_to_dense_view(qtt_ctx* ctx, const View& v, double* dense_dev_out);
 void qtt_from_dense(qtt_ctx* ctx, const double* dense_dev, int nbits, int chi, double eps, OutMps& out);
 double* qtt_dot_view(qtt_ctx* ctx, const View& a, const View& b);  // device scalar in tmp

@@ -886,7 +886,7 @@ std::vector<OutMps> alloc_outs_keep(qtt_ctx* ctx, const std::vector<std::vector<
     out[i].n = n;
     out[i].rcap = caps[i];
     out[i].core.resize(n);
-    for (int k = 0; k < n; ++k) out[i].core[k] = ctx->arena.keep((size_t)caps[i][k] * 4 * caps[i][k + 1]);
+    for (int k = 0; k < n; ++k) out[i].core[k] = ctx->arena.keep((size_t)caps[i][k] * ctx->d * caps[i][k + 1]);
   }
   return out;
 }
@@ -1051,7 +1051,99 @@ void lincomb_round(qtt_ctx* ctx, const std::vector<std::vector<std::pair<double,
   ctx->arena.hi = mark;
 }
 
+// Three components on a 3D grid (d = 8; reading 26): f_i = -sum_j u_j (.) D_j u_i + (1/Re) Lap u_i (oracle rhs3),
+// three batched levels: 12 applies + roundings, 9 zip-ups, 3 four-term sums.
+void rhs3(qtt_ctx* ctx, const View u[3], const MpoData* const Dj[3], const MpoData* Lap, double Re, int chi, double eps,
+          int chi_work, View f[3]) {
+  const int d = ctx->d;
+  std::vector<View> g(12);  // g[4 i + j] = round(D_j u_i), j < 3;  g[4 i + 3] = round(Lap u_i)
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<const MpoData*> W;
+    std::vector<View> X;
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 4; ++j) {
+        W.push_back(j < 3 ? Dj[j] : Lap);
+        X.push_back(u[i]);
+      }
+    std::vector<View> ex;
+    qtt_expand_apply_batch(ctx, W, X, ex);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : ex) caps.push_back(qtt_round_caps(e.r, chi, d));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, ex, chi, eps, out);
+    for (int i = 0; i < 12; ++i) g[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+  std::vector<View> c(9);  // c[3 i + j] = round(u_j (.) g_ij)
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<View> A, B;
+    std::vector<std::vector<int>> caps;
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) {
+        A.push_back(u[j]);
+        B.push_back(g[4 * i + j]);
+        std::vector<int> rw, ro;
+        qtt_zip_caps(A.back().r, B.back().r, chi, chi_work, rw, ro, d);
+        caps.push_back(ro);
+      }
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_product_batch(ctx, A, B, chi, eps, chi_work, out);
+    for (int i = 0; i < 9; ++i) c[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+  {
+    const size_t mark = ctx->arena.hi;
+    std::vector<std::vector<std::pair<double, View>>> terms(3);
+    for (int i = 0; i < 3; ++i)
+      terms[i] = {{-1.0, c[3 * i]}, {-1.0, c[3 * i + 1]}, {-1.0, c[3 * i + 2]}, {1.0 / Re, g[4 * i + 3]}};
+    std::vector<View> s;
+    qtt_concat_batch(ctx, terms, s);
+    std::vector<std::vector<int>> caps;
+    for (auto& e : s) caps.push_back(qtt_round_caps(e.r, chi, d));
+    std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
+    qtt_round_dense_batch(ctx, s, chi, eps, out);
+    for (int i = 0; i < 3; ++i) f[i] = view_of(out[i]);
+    ctx->arena.hi = mark;
+  }
+}
+
 }  // namespace
+
+// Classical RK4 (Eq. 11) on three components in the d = 8 encoding (oracle rk4_step3); eager launches.
+void qtt_rk4_eager3(qtt_ctx* ctx, const View u[3], const MpoData* const Dj[3], const MpoData* Lap, double Re, double dt,
+                    int chi, double eps, int chi_work, OutMps out[3]) {
+  const int d = ctx->d;
+  View k1[3], k2[3], k3[3], k4[3], us[3];
+  auto stage = [&](const View kk[3], double h, View dst[3]) {
+    std::vector<std::vector<std::pair<double, View>>> terms(3);
+    std::vector<std::vector<int>> caps;
+    for (int i = 0; i < 3; ++i) {
+      terms[i] = {{1.0, u[i]}, {h, kk[i]}};
+      std::vector<int> rs(u[i].r.size());
+      for (size_t b = 0; b < rs.size(); ++b) rs[b] = u[i].r[b] + kk[i].r[b];
+      rs.front() = rs.back() = 1;
+      caps.push_back(qtt_round_caps(rs, chi, d));
+    }
+    std::vector<OutMps> o = alloc_outs_keep(ctx, caps);
+    lincomb_round(ctx, terms, chi, eps, o);
+    for (int i = 0; i < 3; ++i) dst[i] = view_of(o[i]);
+  };
+  rhs3(ctx, u, Dj, Lap, Re, chi, eps, chi_work, k1);
+  stage(k1, dt / 2, us);
+  rhs3(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k2);
+  stage(k2, dt / 2, us);
+  rhs3(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k3);
+  stage(k3, dt, us);
+  rhs3(ctx, us, Dj, Lap, Re, chi, eps, chi_work, k4);
+  std::vector<std::vector<std::pair<double, View>>> terms(3);
+  for (int i = 0; i < 3; ++i)
+    terms[i] = {{1.0, u[i]}, {dt / 6, k1[i]}, {dt / 3, k2[i]}, {dt / 3, k3[i]}, {dt / 6, k4[i]}};
+  std::vector<OutMps> o{out[0], out[1], out[2]};
+  lincomb_round(ctx, terms, chi, eps, o);
+  for (int i = 0; i < 3; ++i) out[i] = o[i];
+}
 
 void qtt_rk4_eager(qtt_ctx* ctx, const View u[2], const MpoData* Dx, const MpoData* Dy, const MpoData* Lap, double Re,
                    double dt, int chi, double eps, int chi_work, int skew, OutMps out[2]) {

@@ -236,6 +236,46 @@ def test_rk4_step3_from_primitives_matches_oracle(Q, ctx):
         assert rel(ref, O3.to_dense3(Uo[i])) > 1e-6
 
 
+@pytest.mark.parametrize("n,chi,eps", [(3, 64, 0.0), (4, 12, 0.0), (4, 10, 1e-6), (5, 16, 0.0)])
+def test_rk4_step3_matches_oracle(Q, ctx, n, chi, eps):
+    """qtt_rk4_step3 against oracle rk4_step3 (n = 3 with chi = 64: nothing truncates, so also == the dense RK4 the oracle is
+    pinned to); two steps in a row at n = 4."""
+    import torch
+    Re, dt = 100.0, 2e-3
+    dx = 1.0 / (1 << n)
+    u0 = list(I.taylor_green_3d(n, seed=n, noise=1e-3))
+    Uo = [O3.from_dense3(f, chi) for f in u0]
+    Djo = [O3.mpo_d3(n, j, dx) for j in (1, 2, 3)]
+    Lapo = O3.mpo_laplacian3(n, dx)
+    Dj = [Q.qtt_mpo_central_difference(ctx, n, j, dx) for j in (1, 2, 3)]
+    Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
+    u = [Q.qtt_mps_from_dense(ctx, torch.from_numpy(f).cuda(), chi) for f in u0]
+    for step in range(2 if (n == 4 and eps == 0.0) else 1):
+        Uo = O3.rk4_step3(Uo, Djo, Lapo, Re, dt, chi, eps)
+        Q.qtt_rk4_step3(ctx, u, Dj, Lap, Re, dt, chi, eps)
+        for i in range(3):
+            if eps == 0.0:
+                assert Q.qtt_mps_bonds(u[i]) == O.bonds(Uo[i])
+            assert rel(gpu_dense(Q, ctx, u[i]), O3.to_dense3(Uo[i])) < (TOL if eps == 0.0 else 10 * eps)
+    assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+    if eps > 0.0:  # ranks by the eps rule: equal unless a singular value sits on the threshold (reading 17)
+        for i in range(3):
+            bg, bo = Q.qtt_mps_bonds(u[i]), O.bonds(Uo[i])
+            assert all(abs(a - b) <= 1 for a, b in zip(bg, bo))
+
+
+def test_rk4_step3_needs_a_3d_context(Q):
+    c = Q.Context(device=0, workspace_bytes=256 << 20)
+    try:
+        n, dx = 3, 1.0 / 8
+        a = [Q.qtt_mps_from_cores(c, I.random_cores(n, 4, seed=s)) for s in range(3)]
+        D = [Q.qtt_mpo_central_difference(c, n, 1 + (j % 2), dx) for j in range(3)]
+        with pytest.raises(Q.QttError):
+            Q.qtt_rk4_step3(c, a, D, Q.qtt_mpo_laplacian(c, n, dx), 100.0, 1e-3, 4)
+    finally:
+        c.close()
+
+
 def test_2d_only_calls_refuse_a_3d_context(Q, ctx):
     n = 3
     dx = 1.0 / (1 << n)
