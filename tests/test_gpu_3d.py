@@ -276,6 +276,69 @@ def test_rk4_step3_needs_a_3d_context(Q):
         c.close()
 
 
+def test_edge_cases3(Q, ctx):
+    """One and two sites, a zero operand, bonds that already fit, chi = 1."""
+    # one site: rounding is a copy, the dense cube is the core
+    c1 = I.random_cores(1, 3, seed=4, d=8)
+    x = Q.qtt_mps_from_cores(ctx, c1)
+    Q.qtt_round(ctx, x, 2)
+    assert rel(gpu_dense(Q, ctx, x), O3.to_dense3(c1)) < 1e-15
+    assert abs(Q.qtt_mps_norm(ctx, x) - np.linalg.norm(c1[0])) < 1e-13
+    # two sites, chi = 1 and chi beyond the full rank
+    A = I.random_cores(2, 8, seed=5, d=8)
+    for chi in (1, 3, 100):
+        x = Q.qtt_mps_from_cores(ctx, A)
+        Q.qtt_round(ctx, x, chi)
+        want = O.round_mps(A, chi)
+        assert Q.qtt_mps_bonds(x) == O.bonds(want)
+        assert rel(gpu_dense(Q, ctx, x), O3.to_dense3(want)) < TOL
+    # a zero operand stays zero through product, sum and rounding (no normalisation anywhere)
+    n = 3
+    Bc = I.random_cores(n, 4, seed=6, d=8)
+    Z = [np.zeros_like(c) for c in Bc]
+    b, z = Q.qtt_mps_from_cores(ctx, Bc), Q.qtt_mps_from_cores(ctx, Z)
+    p = Q.qtt_hadamard(ctx, b, z)
+    Q.qtt_round(ctx, p, 4)
+    assert np.all(gpu_dense(Q, ctx, p) == 0.0)
+    s = Q.qtt_mps_clone(ctx, b)
+    Q.qtt_axpy(ctx, 2.0, z, s)
+    Q.qtt_round(ctx, s, 4)
+    assert rel(gpu_dense(Q, ctx, s), O3.to_dense3(O.round_mps(Bc, 4))) < TOL
+    assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+
+
+def test_bench_launch_configuration_zipups3(Q, ctx):
+    """The launch configuration bench.py --three-d 6 --three-d-chi 32 times (64^3, chi = 32, chi_work = 64, a batch of nine
+    zip-ups of 512 x 1024 site matrices and a batch of twelve applies): products and applies of one right-hand side against
+    the oracle, operand by operand."""
+    n, chi = 6, 32
+    dx = 1.0 / (1 << n)
+    u0 = list(I.taylor_green_3d(n, seed=0, noise=1e-3))
+    Uo = [O3.from_dense3(f, chi) for f in u0]
+    u = [Q.qtt_mps_from_cores(ctx, x) for x in Uo]  # both sides start from the same host cores
+    Dj = [Q.qtt_mpo_central_difference(ctx, n, j, dx) for j in (1, 2, 3)]
+    Lap = Q.qtt_mpo_laplacian(ctx, n, dx)
+    Djo = [O3.mpo_d3(n, j, dx) for j in (1, 2, 3)]
+    g = [[Q.qtt_apply_mpo(ctx, Dj[j], u[i]) for j in range(3)] for i in range(3)]
+    lap = [Q.qtt_apply_mpo(ctx, Lap, u[i]) for i in range(3)]
+    Q.qtt_round_batch(ctx, [x for row in g for x in row] + lap, chi)
+    go = [[O.round_mps(O.apply_mpo(Djo[j], Uo[i]), chi) for j in range(3)] for i in range(3)]
+    for i in range(3):
+        for j in range(3):
+            assert Q.qtt_mps_bonds(g[i][j]) == O.bonds(go[i][j])
+            assert O.diff_norm([np.ascontiguousarray(c) for c in Q.qtt_mps_get_cores(ctx, g[i][j])], go[i][j]) < TOL * O.norm(go[i][j])
+    lo = O.round_mps(O.apply_mpo(O3.mpo_laplacian3(n, dx), Uo[0]), chi)
+    assert O.diff_norm([np.ascontiguousarray(c) for c in Q.qtt_mps_get_cores(ctx, lap[0])], lo) < TOL * O.norm(lo)
+    c = [[Q.qtt_hadamard(ctx, u[j], g[i][j]) for j in range(3)] for i in range(3)]
+    Q.qtt_round_batch(ctx, [x for row in c for x in row], chi)
+    for i, j in ((0, 0), (0, 1), (1, 2), (2, 0)):  # sampled operands of the batch of nine (the oracle needs ~2 s each)
+        want = O.round_product(Uo[j], go[i][j], chi)
+        got = [np.ascontiguousarray(x) for x in Q.qtt_mps_get_cores(ctx, c[i][j])]
+        assert Q.qtt_mps_bonds(c[i][j]) == O.bonds(want)
+        assert O.diff_norm(got, want) < TOL * max(O.norm(want), 1e-300)
+    assert Q.qtt_ctx_jacobi_stats(ctx)[1] == 0
+
+
 def test_2d_only_calls_refuse_a_3d_context(Q, ctx):
     n = 3
     dx = 1.0 / (1 << n)
