@@ -1077,9 +1077,9 @@ void rhs3(qtt_ctx* ctx, const View u[3], const MpoData* const Dj[3], const MpoDa
   }
   std::vector<View> c(9);  // c[3 i + j] = round(u_j (.) g_ij)
   {
-    const size_t mark = ctx->arena.hi;
     std::vector<View> A, B;
     std::vector<std::vector<int>> caps;
+    size_t side_need = (size_t)64 << 20;
     for (int i = 0; i < 3; ++i)
       for (int j = 0; j < 3; ++j) {
         A.push_back(u[j]);
@@ -1087,11 +1087,43 @@ void rhs3(qtt_ctx* ctx, const View u[3], const MpoData* const Dj[3], const MpoDa
         std::vector<int> rw, ro;
         qtt_zip_caps(A.back().r, B.back().r, chi, chi_work, rw, ro, d);
         caps.push_back(ro);
+        if (A.size() > 5) {  // scratch of one zip-up: carries, X, T, its copy, the LQ reflectors, factors
+          size_t mx = 1;
+          for (int l = 0; l + 1 < (int)rw.size() - 1; ++l)
+            mx = std::max(mx, (size_t)d * rw[l] * A.back().r[l + 1] * B.back().r[l + 1]);
+          side_need += 8 * sizeof(double) * mx;
+        }
       }
     std::vector<OutMps> out = alloc_outs_keep(ctx, caps);
-    qtt_round_product_batch(ctx, A, B, chi, eps, chi_work, out);
-    for (int i = 0; i < 9; ++i) c[i] = view_of(out[i]);
-    ctx->arena.hi = mark;
+    // Only seven 16-CTA clusters are co-resident on the GPU (profiles/r2_three_d.md): nine factors in one launch run as
+    // 7 + 2.  Two independent chains (five operands here, four on the side stream with its own scratch) share the seven
+    // slots instead, each starting a kernel as soon as the other one leaves room.  Measured (bench.py --three-d): 64^3, chi = 32:
+    // 240.0 -> 203.2 ms per step; 128^3, chi = 64, whose 1024-row factors take the L2-streamed Jacobi (one launch per tournament
+    // round, no clusters): 1168 -> 1502 ms -- so only where the factors are cluster-resident (d chi_work <= 512 rows).
+    const bool forked = ctx->side != nullptr && ctx->side_arena.size >= side_need && (long long)d * chi_work <= 512;
+    if (forked) {
+      std::vector<View> A1(A.begin(), A.begin() + 5), B1(B.begin(), B.begin() + 5), A2(A.begin() + 5, A.end()),
+          B2(B.begin() + 5, B.end());
+      std::vector<OutMps> o1(out.begin(), out.begin() + 5), o2(out.begin() + 5, out.end());
+      QTT_CU(cudaEventRecord(ctx->ev_fork, ctx->stream));
+      QTT_CU(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+      {
+        SideScope sc(ctx);
+        qtt_round_product_batch(ctx, A2, B2, chi, eps, chi_work, o2);
+        QTT_CU(cudaEventRecord(ctx->ev_join, ctx->stream));
+      }
+      const size_t mark = ctx->arena.hi;
+      qtt_round_product_batch(ctx, A1, B1, chi, eps, chi_work, o1);
+      ctx->arena.hi = mark;
+      QTT_CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+      for (int i = 0; i < 5; ++i) c[i] = view_of(o1[i]);
+      for (int i = 0; i < 4; ++i) c[5 + i] = view_of(o2[i]);
+    } else {
+      const size_t mark = ctx->arena.hi;
+      qtt_round_product_batch(ctx, A, B, chi, eps, chi_work, out);
+      for (int i = 0; i < 9; ++i) c[i] = view_of(out[i]);
+      ctx->arena.hi = mark;
+    }
   }
   {
     const size_t mark = ctx->arena.hi;
