@@ -702,6 +702,17 @@ def three_d_bench(args):
             "family_ms": {k: round(v["ms"], 3) for k, v in fam.items()},
             "gemm_tflops": g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12,
             "gemm_frac_of_dmma_peak": (g["work"] / max(g["ms"] * 1e-3, 1e-12) * 1e-12) / peaks["dmma"], "fp64_peaks_tflops": peaks}
+    # roofline of the dominant family and of the whole right-hand side: algorithmic flops as counted per launch by the library
+    # (the formulas of DESIGN.md section 6: nominal SVD / Householder / GEMM counts) over the measured times
+    flop_fams = ("gemm", "lq_panel", "lq_update", "rowjacobi", "qrcp")
+    dom = max(flop_fams, key=lambda k: fam[k]["ms"])
+    dpeak = peaks["dmma"] if dom in ("gemm", "lq_update") else peaks["dfma"]
+    dach = fam[dom]["work"] / max(fam[dom]["ms"] * 1e-3, 1e-12) * 1e-12
+    flops = float(sum(fam[k]["work"] for k in flop_fams))
+    line["roofline"] = {"kernel": dom + " family, summed over one right-hand side", "bound": "tensor" if dpeak == peaks["dmma"] else "alu",
+                        "achieved": dach, "peak": dpeak, "unit": "TFLOP/s", "frac": dach / dpeak, "traffic": None}
+    line["roofline_rhs"] = {"flops": flops, "achieved": flops / (ms * 1e-3) * 1e-12, "peak": peaks["dmma"], "unit": "TFLOP/s",
+                            "frac": flops / (ms * 1e-3) * 1e-12 / peaks["dmma"]}
     print(json.dumps(line), flush=True)
     return 0
 
